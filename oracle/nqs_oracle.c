@@ -1,0 +1,303 @@
+/*
+ * oracle/nqs_oracle.c -- float64 CPU oracle for the batched RBM local energy.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Nothing under paper_2108_03409_b200/ (the product) may include,
+ * link, import or call this file; only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs use it.  It shares no code, header, table or helper
+ * with the CUDA path.  Plain, slow, written to be checked against the paper by eye.
+ *
+ * What it computes (citations are /root/reference/PAPER.md line numbers):
+ *   log psi(s) = sum_i a_i s_i + sum_j log cosh(b_j + sum_i W_ji s_i)      Eq. 38, :385-390
+ *                (index reading Q1 of DESIGN.md: j hidden, i visible, W is [M,N])
+ *   E_loc(s)   = sum_s' <s|H|s'> psi(s') / psi(s)                           Eq. 4,  :63-68, :89
+ *   H          = sum_t c_t P_t,  P_t a product of at most two Pauli matrices on distinct
+ *                sites; its action on a basis configuration is the map of      Eq. 39, :418-426
+ *                s -> (s', <s|P_t|s'>) ("branch-free": one non-zero per row, :473).
+ *
+ * Inputs are the SAME BYTES the GPU gets (int8 spins, complex64 parameters); they are
+ * promoted exactly to double.  All arithmetic is double / double complex.
+ *
+ * Two modes:
+ *   definition mode  oracle_local_energy_definition(): Algorithm 1 lines 6-8 (:163-194,
+ *       :464-469) literally -- every term in list order, no grouping, s' built explicitly,
+ *       log psi(s') recomputed from scratch with log cosh = clog(ccosh(.)) from libm.
+ *       This is the parity authority.
+ *   fast mode        oracle_local_energy_fast(): same float64 arithmetic, but terms are grouped
+ *       by flip set and theta' = theta - 2 sum_{i in F} W_:,i s_i is used with differences of
+ *       a stable log cosh (formula F1 below).  Pinned to definition mode (pin P8) and used for
+ *       full-batch parity and as the timed CPU baseline.
+ *
+ * Parity pins: see tests/test_oracle_pins.py (P1 dense H brute force, P2 Eq. 2-3 identity,
+ * P3 zero parameters closed form, P4 product eigenstate, P5 singlet, P6 spin-flip symmetry,
+ * P7 Pfeuty closed form for the dense-H builder, P8 definition<->fast, P9 log cosh special
+ * cases).  No function here is "parity unpinned".
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef double complex cplx;
+
+enum { P_I = 0, P_X = 1, P_Y = 2, P_Z = 3 };
+
+/* complex64 (interleaved float re, im) element k -> double complex, exact promotion */
+static inline cplx c64(const float *p, int64_t k) { return (double)p[2 * k] + I * (double)p[2 * k + 1]; }
+
+/* ---------------------------------------------------------------------------------------
+ * log cosh
+ * ------------------------------------------------------------------------------------- */
+
+/* Definition: the principal complex logarithm of cosh z, straight from libm. */
+static inline cplx lncosh_def(cplx z) { return clog(ccosh(z)); }
+
+/* F1 (reading Q6): z = x + iy, sgn = sign(x) (+1 at 0), u = |x|, yt = sgn*y,
+ * q = exp(-2u), D = 1 + 2 q cos 2yt + q^2 = |1 + q e^{2 i yt}|^2.  Since cosh z = cosh(sgn z)
+ * = e^{u + i yt} (1 + q e^{-2 i yt}) / 2 ... written out:
+ *   Re = u - ln 2 + (1/2) log D,   Im = yt + atan2(-q sin 2yt, 1 + q cos 2yt).
+ * Never overflows.  Im is an unwrapped phase: equal to the principal value when |y| < pi/2,
+ * else it differs by a multiple of 2 pi. */
+static inline cplx lncosh_stable(cplx z) {
+    double x = creal(z), y = cimag(z);
+    double sgn = (x < 0.0) ? -1.0 : 1.0;
+    double u = fabs(x), yt = sgn * y;
+    double q = exp(-2.0 * u);
+    double c = cos(2.0 * yt), s = sin(2.0 * yt);
+    double D = 1.0 + 2.0 * q * c + q * q;
+    return (u - M_LN2 + 0.5 * log(D)) + I * (yt + atan2(-q * s, 1.0 + q * c));
+}
+
+/* exported pointwise for pin P9: mode 0 = definition, 1 = F1 */
+void oracle_lncosh(const double *z_re_im, int64_t n, int mode, double *out_re_im) {
+    for (int64_t k = 0; k < n; ++k) {
+        cplx z = z_re_im[2 * k] + I * z_re_im[2 * k + 1];
+        cplx r = mode ? lncosh_stable(z) : lncosh_def(z);
+        out_re_im[2 * k] = creal(r);
+        out_re_im[2 * k + 1] = cimag(r);
+    }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * log psi, Eq. 38
+ * ------------------------------------------------------------------------------------- */
+static cplx log_psi_one(const int8_t *s, int N, int M, const float *a, const float *b, const float *W,
+                        int stable) {
+    cplx acc = 0.0;
+    for (int i = 0; i < N; ++i) acc += c64(a, i) * (double)s[i];
+    for (int j = 0; j < M; ++j) {
+        cplx theta = c64(b, j);
+        for (int i = 0; i < N; ++i) theta += c64(W, (int64_t)j * N + i) * (double)s[i];
+        acc += stable ? lncosh_stable(theta) : lncosh_def(theta);
+    }
+    return acc;
+}
+
+/* spins [B,N] int8, a [N], b [M], W [M,N] complex64; out [B] complex128 (re, im doubles).
+ * mode 0: log cosh by definition; mode 1: F1. */
+void oracle_log_psi(const int8_t *spins, int64_t B, int N, int M, const float *a, const float *b,
+                    const float *W, int mode, double *out_logpsi) {
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < B; ++n) {
+        cplx lp = log_psi_one(spins + n * N, N, M, a, b, W, mode);
+        out_logpsi[2 * n] = creal(lp);
+        out_logpsi[2 * n + 1] = cimag(lp);
+    }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * matrix element of one Pauli on one site, row convention (reading Q3):
+ *   <s|X_k|s'> = 1,  <s|Y_k|s'> = -i s_k  (s' = s with site k flipped),
+ *   <s|Z_k|s>  = s_k, identity = 1.   s_k is the spin of the ROW configuration s.
+ * ------------------------------------------------------------------------------------- */
+static inline cplx pauli_factor(int p, int sk, int *flips) {
+    switch (p) {
+    case P_X: *flips = 1; return 1.0;
+    case P_Y: *flips = 1; return -I * (double)sk;
+    case P_Z: *flips = 0; return (double)sk;
+    default:  *flips = 0; return 1.0;
+    }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * definition mode: Eq. 4 + Eq. 39 + Eq. 38, term by term (Algorithm 1 lines 6-8)
+ * ------------------------------------------------------------------------------------- */
+void oracle_local_energy_definition(const int8_t *spins, int64_t B, int N, int M, const float *a,
+                                    const float *b, const float *W, int T, const int32_t *sites,
+                                    const uint8_t *paulis, const float *coeffs, double *out_eloc,
+                                    double *out_logpsi) {
+#pragma omp parallel
+    {
+        int8_t *sp = (int8_t *)malloc((size_t)N);
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t n = 0; n < B; ++n) {
+            const int8_t *s = spins + n * N;
+            cplx lp = log_psi_one(s, N, M, a, b, W, 0);
+            cplx E = 0.0;
+            for (int t = 0; t < T; ++t) {
+                cplx m = c64(coeffs, t);
+                memcpy(sp, s, (size_t)N);
+                for (int k = 0; k < 2; ++k) {
+                    int site = sites[2 * t + k];
+                    if (site < 0) continue; /* unused slot */
+                    int flips = 0;
+                    m *= pauli_factor(paulis[2 * t + k], s[site], &flips);
+                    if (flips) sp[site] = (int8_t)(-sp[site]);
+                }
+                if (m == 0.0) continue; /* "non-zero matrix elements", :458 (reading Q5) */
+                cplx lpp = log_psi_one(sp, N, M, a, b, W, 0);
+                E += m * cexp(lpp - lp);
+            }
+            out_eloc[2 * n] = creal(E);
+            out_eloc[2 * n + 1] = cimag(E);
+            if (out_logpsi) {
+                out_logpsi[2 * n] = creal(lp);
+                out_logpsi[2 * n + 1] = cimag(lp);
+            }
+        }
+        free(sp);
+    }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * fast mode: flip grouping + low-rank theta update, same float64 arithmetic
+ * ------------------------------------------------------------------------------------- */
+typedef struct { int f0, f1; int first, count; } group_t; /* flip set {f0,f1}, f1=-1 if single, f0=-1 diag */
+
+static int key_of(const int32_t *sites, const uint8_t *paulis, int t, int *f0, int *f1) {
+    int f[2], nf = 0;
+    for (int k = 0; k < 2; ++k) {
+        int site = sites[2 * t + k];
+        int p = paulis[2 * t + k];
+        if (site >= 0 && (p == P_X || p == P_Y)) f[nf++] = site;
+    }
+    if (nf == 2 && f[0] > f[1]) { int tmp = f[0]; f[0] = f[1]; f[1] = tmp; }
+    *f0 = nf > 0 ? f[0] : -1;
+    *f1 = nf > 1 ? f[1] : -1;
+    return nf;
+}
+
+void oracle_local_energy_fast(const int8_t *spins, int64_t B, int N, int M, const float *a,
+                              const float *b, const float *W, int T, const int32_t *sites,
+                              const uint8_t *paulis, const float *coeffs, double *out_eloc,
+                              double *out_logpsi) {
+    /* group terms by flip set: order[] lists term ids group by group (O(T^2), T is small) */
+    int *order = (int *)malloc(sizeof(int) * (size_t)(T > 0 ? T : 1));
+    group_t *groups = (group_t *)malloc(sizeof(group_t) * (size_t)(T > 0 ? T : 1));
+    char *done = (char *)calloc((size_t)(T > 0 ? T : 1), 1);
+    int G = 0, pos = 0;
+    for (int t = 0; t < T; ++t) {
+        if (done[t]) continue;
+        int f0, f1;
+        key_of(sites, paulis, t, &f0, &f1);
+        groups[G].f0 = f0; groups[G].f1 = f1; groups[G].first = pos; groups[G].count = 0;
+        for (int u = t; u < T; ++u) {
+            int g0, g1;
+            if (done[u]) continue;
+            key_of(sites, paulis, u, &g0, &g1);
+            if (g0 == f0 && g1 == f1) { order[pos++] = u; done[u] = 1; groups[G].count++; }
+        }
+        ++G;
+    }
+
+#pragma omp parallel
+    {
+        cplx *theta = (cplx *)malloc(sizeof(cplx) * (size_t)(M > 0 ? M : 1));
+        cplx *L = (cplx *)malloc(sizeof(cplx) * (size_t)(M > 0 ? M : 1));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t n = 0; n < B; ++n) {
+            const int8_t *s = spins + n * N;
+            cplx lp = 0.0;
+            for (int i = 0; i < N; ++i) lp += c64(a, i) * (double)s[i];
+            for (int j = 0; j < M; ++j) {
+                cplx th = c64(b, j);
+                for (int i = 0; i < N; ++i) th += c64(W, (int64_t)j * N + i) * (double)s[i];
+                theta[j] = th;
+                L[j] = lncosh_stable(th);
+                lp += L[j];
+            }
+            cplx E = 0.0;
+            for (int g = 0; g < G; ++g) {
+                /* summed matrix element of the group's terms (they all reach the same s') */
+                cplx m = 0.0;
+                for (int q = 0; q < groups[g].count; ++q) {
+                    int t = order[groups[g].first + q];
+                    cplx mt = c64(coeffs, t);
+                    for (int k = 0; k < 2; ++k) {
+                        int site = sites[2 * t + k];
+                        if (site < 0) continue;
+                        int flips;
+                        mt *= pauli_factor(paulis[2 * t + k], s[site], &flips);
+                    }
+                    m += mt;
+                }
+                if (groups[g].f0 < 0) { E += m; continue; } /* diagonal: s' = s, ratio 1 */
+                if (m == 0.0) continue;
+                int f0 = groups[g].f0, f1 = groups[g].f1;
+                cplx dlog = -2.0 * c64(a, f0) * (double)s[f0];
+                if (f1 >= 0) dlog += -2.0 * c64(a, f1) * (double)s[f1];
+                for (int j = 0; j < M; ++j) {
+                    cplx thp = theta[j] - 2.0 * c64(W, (int64_t)j * N + f0) * (double)s[f0];
+                    if (f1 >= 0) thp -= 2.0 * c64(W, (int64_t)j * N + f1) * (double)s[f1];
+                    dlog += lncosh_stable(thp) - L[j];
+                }
+                E += m * cexp(dlog);
+            }
+            out_eloc[2 * n] = creal(E);
+            out_eloc[2 * n + 1] = cimag(E);
+            if (out_logpsi) {
+                out_logpsi[2 * n] = creal(lp);
+                out_logpsi[2 * n + 1] = cimag(lp);
+            }
+        }
+        free(theta);
+        free(L);
+    }
+    free(order);
+    free(groups);
+    free(done);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Eq. 39 as data: connected configurations and matrix elements, term by term (no grouping).
+ * sprime [B,T,N] int8, mel [B,T] complex128.  Used to check the GPU enumerator.
+ * ------------------------------------------------------------------------------------- */
+void oracle_connected(const int8_t *spins, int64_t B, int N, int T, const int32_t *sites,
+                      const uint8_t *paulis, const float *coeffs, int8_t *sprime, double *mel) {
+    for (int64_t n = 0; n < B; ++n) {
+        const int8_t *s = spins + n * N;
+        for (int t = 0; t < T; ++t) {
+            int8_t *sp = sprime + ((n * T) + t) * N;
+            memcpy(sp, s, (size_t)N);
+            cplx m = c64(coeffs, t);
+            for (int k = 0; k < 2; ++k) {
+                int site = sites[2 * t + k];
+                if (site < 0) continue;
+                int flips = 0;
+                m *= pauli_factor(paulis[2 * t + k], s[site], &flips);
+                if (flips) sp[site] = (int8_t)(-sp[site]);
+            }
+            mel[2 * (n * T + t)] = creal(m);
+            mel[2 * (n * T + t) + 1] = cimag(m);
+        }
+    }
+}
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}

@@ -1,0 +1,132 @@
+"""ctypes front end of oracle/nqs_oracle.c (float64 CPU oracle; TEST INFRASTRUCTURE ONLY).
+
+`build()` compiles the C file with gcc (-O2 -fopenmp) into oracle/liboracle_nqs.so;
+every other function marshals numpy arrays and calls it.  No arithmetic of the method
+lives in this file.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "nqs_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle_nqs.so")
+_lock = threading.Lock()
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle (gcc, float64, OpenMP over samples).  Returns the .so path."""
+    with _lock:
+        stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
+        if force or stale:
+            tmp = _LIB + f".tmp{os.getpid()}"
+            cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"]
+            subprocess.run(cmd, check=True)
+            os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+        lib.oracle_lncosh.argtypes = [vp, i64, i32, vp]
+        lib.oracle_lncosh.restype = None
+        lib.oracle_log_psi.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp]
+        lib.oracle_log_psi.restype = None
+        for fn in (lib.oracle_local_energy_definition, lib.oracle_local_energy_fast):
+            fn.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp]
+            fn.restype = None
+        lib.oracle_connected.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp]
+        lib.oracle_connected.restype = None
+        lib.oracle_num_threads.restype = i32
+        lib.oracle_set_num_threads.argtypes = [i32]
+        _lib = lib
+    return _lib
+
+
+def _p(x: np.ndarray):
+    return x.ctypes.data_as(ctypes.c_void_p)
+
+
+def _c(x, dtype):
+    x = np.ascontiguousarray(x, dtype=dtype)
+    return x
+
+
+def _params(spins, a, b, W):
+    spins = _c(spins, np.int8)
+    a, b, W = _c(a, np.complex64), _c(b, np.complex64), _c(W, np.complex64)
+    B, N = spins.shape
+    M = b.shape[0]
+    assert a.shape == (N,) and W.shape == (M, N), (a.shape, b.shape, W.shape, spins.shape)
+    return spins, a, b, W, B, N, M
+
+
+def _terms(sites, paulis, coeffs):
+    sites, paulis, coeffs = _c(sites, np.int32), _c(paulis, np.uint8), _c(coeffs, np.complex64)
+    T = coeffs.shape[0]
+    assert sites.shape == (T, 2) and paulis.shape == (T, 2)
+    return sites, paulis, coeffs, T
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().oracle_set_num_threads(int(n))
+
+
+def lncosh(z: np.ndarray, stable: bool) -> np.ndarray:
+    """Pointwise log cosh: libm definition (stable=False) or formula F1 (stable=True)."""
+    z = _c(z, np.complex128).ravel()
+    out = np.empty_like(z)
+    _load().oracle_lncosh(_p(z), z.size, int(stable), _p(out))
+    return out
+
+
+def log_psi(spins, a, b, W, stable: bool = False) -> np.ndarray:
+    """complex128 [B]: Eq. 38."""
+    spins, a, b, W, B, N, M = _params(spins, a, b, W)
+    out = np.empty(B, dtype=np.complex128)
+    _load().oracle_log_psi(_p(spins), B, N, M, _p(a), _p(b), _p(W), int(stable), _p(out))
+    return out
+
+
+def _eloc(fn, spins, a, b, W, sites, paulis, coeffs):
+    spins, a, b, W, B, N, M = _params(spins, a, b, W)
+    sites, paulis, coeffs, T = _terms(sites, paulis, coeffs)
+    eloc = np.empty(B, dtype=np.complex128)
+    logpsi = np.empty(B, dtype=np.complex128)
+    fn(_p(spins), B, N, M, _p(a), _p(b), _p(W), T, _p(sites), _p(paulis), _p(coeffs), _p(eloc), _p(logpsi))
+    return eloc, logpsi
+
+
+def local_energy_definition(spins, a, b, W, sites, paulis, coeffs):
+    """(E_loc, log psi) complex128 [B]; definition mode -- the parity authority."""
+    return _eloc(_load().oracle_local_energy_definition, spins, a, b, W, sites, paulis, coeffs)
+
+
+def local_energy_fast(spins, a, b, W, sites, paulis, coeffs):
+    """(E_loc, log psi) complex128 [B]; fast mode (flip grouping + low-rank theta update)."""
+    return _eloc(_load().oracle_local_energy_fast, spins, a, b, W, sites, paulis, coeffs)
+
+
+def connected(spins, sites, paulis, coeffs):
+    """Eq. 39 as data, term by term: s' int8 [B,T,N] and matrix elements complex128 [B,T]."""
+    spins = _c(spins, np.int8)
+    B, N = spins.shape
+    sites, paulis, coeffs, T = _terms(sites, paulis, coeffs)
+    sp = np.empty((B, T, N), dtype=np.int8)
+    mel = np.empty((B, T), dtype=np.complex128)
+    _load().oracle_connected(_p(spins), B, N, T, _p(sites), _p(paulis), _p(coeffs), _p(sp), _p(mel))
+    return sp, mel
