@@ -1,0 +1,156 @@
+/*
+ * nqs.h -- C ABI of the B200-native batched local-energy library (libnqs_b200.so).
+ *
+ * What it computes (citations: /root/reference/PAPER.md line numbers):
+ *
+ *   log psi(s) = sum_i a_i s_i + sum_j log cosh(b_j + sum_i W_ji s_i)       Eq. 38, :385-390
+ *       complex-parameter (holomorphic, :299 option 1) Restricted Boltzmann Machine;
+ *       j = 0..M-1 hidden units, i = 0..N-1 sites, W is [M,N] row-major (W[j*N+i]).
+ *
+ *   E_loc(s)   = sum_s' <s|H|s'> psi(s') / psi(s)                            Eq. 4, :63-68, :89
+ *       for H = sum_t c_t P_t with P_t a product of at most two Pauli matrices on distinct
+ *       sites ("branch-free" operators, :473); the connected configurations s' and matrix
+ *       elements <s|P_t|s'> are generated on the fly on the device (Eq. 39, :418-426;
+ *       Algorithm 1 lines 6-8, :163-194; the four-call sequence at :464-469).
+ *
+ * Conventions: spins are int8 +1/-1, +1 = up = sigma^z eigenvalue +1.
+ * Row convention for matrix elements: <s|X_k|s'> = 1, <s|Y_k|s'> = -i s_k, <s|Z_k|s> = s_k,
+ * with s' = s with site k flipped for X and Y.  Terms reaching the same s' are summed; a
+ * (summed) matrix element that is exactly zero contributes nothing (":458 non-zero matrix
+ * elements").  Im log psi is defined mod 2 pi (sum over hidden units of an unwrapped phase).
+ *
+ * General rules for every entry point
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The caller owns every
+ *     buffer; the library never frees or retains caller memory.  Term arrays (h_sites,
+ *     h_paulis, h_coeffs) are read before the call returns.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
+ *     entry points are asynchronous on that stream and never synchronise the device.  Scratch
+ *     memory (parameter tables, tanh(theta)) is taken from the CUDA stream-ordered allocator
+ *     (cudaMallocAsync on `stream`) and returned to it before the call returns; no global
+ *     mutable state is kept besides a small cache of compiled Hamiltonians.
+ *   - *_host entry points take HOST buffers, copy them to the device, run the same kernels,
+ *     copy the result back and synchronise before returning.
+ *   - Return value: 0 (NQS_OK) or a negative NQS_ERR_* code; nqs_last_error() then returns a
+ *     thread-local message.  No partial results are promised on error.  B == 0 is a no-op.
+ *   - There is NO CPU fallback: without a usable CUDA device every compute call returns
+ *     NQS_ERR_CUDA.
+ *   - Spin values other than +1/-1 are undefined behaviour.  psi(s) = 0 or overflow follow
+ *     IEEE (inf/NaN in the output), not an error.
+ */
+#ifndef NQS_B200_H
+#define NQS_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct { float re, im; } nqs_c64; /* == complex64, interleaved */
+
+enum { NQS_I = 0, NQS_X = 1, NQS_Y = 2, NQS_Z = 3 };
+
+enum {
+    NQS_OK = 0,
+    NQS_ERR_INVALID_ARG = -1,  /* NULL pointer, negative size, N/M out of range            */
+    NQS_ERR_INVALID_TERM = -2, /* site out of range, Pauli code > 3, same site twice,      */
+                               /* non-identity Pauli on an unused (-1) slot                */
+    NQS_ERR_CUDA = -3,         /* CUDA runtime error or no device                          */
+    NQS_ERR_UNSUPPORTED = -4   /* shape outside what the kernels support                   */
+};
+
+/* Opaque compiled Hamiltonian (step a0 of DESIGN.md): terms grouped by flip set, diagonal
+ * list, per-group matrix-element programs, uploaded to the device once. */
+typedef struct nqs_hamiltonian nqs_hamiltonian;
+
+/* ---------------------------------------------------------------------------------------
+ * log psi(s) for a batch (Eq. 38).
+ *   d_spins  [B,N] int8 row-major, values +1/-1            d_a [N], d_b [M], d_W [M,N] complex64
+ *   d_logpsi [B]   complex64 out
+ * ------------------------------------------------------------------------------------- */
+int nqs_log_psi(const int8_t *d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64 *d_a,
+                const nqs_c64 *d_b, const nqs_c64 *d_W, nqs_c64 *d_logpsi, void *stream);
+
+/* ---------------------------------------------------------------------------------------
+ * E_loc(s) for a batch (Eq. 4; Algorithm 1 lines 6-8).
+ *   T terms: h_sites [T,2] int32 (-1 = unused slot), h_paulis [T,2] uint8 (NQS_I..NQS_Z),
+ *   h_coeffs [T] complex64.  Both slots unused / identity = constant term c * 1.
+ *   d_eloc [B] complex64 out; d_logpsi [B] complex64 out or NULL.
+ * Compiles (or fetches from an internal cache keyed by the term bytes) the Hamiltonian, then
+ * behaves as nqs_local_energy_h.
+ * ------------------------------------------------------------------------------------- */
+int nqs_local_energy(const int8_t *d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64 *d_a,
+                     const nqs_c64 *d_b, const nqs_c64 *d_W, int32_t T, const int32_t *h_sites,
+                     const uint8_t *h_paulis, const nqs_c64 *h_coeffs, nqs_c64 *d_eloc,
+                     nqs_c64 *d_logpsi, void *stream);
+
+/* Same with HOST buffers for everything (spins, parameters, outputs): H2D copies, kernels,
+ * D2H copies, stream synchronise.  h_logpsi may be NULL. */
+int nqs_local_energy_host(const int8_t *h_spins, int64_t B, int32_t N, int32_t M, const nqs_c64 *h_a,
+                          const nqs_c64 *h_b, const nqs_c64 *h_W, int32_t T, const int32_t *h_sites,
+                          const uint8_t *h_paulis, const nqs_c64 *h_coeffs, nqs_c64 *h_eloc,
+                          nqs_c64 *h_logpsi);
+
+int nqs_log_psi_host(const int8_t *h_spins, int64_t B, int32_t N, int32_t M, const nqs_c64 *h_a,
+                     const nqs_c64 *h_b, const nqs_c64 *h_W, nqs_c64 *h_logpsi);
+
+/* ---------------------------------------------------------------------------------------
+ * Compiled-Hamiltonian handle (static for a whole simulation; parameters change every step).
+ * nqs_hamiltonian_create validates the terms (NQS_ERR_INVALID_TERM), groups them by flip set
+ * (Eq. 39: all terms of a group reach the same s') and uploads the result to the current
+ * device.  The handle is immutable and may be used from several streams.
+ * ------------------------------------------------------------------------------------- */
+int nqs_hamiltonian_create(int32_t N, int32_t T, const int32_t *h_sites, const uint8_t *h_paulis,
+                           const nqs_c64 *h_coeffs, nqs_hamiltonian **out);
+int nqs_hamiltonian_destroy(nqs_hamiltonian *h);
+
+/* Host-side description of the compiled form (no device work; usable without a GPU when the
+ * handle was made with nqs_hamiltonian_compile_host):
+ *   info[0] = G  number of flip groups (distinct non-empty flip sets)
+ *   info[1] = C  number of table columns (1 per single-flip group, 1 or 2 per pair group)
+ *   info[2] = number of diagonal terms (empty flip set)
+ *   info[3] = number of terms in flip groups
+ *   info[4] = N
+ * flip_sites, if not NULL, receives [G,2] int32: the group's flip set (second = -1 if single),
+ * in group order (order of first appearance in the term list). */
+int nqs_hamiltonian_info(const nqs_hamiltonian *h, int32_t info[5], int32_t *flip_sites);
+
+/* Host-only compile (validation + grouping, nothing uploaded): for tests of the host logic on
+ * machines without a GPU.  A handle made this way is rejected by the compute entry points. */
+int nqs_hamiltonian_compile_host(int32_t N, int32_t T, const int32_t *h_sites, const uint8_t *h_paulis,
+                                 const nqs_c64 *h_coeffs, nqs_hamiltonian **out);
+
+int nqs_local_energy_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t B, int32_t M,
+                       const nqs_c64 *d_a, const nqs_c64 *d_b, const nqs_c64 *d_W, nqs_c64 *d_eloc,
+                       nqs_c64 *d_logpsi, void *stream);
+
+/* ---------------------------------------------------------------------------------------
+ * Test/debug entry (small inputs): materialise Eq. 39 -- the connected configurations and
+ * summed matrix elements per flip group (PAPER.md:456-458 get_s_primes).  Slot 0 is the
+ * diagonal (s' = s, element = sum of the diagonal terms), slot 1+g is flip group g:
+ *   d_sprime [B,G+1,N] int8, d_mel [B,G+1] complex64.  A zero element means "not connected".
+ * ------------------------------------------------------------------------------------- */
+int nqs_enumerate_connected(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t B,
+                            int8_t *d_sprime, nqs_c64 *d_mel, void *stream);
+
+/* Optional per-kernel timing for benchmarks.  nqs_profile_enable(1) makes every following
+ * nqs_local_energy* call record CUDA events on its stream around its four kernels;
+ * nqs_profile_last() waits for the most recent such call and returns the elapsed milliseconds of
+ * ms[0] parameter tables (a1), ms[1] theta / log psi / tanh (a2, a3), ms[2] connected amplitudes
+ * (a4, a5), ms[3] final reduction (a6).  Not thread-safe; off by default. */
+int nqs_profile_enable(int on);
+int nqs_profile_last(float ms[4]);
+
+/* Thread-local message of the last error on this thread ("" if none). */
+const char *nqs_last_error(void);
+
+/* Drops the internal cache of compiled Hamiltonians (device memory freed). */
+int nqs_release(void);
+
+/* "major.minor.patch sm_100a" */
+const char *nqs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NQS_B200_H */

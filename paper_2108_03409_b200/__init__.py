@@ -1,0 +1,24 @@
+"""B200-native batched RBM local energy (jVMC hot path, arxiv 2108.03409).
+
+Thin Python binding over the C-ABI library libnqs_b200.so (include/nqs.h): argument
+marshalling only -- every step of the path runs in the CUDA kernels.  PyTorch is used for
+device memory and streams.  There is no CPU fallback: without the built library or without a
+CUDA device the calls raise.
+"""
+from .binding import (  # noqa: F401
+    Hamiltonian,
+    NqsError,
+    enumerate_connected,
+    hamiltonian_info_host,
+    last_error,
+    lib_path,
+    load_library,
+    local_energy,
+    local_energy_host,
+    log_psi,
+    log_psi_host,
+    profile_enable,
+    profile_last,
+    release,
+    version,
+)

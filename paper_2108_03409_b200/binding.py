@@ -1,0 +1,254 @@
+"""ctypes binding of libnqs_b200.so -- same names as include/nqs.h, marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libnqs_b200.so")
+_lock = threading.Lock()
+_lib = None
+
+NQS_OK = 0
+ERROR_NAMES = {-1: "NQS_ERR_INVALID_ARG", -2: "NQS_ERR_INVALID_TERM", -3: "NQS_ERR_CUDA", -4: "NQS_ERR_UNSUPPORTED"}
+
+
+class NqsError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"{ERROR_NAMES.get(code, code)}: {message}")
+        self.code = code
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library() -> ctypes.CDLL:
+    """Loads libnqs_b200.so; raises if it has not been built (python -m paper_2108_03409_b200.build)."""
+    global _lib
+    with _lock:
+        if _lib is None:
+            if not os.path.exists(_LIB_PATH):
+                raise FileNotFoundError(
+                    f"{_LIB_PATH} is missing: build it with `python -m paper_2108_03409_b200.build` "
+                    "(there is no CPU fallback)")
+            lib = ctypes.CDLL(_LIB_PATH)
+            vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32
+            lib.nqs_log_psi.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp]
+            lib.nqs_local_energy.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp]
+            lib.nqs_local_energy_host.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp]
+            lib.nqs_log_psi_host.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp]
+            lib.nqs_hamiltonian_create.argtypes = [i32, i32, vp, vp, vp, ctypes.POINTER(vp)]
+            lib.nqs_hamiltonian_compile_host.argtypes = [i32, i32, vp, vp, vp, ctypes.POINTER(vp)]
+            lib.nqs_hamiltonian_destroy.argtypes = [vp]
+            lib.nqs_hamiltonian_info.argtypes = [vp, vp, vp]
+            lib.nqs_local_energy_h.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, vp]
+            lib.nqs_enumerate_connected.argtypes = [vp, vp, i64, vp, vp, vp]
+            lib.nqs_profile_enable.argtypes = [i32]
+            lib.nqs_profile_last.argtypes = [vp]
+            lib.nqs_last_error.restype = ctypes.c_char_p
+            lib.nqs_version.restype = ctypes.c_char_p
+            for name in ("nqs_log_psi", "nqs_local_energy", "nqs_local_energy_host", "nqs_log_psi_host",
+                         "nqs_hamiltonian_create", "nqs_hamiltonian_compile_host", "nqs_hamiltonian_destroy",
+                         "nqs_hamiltonian_info", "nqs_local_energy_h", "nqs_enumerate_connected", "nqs_release",
+                         "nqs_profile_enable", "nqs_profile_last"):
+                getattr(lib, name).restype = ctypes.c_int
+            _lib = lib
+    return _lib
+
+
+def last_error() -> str:
+    return load_library().nqs_last_error().decode()
+
+
+def version() -> str:
+    return load_library().nqs_version().decode()
+
+
+def release() -> None:
+    _check(load_library().nqs_release())
+
+
+def profile_enable(on: bool) -> None:
+    _check(load_library().nqs_profile_enable(int(on)))
+
+
+def profile_last() -> dict:
+    """Milliseconds of the four kernels of the most recent profiled nqs_local_energy* call."""
+    ms = (ctypes.c_float * 4)()
+    _check(load_library().nqs_profile_last(ms))
+    return dict(table=ms[0], theta=ms[1], eloc=ms[2], finalize=ms[3])
+
+
+def _check(rc: int) -> None:
+    if rc != NQS_OK:
+        raise NqsError(rc, last_error())
+
+
+def _np(x, dtype, shape_tail=None):
+    x = np.ascontiguousarray(x, dtype=dtype)
+    if shape_tail is not None:
+        assert x.shape[1:] == shape_tail, (x.shape, shape_tail)
+    return x
+
+
+def _terms(sites, paulis, coeffs):
+    sites = _np(sites, np.int32).reshape(-1, 2)
+    paulis = _np(paulis, np.uint8).reshape(-1, 2)
+    coeffs = _np(coeffs, np.complex64).reshape(-1)
+    assert sites.shape[0] == paulis.shape[0] == coeffs.shape[0]
+    return sites, paulis, coeffs
+
+
+def _hp(x: np.ndarray):
+    return x.ctypes.data_as(ctypes.c_void_p)
+
+
+def _stream():
+    import torch
+
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(t, dtype, name):
+    import torch
+
+    if not (isinstance(t, torch.Tensor) and t.is_cuda):
+        raise TypeError(f"{name} must be a CUDA tensor")
+    if t.dtype != dtype:
+        raise TypeError(f"{name} must have dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _shapes(spins, a, b, W):
+    B, N = spins.shape
+    M = b.shape[0]
+    if tuple(a.shape) != (N,) or tuple(W.shape) != (M, N):
+        raise ValueError(f"shape mismatch: spins {tuple(spins.shape)}, a {tuple(a.shape)}, b {tuple(b.shape)}, "
+                         f"W {tuple(W.shape)}")
+    return B, N, M
+
+
+class Hamiltonian:
+    """Compiled term list (nqs_hamiltonian_create / _compile_host / _destroy / _info)."""
+
+    def __init__(self, N: int, sites, paulis, coeffs, host_only: bool = False):
+        lib = load_library()
+        sites, paulis, coeffs = _terms(sites, paulis, coeffs)
+        self.N = int(N)
+        self.T = int(coeffs.shape[0])
+        self._h = ctypes.c_void_p()
+        fn = lib.nqs_hamiltonian_compile_host if host_only else lib.nqs_hamiltonian_create
+        _check(fn(self.N, self.T, _hp(sites), _hp(paulis), _hp(coeffs), ctypes.byref(self._h)))
+        info = np.zeros(5, np.int32)
+        _check(lib.nqs_hamiltonian_info(self._h, _hp(info), None))
+        self.G, self.C, self.n_diag, self.n_group_terms = (int(v) for v in info[:4])
+        flips = np.zeros((max(self.G, 1), 2), np.int32)
+        _check(lib.nqs_hamiltonian_info(self._h, _hp(info), _hp(flips)))
+        self.flip_sites = flips[: self.G].copy()
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            load_library().nqs_hamiltonian_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def local_energy(self, spins, a, b, W, want_logpsi: bool = True):
+        import torch
+
+        B, N, M = _shapes(spins, a, b, W)
+        if N != self.N:
+            raise ValueError("N mismatch with the compiled Hamiltonian")
+        eloc = torch.empty(B, dtype=torch.complex64, device=spins.device)
+        logpsi = torch.empty(B, dtype=torch.complex64, device=spins.device) if want_logpsi else None
+        with torch.cuda.device(spins.device):
+            _check(load_library().nqs_local_energy_h(
+                self._h, _dev(spins, torch.int8, "spins"), B, M, _dev(a, torch.complex64, "a"),
+                _dev(b, torch.complex64, "b"), _dev(W, torch.complex64, "W"), ctypes.c_void_p(eloc.data_ptr()),
+                ctypes.c_void_p(logpsi.data_ptr()) if want_logpsi else None, _stream()))
+        return (eloc, logpsi) if want_logpsi else eloc
+
+
+def hamiltonian_info_host(N: int, sites, paulis, coeffs) -> dict:
+    """Host-only compile (no GPU needed): grouping of the term list by flip set."""
+    h = Hamiltonian(N, sites, paulis, coeffs, host_only=True)
+    out = dict(G=h.G, C=h.C, n_diag=h.n_diag, n_group_terms=h.n_group_terms, flip_sites=h.flip_sites)
+    h.close()
+    return out
+
+
+def log_psi(spins, a, b, W):
+    """nqs_log_psi: complex64 [B] CUDA tensor (Eq. 38)."""
+    import torch
+
+    B, N, M = _shapes(spins, a, b, W)
+    out = torch.empty(B, dtype=torch.complex64, device=spins.device)
+    with torch.cuda.device(spins.device):
+        _check(load_library().nqs_log_psi(_dev(spins, torch.int8, "spins"), B, N, M, _dev(a, torch.complex64, "a"),
+                                          _dev(b, torch.complex64, "b"), _dev(W, torch.complex64, "W"),
+                                          ctypes.c_void_p(out.data_ptr()), _stream()))
+    return out
+
+
+def local_energy(spins, a, b, W, sites, paulis, coeffs, want_logpsi: bool = True):
+    """nqs_local_energy: (E_loc, log psi) complex64 [B] CUDA tensors (Eq. 4)."""
+    import torch
+
+    B, N, M = _shapes(spins, a, b, W)
+    sites, paulis, coeffs = _terms(sites, paulis, coeffs)
+    eloc = torch.empty(B, dtype=torch.complex64, device=spins.device)
+    logpsi = torch.empty(B, dtype=torch.complex64, device=spins.device) if want_logpsi else None
+    with torch.cuda.device(spins.device):
+        _check(load_library().nqs_local_energy(
+            _dev(spins, torch.int8, "spins"), B, N, M, _dev(a, torch.complex64, "a"), _dev(b, torch.complex64, "b"),
+            _dev(W, torch.complex64, "W"), int(coeffs.shape[0]), _hp(sites), _hp(paulis), _hp(coeffs),
+            ctypes.c_void_p(eloc.data_ptr()), ctypes.c_void_p(logpsi.data_ptr()) if want_logpsi else None,
+            _stream()))
+    return (eloc, logpsi) if want_logpsi else eloc
+
+
+def local_energy_host(spins, a, b, W, sites, paulis, coeffs, eloc_out=None, logpsi_out=None, want_logpsi=True):
+    """nqs_local_energy_host: numpy (or pinned torch CPU) buffers in, numpy out; copies inside."""
+    spins = _np(spins, np.int8)
+    a, b, W = _np(a, np.complex64), _np(b, np.complex64), _np(W, np.complex64)
+    B, N, M = _shapes(spins, a, b, W)
+    sites, paulis, coeffs = _terms(sites, paulis, coeffs)
+    eloc = np.empty(B, np.complex64) if eloc_out is None else eloc_out
+    logpsi = (np.empty(B, np.complex64) if logpsi_out is None else logpsi_out) if want_logpsi else None
+    _check(load_library().nqs_local_energy_host(
+        _hp(spins), B, N, M, _hp(a), _hp(b), _hp(W), int(coeffs.shape[0]), _hp(sites), _hp(paulis), _hp(coeffs),
+        _hp(eloc), _hp(logpsi) if want_logpsi else None))
+    return (eloc, logpsi) if want_logpsi else eloc
+
+
+def log_psi_host(spins, a, b, W):
+    spins = _np(spins, np.int8)
+    a, b, W = _np(a, np.complex64), _np(b, np.complex64), _np(W, np.complex64)
+    B, N, M = _shapes(spins, a, b, W)
+    out = np.empty(B, np.complex64)
+    _check(load_library().nqs_log_psi_host(_hp(spins), B, N, M, _hp(a), _hp(b), _hp(W), _hp(out)))
+    return out
+
+
+def enumerate_connected(ham: Hamiltonian, spins):
+    """nqs_enumerate_connected: s' int8 [B,G+1,N], elements complex64 [B,G+1] (slot 0 = diagonal)."""
+    import torch
+
+    B, N = spins.shape
+    sp = torch.empty((B, ham.G + 1, N), dtype=torch.int8, device=spins.device)
+    mel = torch.empty((B, ham.G + 1), dtype=torch.complex64, device=spins.device)
+    with torch.cuda.device(spins.device):
+        _check(load_library().nqs_enumerate_connected(ham._h, _dev(spins, torch.int8, "spins"), B,
+                                                      ctypes.c_void_p(sp.data_ptr()),
+                                                      ctypes.c_void_p(mel.data_ptr()), _stream()))
+    return sp, mel

@@ -1,0 +1,540 @@
+// C ABI of libnqs_b200.so (declared in include/nqs.h): argument checks, workspace, launches.
+// Every step of the path runs in the kernels of nqs_kernels.cuh; there is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <list>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "../../include/nqs.h"
+#include "nqs_hamiltonian.h"
+#include "nqs_kernels.cuh"
+
+using namespace nqs;
+
+// ----------------------------------------------------------------------------------------
+// errors
+// ----------------------------------------------------------------------------------------
+static thread_local std::string g_err;
+
+static int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+#define NQS_CUDA(call)                                                                             \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess)                                                                    \
+            return fail(NQS_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__));        \
+    } while (0)
+
+extern "C" const char* nqs_last_error(void) { return g_err.c_str(); }
+extern "C" const char* nqs_version(void) { return "0.1.0 sm_100a"; }
+
+// ----------------------------------------------------------------------------------------
+// handle
+// ----------------------------------------------------------------------------------------
+struct nqs_hamiltonian {
+    HostCompiled hc;
+    int device = -1;       // -1: host-only compile
+    void* d_blob = nullptr;
+    DevHam dev{};
+    int C = 0;
+    // launch plan (static for the handle): column tiling of the a5 kernel
+    int WC = 1, WS = 2, TC = 16, nTiles = 1, C_pad = 16;
+};
+
+static constexpr int KJ = 16;
+static constexpr int MAX_WC = 5;
+
+static void plan_tiles(nqs_hamiltonian* h) {
+    const int C = (int)h->hc.col_i.size();
+    h->C = C;
+    const int slices = C > 0 ? (C + 15) / 16 : 1;
+    // fewest padded 16-column slices; ties -> wider blocks (less re-staging of tanh(theta))
+    int best = 1;
+    double best_cost = 1e30;
+    for (int wc = 1; wc <= MAX_WC; ++wc) {
+        const int tiles = (slices + wc - 1) / wc;
+        const double cost = (double)tiles * wc * (1.0 + 0.08 / wc);
+        if (cost < best_cost - 1e-9 || (cost < best_cost + 1e-9 && wc > best)) {
+            best_cost = cost;
+            best = wc;
+        }
+    }
+    h->WC = best;
+    h->WS = 2;
+    h->TC = 16 * best;
+    h->nTiles = (slices + best - 1) / best;
+    h->C_pad = h->nTiles * h->TC;
+}
+
+static int upload(nqs_hamiltonian* h) {
+    const HostCompiled& hc = h->hc;
+    const int G = (int)hc.groups.size(), Td = (int)hc.diag_c.size(), Tg = (int)hc.gt_c.size();
+    const int C_pad = h->C_pad;
+    // blob layout: ints then float2s
+    std::vector<int> ints;
+    auto push = [&](const std::vector<int32_t>& v) {
+        size_t o = ints.size();
+        ints.insert(ints.end(), v.begin(), v.end());
+        return o;
+    };
+    std::vector<int32_t> f0(G), f1(G), first(G), count(G);
+    for (int g = 0; g < G; ++g) {
+        f0[g] = hc.groups[g].f0;
+        f1[g] = hc.groups[g].f1;
+        first[g] = hc.groups[g].term_first;
+        count[g] = hc.groups[g].term_count;
+    }
+    std::vector<int32_t> ci(C_pad, 0), ck(C_pad, -1), cp(C_pad, 1), cg(C_pad, -1);
+    for (int c = 0; c < h->C; ++c) {
+        ci[c] = hc.col_i[c];
+        ck[c] = hc.col_k[c];
+        cp[c] = hc.col_p[c];
+        cg[c] = hc.col_group[c];
+    }
+    const size_t o_dz0 = push(hc.diag_z0), o_dz1 = push(hc.diag_z1);
+    const size_t o_f0 = push(f0), o_f1 = push(f1), o_first = push(first), o_count = push(count);
+    const size_t o_gz0 = push(hc.gt_z0), o_gz1 = push(hc.gt_z1);
+    const size_t o_ci = push(ci), o_ck = push(ck), o_cp = push(cp), o_cg = push(cg);
+    size_t int_bytes = (ints.size() * sizeof(int) + 15) / 16 * 16;
+    std::vector<nqs_c64> cs;
+    cs.insert(cs.end(), hc.diag_c.begin(), hc.diag_c.end());
+    cs.insert(cs.end(), hc.gt_c.begin(), hc.gt_c.end());
+    const size_t total = int_bytes + cs.size() * sizeof(nqs_c64) + 16;
+    std::vector<unsigned char> blob(total, 0);
+    if (!ints.empty()) memcpy(blob.data(), ints.data(), ints.size() * sizeof(int));
+    if (!cs.empty()) memcpy(blob.data() + int_bytes, cs.data(), cs.size() * sizeof(nqs_c64));
+    NQS_CUDA(cudaGetDevice(&h->device));
+    NQS_CUDA(cudaMalloc(&h->d_blob, total));
+    NQS_CUDA(cudaMemcpy(h->d_blob, blob.data(), total, cudaMemcpyHostToDevice));
+    const int* di = reinterpret_cast<const int*>(h->d_blob);
+    const float2* dc = reinterpret_cast<const float2*>(reinterpret_cast<const unsigned char*>(h->d_blob) + int_bytes);
+    DevHam& D = h->dev;
+    D.N = hc.N;
+    D.G = G;
+    D.C = h->C;
+    D.Td = Td;
+    D.Tg = Tg;
+    D.diag_z0 = di + o_dz0;
+    D.diag_z1 = di + o_dz1;
+    D.diag_c = dc;
+    D.grp_f0 = di + o_f0;
+    D.grp_f1 = di + o_f1;
+    D.grp_first = di + o_first;
+    D.grp_count = di + o_count;
+    D.gt_z0 = di + o_gz0;
+    D.gt_z1 = di + o_gz1;
+    D.gt_c = dc + Td;
+    D.col_i = di + o_ci;
+    D.col_k = di + o_ck;
+    D.col_p = di + o_cp;
+    D.col_group = di + o_cg;
+    return NQS_OK;
+}
+
+static int create_impl(int32_t N, int32_t T, const int32_t* s, const uint8_t* p, const nqs_c64* c, bool device,
+                       nqs_hamiltonian** out) {
+    if (!out) return fail(NQS_ERR_INVALID_ARG, "nqs_hamiltonian_create: out is NULL");
+    *out = nullptr;
+    auto* h = new nqs_hamiltonian();
+    std::string err;
+    int rc = compile_hamiltonian(N, T, s, p, c, h->hc, err);
+    if (rc != NQS_OK) {
+        delete h;
+        return fail(rc, err);
+    }
+    plan_tiles(h);
+    if (device) {
+        rc = upload(h);
+        if (rc != NQS_OK) {
+            if (h->d_blob) cudaFree(h->d_blob);
+            delete h;
+            return rc;
+        }
+    }
+    *out = h;
+    return NQS_OK;
+}
+
+extern "C" int nqs_hamiltonian_create(int32_t N, int32_t T, const int32_t* h_sites, const uint8_t* h_paulis,
+                                      const nqs_c64* h_coeffs, nqs_hamiltonian** out) {
+    return create_impl(N, T, h_sites, h_paulis, h_coeffs, true, out);
+}
+extern "C" int nqs_hamiltonian_compile_host(int32_t N, int32_t T, const int32_t* h_sites, const uint8_t* h_paulis,
+                                            const nqs_c64* h_coeffs, nqs_hamiltonian** out) {
+    return create_impl(N, T, h_sites, h_paulis, h_coeffs, false, out);
+}
+extern "C" int nqs_hamiltonian_destroy(nqs_hamiltonian* h) {
+    if (!h) return NQS_OK;
+    if (h->d_blob) cudaFree(h->d_blob);
+    delete h;
+    return NQS_OK;
+}
+extern "C" int nqs_hamiltonian_info(const nqs_hamiltonian* h, int32_t info[5], int32_t* flip_sites) {
+    if (!h || !info) return fail(NQS_ERR_INVALID_ARG, "nqs_hamiltonian_info: NULL argument");
+    info[0] = (int32_t)h->hc.groups.size();
+    info[1] = (int32_t)h->hc.col_i.size();
+    info[2] = (int32_t)h->hc.diag_c.size();
+    info[3] = (int32_t)h->hc.gt_c.size();
+    info[4] = h->hc.N;
+    if (flip_sites)
+        for (size_t g = 0; g < h->hc.groups.size(); ++g) {
+            flip_sites[2 * g] = h->hc.groups[g].f0;
+            flip_sites[2 * g + 1] = h->hc.groups[g].f1;
+        }
+    return NQS_OK;
+}
+
+// ----------------------------------------------------------------------------------------
+// cache of compiled Hamiltonians for the term-list entry points
+// ----------------------------------------------------------------------------------------
+struct CacheEntry {
+    int device, N, T;
+    std::vector<unsigned char> key;
+    nqs_hamiltonian* h;
+};
+static std::mutex g_cache_mu;
+static std::list<CacheEntry> g_cache;
+
+static int cached_hamiltonian(int32_t N, int32_t T, const int32_t* s, const uint8_t* p, const nqs_c64* c,
+                              nqs_hamiltonian** out) {
+    if (T < 0 || (T > 0 && (!s || !p || !c))) return fail(NQS_ERR_INVALID_ARG, "term arrays are NULL or T < 0");
+    int dev = 0;
+    NQS_CUDA(cudaGetDevice(&dev));
+    std::vector<unsigned char> key((size_t)T * (8 + 2 + 8));
+    if (T > 0) {
+        memcpy(key.data(), s, (size_t)T * 8);
+        memcpy(key.data() + (size_t)T * 8, p, (size_t)T * 2);
+        memcpy(key.data() + (size_t)T * 10, c, (size_t)T * 8);
+    }
+    std::lock_guard<std::mutex> lk(g_cache_mu);
+    for (auto it = g_cache.begin(); it != g_cache.end(); ++it)
+        if (it->device == dev && it->N == N && it->T == T && it->key == key) {
+            g_cache.splice(g_cache.begin(), g_cache, it);
+            *out = g_cache.front().h;
+            return NQS_OK;
+        }
+    nqs_hamiltonian* h = nullptr;
+    int rc = nqs_hamiltonian_create(N, T, s, p, c, &h);
+    if (rc != NQS_OK) return rc;
+    g_cache.push_front(CacheEntry{dev, N, T, std::move(key), h});
+    if (g_cache.size() > 8) {
+        // an evicted handle may still be in use by kernels in flight on some stream
+        cudaDeviceSynchronize();
+        nqs_hamiltonian_destroy(g_cache.back().h);
+        g_cache.pop_back();
+    }
+    *out = h;
+    return NQS_OK;
+}
+
+extern "C" int nqs_release(void) {
+    std::lock_guard<std::mutex> lk(g_cache_mu);
+    if (!g_cache.empty()) cudaDeviceSynchronize();
+    for (auto& e : g_cache) nqs_hamiltonian_destroy(e.h);
+    g_cache.clear();
+    return NQS_OK;
+}
+
+// ----------------------------------------------------------------------------------------
+// optional per-kernel timing (bench.py's roofline leg): CUDA events recorded on the caller's
+// stream around the four kernels of the most recent nqs_local_energy* call
+// ----------------------------------------------------------------------------------------
+static bool g_prof_on = false;
+static cudaEvent_t g_prof_ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+static bool g_prof_valid = false;
+
+extern "C" int nqs_profile_enable(int on) {
+    if (on && !g_prof_ev[0])
+        for (auto& e : g_prof_ev) NQS_CUDA(cudaEventCreate(&e));
+    g_prof_on = on != 0;
+    g_prof_valid = false;
+    return NQS_OK;
+}
+extern "C" int nqs_profile_last(float ms[4]) {
+    if (!ms) return fail(NQS_ERR_INVALID_ARG, "ms is NULL");
+    if (!g_prof_valid) return fail(NQS_ERR_INVALID_ARG, "no profiled call recorded");
+    NQS_CUDA(cudaEventSynchronize(g_prof_ev[4]));
+    for (int k = 0; k < 4; ++k) NQS_CUDA(cudaEventElapsedTime(&ms[k], g_prof_ev[k], g_prof_ev[k + 1]));
+    return NQS_OK;
+}
+#define NQS_PROF(k, st)                                            \
+    do {                                                           \
+        if (g_prof_on) NQS_CUDA(cudaEventRecord(g_prof_ev[k], st)); \
+    } while (0)
+
+// ----------------------------------------------------------------------------------------
+// device checks, workspace
+// ----------------------------------------------------------------------------------------
+static int check_device() {
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n == 0) {
+        cudaGetLastError();
+        return fail(NQS_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
+    }
+    static std::once_flag once;
+    std::call_once(once, [&] {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long thr = ~0ull;  // keep freed workspace cached in the pool
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        }
+    });
+    return NQS_OK;
+}
+
+static inline long long round_up(long long x, long long m) { return (x + m - 1) / m * m; }
+
+static int launch_theta(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
+                        const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad, nqs_c64* d_logpsi,
+                        cudaStream_t st) {
+    const long long rows = tp ? nPairsPad * 2 : B;
+    const unsigned grid = (unsigned)((rows + 63) / 64);
+    static bool attr_set = false;
+    if (!attr_set) {
+        NQS_CUDA(cudaFuncSetAttribute(theta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TH_SMEM));
+        attr_set = true;
+    }
+    theta_kernel<<<grid, 256, TH_SMEM, st>>>(d_spins, (long long)B, N, M, M_pad, (const float2*)d_a, (const float2*)d_b,
+                                       (const float2*)d_W, tp, nPairsPad, (float2*)d_logpsi);
+    NQS_CUDA(cudaGetLastError());
+    return NQS_OK;
+}
+
+template <int WC, int WS>
+static int launch_eloc_t(const ElocParams& p, long long nBlocksY, cudaStream_t st) {
+    using Cfg = ElocCfg<WC, WS, KJ>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        NQS_CUDA(cudaFuncSetAttribute(eloc_kernel<WC, WS, KJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)Cfg::SMEM));
+        attr_set = true;
+    }
+    dim3 grid((unsigned)p.nTiles, (unsigned)nBlocksY);
+    eloc_kernel<WC, WS, KJ><<<grid, Cfg::NT, Cfg::SMEM, st>>>(p);
+    NQS_CUDA(cudaGetLastError());
+    return NQS_OK;
+}
+
+static int launch_eloc(const nqs_hamiltonian* h, const ElocParams& p, long long B_pad, cudaStream_t st) {
+    const long long nby = B_pad / (32 * h->WS);
+    switch (h->WC) {
+        case 1: return launch_eloc_t<1, 2>(p, nby, st);
+        case 2: return launch_eloc_t<2, 2>(p, nby, st);
+        case 3: return launch_eloc_t<3, 2>(p, nby, st);
+        case 4: return launch_eloc_t<4, 2>(p, nby, st);
+        case 5: return launch_eloc_t<5, 2>(p, nby, st);
+    }
+    return fail(NQS_ERR_UNSUPPORTED, "unsupported column tiling");
+}
+
+static int check_common(const void* spins, int64_t B, int32_t N, int32_t M, const void* a, const void* b,
+                        const void* W) {
+    if (B < 0) return fail(NQS_ERR_INVALID_ARG, "B < 0");
+    if (N <= 0 || M <= 0) return fail(NQS_ERR_INVALID_ARG, "N and M must be positive");
+    if (B > 0 && (!spins || !a || !b || !W)) return fail(NQS_ERR_INVALID_ARG, "NULL spins/parameter pointer");
+    if ((long long)B * N > (1ll << 40)) return fail(NQS_ERR_UNSUPPORTED, "B*N too large");
+    return NQS_OK;
+}
+
+extern "C" int nqs_log_psi(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
+                           const nqs_c64* d_b, const nqs_c64* d_W, nqs_c64* d_logpsi, void* stream) {
+    int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
+    if (rc) return rc;
+    if (B > 0 && !d_logpsi) return fail(NQS_ERR_INVALID_ARG, "d_logpsi is NULL");
+    if ((rc = check_device())) return rc;
+    if (B == 0) return NQS_OK;
+    return launch_theta(d_spins, B, N, M, (int)round_up(M, KJ), d_a, d_b, d_W, nullptr, 0, d_logpsi,
+                        (cudaStream_t)stream);
+}
+
+extern "C" int nqs_local_energy_h(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int32_t M,
+                                  const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, nqs_c64* d_eloc,
+                                  nqs_c64* d_logpsi, void* stream) {
+    if (!h) return fail(NQS_ERR_INVALID_ARG, "hamiltonian handle is NULL");
+    const int N = h->hc.N;
+    int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
+    if (rc) return rc;
+    if (B > 0 && !d_eloc) return fail(NQS_ERR_INVALID_ARG, "d_eloc is NULL");
+    if ((rc = check_device())) return rc;
+    if (h->device < 0) return fail(NQS_ERR_INVALID_ARG, "handle was compiled host-only (nqs_hamiltonian_compile_host)");
+    int dev = 0;
+    NQS_CUDA(cudaGetDevice(&dev));
+    if (dev != h->device) return fail(NQS_ERR_INVALID_ARG, "handle belongs to another device");
+    if (B == 0) return NQS_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    const int M_pad = (int)round_up(M, KJ);
+    const long long B_pad = round_up(B, 256);
+    const long long nPairsPad = B_pad / 2;
+    const int nTiles = h->nTiles, TC = h->TC, C_pad = h->C_pad;
+
+    float4 *tp = nullptr, *tab = nullptr, *rho = nullptr;
+    float2* partial = nullptr;
+    const bool have_cols = h->C > 0;
+    if (have_cols) {
+        NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
+        NQS_CUDA(cudaMallocAsync(&tab, sizeof(float4) * (size_t)nTiles * M_pad * TC, st));
+        NQS_CUDA(cudaMallocAsync(&rho, sizeof(float4) * (size_t)C_pad, st));
+        NQS_CUDA(cudaMallocAsync(&partial, sizeof(float2) * (size_t)B * nTiles, st));
+        NQS_PROF(0, st);
+        const long long total = (long long)M_pad * C_pad;
+        const unsigned tgrid = (unsigned)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
+        table_kernel<<<tgrid, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, h->C, TC, nTiles,
+                                            h->dev.col_i, h->dev.col_k, h->dev.col_p, tab, rho);
+        NQS_CUDA(cudaGetLastError());
+    }
+    if (have_cols) NQS_PROF(1, st);
+    if (have_cols || d_logpsi) {
+        rc = launch_theta(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st);
+        if (rc) return rc;
+    }
+    if (have_cols) {
+        NQS_PROF(2, st);
+        ElocParams p;
+        p.tp = tp;
+        p.nPairsPad = nPairsPad;
+        p.tab = tab;
+        p.rho = rho;
+        p.spins = d_spins;
+        p.B = B;
+        p.N = N;
+        p.M_pad = M_pad;
+        p.nTiles = nTiles;
+        p.H = h->dev;
+        p.partial = partial;
+        rc = launch_eloc(h, p, B_pad, st);
+        if (rc) return rc;
+        NQS_PROF(3, st);
+    }
+    finalize_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(d_spins, (long long)B, N, h->dev, partial,
+                                                                 have_cols ? nTiles : 0, (float2*)d_eloc);
+    NQS_CUDA(cudaGetLastError());
+    if (have_cols) {
+        NQS_PROF(4, st);
+        g_prof_valid = g_prof_on;
+        NQS_CUDA(cudaFreeAsync(tp, st));
+        NQS_CUDA(cudaFreeAsync(tab, st));
+        NQS_CUDA(cudaFreeAsync(rho, st));
+        NQS_CUDA(cudaFreeAsync(partial, st));
+    }
+    return NQS_OK;
+}
+
+extern "C" int nqs_local_energy(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
+                                const nqs_c64* d_b, const nqs_c64* d_W, int32_t T, const int32_t* h_sites,
+                                const uint8_t* h_paulis, const nqs_c64* h_coeffs, nqs_c64* d_eloc,
+                                nqs_c64* d_logpsi, void* stream) {
+    int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
+    if (rc) return rc;
+    if ((rc = check_device())) return rc;
+    nqs_hamiltonian* h = nullptr;
+    if ((rc = cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, &h))) return rc;
+    return nqs_local_energy_h(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream);
+}
+
+extern "C" int nqs_enumerate_connected(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B,
+                                       int8_t* d_sprime, nqs_c64* d_mel, void* stream) {
+    if (!h) return fail(NQS_ERR_INVALID_ARG, "hamiltonian handle is NULL");
+    if (B < 0 || (B > 0 && (!d_spins || !d_sprime || !d_mel))) return fail(NQS_ERR_INVALID_ARG, "bad arguments");
+    int rc = check_device();
+    if (rc) return rc;
+    if (h->device < 0) return fail(NQS_ERR_INVALID_ARG, "handle was compiled host-only");
+    if (B == 0) return NQS_OK;
+    const long long total = (long long)B * (h->dev.G + 1);
+    const unsigned grid = (unsigned)((total + 127) / 128 < 65535 ? (total + 127) / 128 : 65535);
+    enumerate_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(d_spins, (long long)B, h->hc.N, h->dev, d_sprime,
+                                                             (float2*)d_mel);
+    NQS_CUDA(cudaGetLastError());
+    return NQS_OK;
+}
+
+// ----------------------------------------------------------------------------------------
+// host-buffer entry points (end-to-end: H2D, kernels, D2H, synchronise)
+// ----------------------------------------------------------------------------------------
+struct HostStage {
+    cudaStream_t st = nullptr;
+    std::vector<void*> bufs;
+    ~HostStage() {
+        for (void* b : bufs) cudaFreeAsync(b, st);
+        if (st) {
+            cudaStreamSynchronize(st);
+            cudaStreamDestroy(st);
+        }
+    }
+    int init() {
+        NQS_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+        return NQS_OK;
+    }
+    int to_device(const void* h, size_t bytes, void** d) {
+        NQS_CUDA(cudaMallocAsync(d, bytes ? bytes : 16, st));
+        bufs.push_back(*d);
+        if (bytes) NQS_CUDA(cudaMemcpyAsync(*d, h, bytes, cudaMemcpyHostToDevice, st));
+        return NQS_OK;
+    }
+    int alloc(size_t bytes, void** d) {
+        NQS_CUDA(cudaMallocAsync(d, bytes ? bytes : 16, st));
+        bufs.push_back(*d);
+        return NQS_OK;
+    }
+};
+
+extern "C" int nqs_local_energy_host(const int8_t* h_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* h_a,
+                                     const nqs_c64* h_b, const nqs_c64* h_W, int32_t T, const int32_t* h_sites,
+                                     const uint8_t* h_paulis, const nqs_c64* h_coeffs, nqs_c64* h_eloc,
+                                     nqs_c64* h_logpsi) {
+    int rc = check_common(h_spins, B, N, M, h_a, h_b, h_W);
+    if (rc) return rc;
+    if (B > 0 && !h_eloc) return fail(NQS_ERR_INVALID_ARG, "h_eloc is NULL");
+    if ((rc = check_device())) return rc;
+    nqs_hamiltonian* h = nullptr;
+    if ((rc = cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, &h))) return rc;
+    if (B == 0) return NQS_OK;
+    HostStage S;
+    if ((rc = S.init())) return rc;
+    void *ds, *da, *db, *dW, *de, *dl = nullptr;
+    if ((rc = S.to_device(h_spins, (size_t)B * N, &ds))) return rc;
+    if ((rc = S.to_device(h_a, sizeof(nqs_c64) * N, &da))) return rc;
+    if ((rc = S.to_device(h_b, sizeof(nqs_c64) * M, &db))) return rc;
+    if ((rc = S.to_device(h_W, sizeof(nqs_c64) * (size_t)M * N, &dW))) return rc;
+    if ((rc = S.alloc(sizeof(nqs_c64) * B, &de))) return rc;
+    if (h_logpsi && (rc = S.alloc(sizeof(nqs_c64) * B, &dl))) return rc;
+    rc = nqs_local_energy_h(h, (const int8_t*)ds, B, M, (const nqs_c64*)da, (const nqs_c64*)db, (const nqs_c64*)dW,
+                            (nqs_c64*)de, (nqs_c64*)dl, S.st);
+    if (rc) return rc;
+    NQS_CUDA(cudaMemcpyAsync(h_eloc, de, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
+    if (h_logpsi) NQS_CUDA(cudaMemcpyAsync(h_logpsi, dl, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
+    NQS_CUDA(cudaStreamSynchronize(S.st));
+    return NQS_OK;
+}
+
+extern "C" int nqs_log_psi_host(const int8_t* h_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* h_a,
+                                const nqs_c64* h_b, const nqs_c64* h_W, nqs_c64* h_logpsi) {
+    int rc = check_common(h_spins, B, N, M, h_a, h_b, h_W);
+    if (rc) return rc;
+    if (B > 0 && !h_logpsi) return fail(NQS_ERR_INVALID_ARG, "h_logpsi is NULL");
+    if ((rc = check_device())) return rc;
+    if (B == 0) return NQS_OK;
+    HostStage S;
+    if ((rc = S.init())) return rc;
+    void *ds, *da, *db, *dW, *dl;
+    if ((rc = S.to_device(h_spins, (size_t)B * N, &ds))) return rc;
+    if ((rc = S.to_device(h_a, sizeof(nqs_c64) * N, &da))) return rc;
+    if ((rc = S.to_device(h_b, sizeof(nqs_c64) * M, &db))) return rc;
+    if ((rc = S.to_device(h_W, sizeof(nqs_c64) * (size_t)M * N, &dW))) return rc;
+    if ((rc = S.alloc(sizeof(nqs_c64) * B, &dl))) return rc;
+    rc = nqs_log_psi((const int8_t*)ds, B, N, M, (const nqs_c64*)da, (const nqs_c64*)db, (const nqs_c64*)dW,
+                     (nqs_c64*)dl, S.st);
+    if (rc) return rc;
+    NQS_CUDA(cudaMemcpyAsync(h_logpsi, dl, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
+    NQS_CUDA(cudaStreamSynchronize(S.st));
+    return NQS_OK;
+}

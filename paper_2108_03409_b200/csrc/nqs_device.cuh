@@ -1,0 +1,130 @@
+// Device-side data structures and math helpers shared by the kernels (sm_100a only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace nqs {
+
+// Device image of the compiled Hamiltonian (see nqs_hamiltonian.h).  All pointers are device
+// pointers into one allocation owned by the nqs_hamiltonian handle.
+struct DevHam {
+    int N, G, C, Td, Tg;
+    const int* diag_z0;
+    const int* diag_z1;
+    const float2* diag_c;
+    const int* grp_f0;
+    const int* grp_f1;
+    const int* grp_first;
+    const int* grp_count;
+    const int* gt_z0;
+    const int* gt_z1;
+    const float2* gt_c;
+    // columns, padded to C_pad entries (col_group = -1 marks padding)
+    const int* col_i;
+    const int* col_k;
+    const int* col_p;
+    const int* col_group;
+};
+
+__device__ __forceinline__ float2 bc2(float x) { return make_float2(x, x); }
+__device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
+
+// Summed matrix element of flip group g for the configuration `srow` (Eq. 39):
+// m = sum_{t in g} c'_t * s[z0_t] * s[z1_t]   (c' carries (-i)^{n_Y}; z = -1 means factor 1).
+__device__ __forceinline__ float2 group_element(const DevHam& H, const int8_t* __restrict__ srow, int g) {
+    const int first = H.grp_first[g], count = H.grp_count[g];
+    float mr = 0.f, mi = 0.f;
+    for (int q = 0; q < count; ++q) {
+        const int z0 = H.gt_z0[first + q], z1 = H.gt_z1[first + q];
+        float f = 1.f;
+        if (z0 >= 0) f *= (float)srow[z0];
+        if (z1 >= 0) f *= (float)srow[z1];
+        const float2 c = H.gt_c[first + q];
+        mr = fmaf(c.x, f, mr);
+        mi = fmaf(c.y, f, mi);
+    }
+    return make_float2(mr, mi);
+}
+
+// Sum of the diagonal terms (empty flip set): d = sum_t c_t * s[z0] * s[z1].
+__device__ __forceinline__ float2 diagonal_element(const DevHam& H, const int8_t* __restrict__ srow) {
+    float dr = 0.f, di = 0.f;
+    for (int t = 0; t < H.Td; ++t) {
+        const int z0 = H.diag_z0[t], z1 = H.diag_z1[t];
+        float f = 1.f;
+        if (z0 >= 0) f *= (float)srow[z0];
+        if (z1 >= 0) f *= (float)srow[z1];
+        const float2 c = H.diag_c[t];
+        dr = fmaf(c.x, f, dr);
+        di = fmaf(c.y, f, di);
+    }
+    return make_float2(dr, di);
+}
+
+// log cosh z and tanh z for z = x + i y, float32, written for accuracy at small |z| (the
+// log psi tolerance is 1e-5 absolute on a sum of M terms) and stability at large |x|.
+//   |cosh z|^2 = cosh^2 x - sin^2 y = 1 + (sinh^2 x - sin^2 y)
+//   arg cosh z = atan2(tanh x sin y, cos y)            (principal value per hidden unit, Q6)
+//   tanh z     = [tanh x + i sin y cos y sech^2 x] / (cos^2 y + tanh^2 x sin^2 y)
+__device__ __forceinline__ void lncosh_tanh(float x, float y, float& lr, float& li, float& tr, float& ti) {
+    const float ax = fabsf(x);
+    float s, c;
+    sincosf(y, &s, &c);
+    float th, sech2;
+    if (ax < 4.0f) {
+        const float sh = sinhf(x);
+        const float ch2 = fmaf(sh, sh, 1.0f);
+        th = sh * rsqrtf(ch2);
+        sech2 = 1.0f / ch2;
+        // |cosh z|^2 = 1 + (sinh^2 x - sin^2 y) = sinh^2 x + cos^2 y: the first form keeps relative
+        // accuracy at small |z|, the second near the zeros of cosh (y -> pi/2, x -> 0)
+        const float s2 = s * s;
+        lr = (s2 > 0.5f) ? 0.5f * logf(fmaf(sh, sh, c * c)) : 0.5f * log1pf(fmaf(sh, sh, -s2));
+    } else {
+        const float q = expf(-2.0f * ax);  // <= 3.4e-4
+        const float d = 1.0f + q;
+        th = copysignf((1.0f - q) / d, x);
+        sech2 = 4.0f * q / (d * d);
+        const float cos2y2 = 2.0f * (c * c - s * s);
+        lr = ax - 0.69314718055994531f + 0.5f * log1pf(q * (cos2y2 + q));
+    }
+    li = atan2f(th * s, c);
+    const float D = fmaf(c, c, th * th * s * s);
+    const float inv = 1.0f / D;
+    tr = th * inv;
+    ti = s * c * sech2 * inv;
+}
+
+// ---- mbarrier / bulk-copy (TMA engine, non-tensor) helpers: PTX for sm_90+/sm_100a ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// global -> shared bulk copy, completion signalled on an mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+}  // namespace nqs
