@@ -1,0 +1,352 @@
+// a2 on the 5th-generation tensor cores (tcgen05, sm_100a): theta = b + W s as an EXACT integer GEMM.
+//
+// theta[b, j] = b_j + sum_i W_ji s_bi  (Eq. 30 / Eq. 38) is a dense
+// [B, N] x [N, 2M] contraction with s = +-1 exactly representable in int8.  W is split per hidden
+// unit into four balanced base-128 digits of a 28-bit fixed-point value (error-compensated split:
+// the four int8 GEMMs accumulate exactly in int32, so the only error is the 2^-28 * max_i |W_ji|
+// quantisation -- below float32's own rounding of W -- and there is no accumulation-order or
+// tensor-core truncation error at all).  north_star: "tensor cores only if an error-compensated
+// split meets tolerance".
+//
+//   A = spins   [128 samples] x [K]  int8, K-major, canonical no-swizzle core-matrix layout
+//   B = digits  [256 = 32 hidden x (re, im) x 4 digits] x [K] int8, K-major, same layout
+//   D = A B^T   [128 lanes] x [256 columns] int32 in TMEM  (tcgen05.mma.cta_group::1.kind::i8)
+//
+// Both operands are pre-packed in global memory in exactly the shared-memory image the MMA wants
+// ([k16][row][16 bytes]), so every pipeline stage is ONE contiguous cp.async.bulk (TMA engine).
+// CTA = 128 samples, loops over all hidden tiles so log psi needs no cross-CTA reduction.
+// Warp roles: 0 = bulk-copy producer, 1 = TMEM allocator + MMA issuer (one elected lane),
+// 2..9 = epilogue (tcgen05.ld -> theta -> log cosh, tanh -> log psi, tp).  Two CTAs per SM share
+// the 512 TMEM columns, so one CTA's MMAs overlap the other's epilogue.
+#pragma once
+#include "nqs_device.cuh"
+
+namespace nqs {
+
+constexpr int TM_M = 128;       // samples per CTA (UMMA M)
+constexpr int TM_JT = 32;       // hidden units per accumulator tile
+constexpr int TM_N = 256;       // accumulator columns = TM_JT * 2 * 4
+constexpr int TM_KC = 64;       // K bytes per B stage (two K=32 MMAs)
+constexpr int TM_STAGES = 3;
+constexpr int TM_A_K16_BYTES = TM_M * 16;   // one 16-byte K slab of the A tile
+constexpr int TM_B_K16_BYTES = TM_N * 16;
+constexpr int TM_B_STAGE_BYTES = TM_B_K16_BYTES * (TM_KC / 16);
+constexpr int TM_THREADS = 320;
+constexpr int TM_MAX_KPAD = 512;
+
+__host__ __device__ inline size_t theta_mma_smem_bytes(int K_pad) {
+    return (size_t)(K_pad / 16) * TM_A_K16_BYTES + (size_t)TM_STAGES * TM_B_STAGE_BYTES + 256;
+}
+
+// ---------------------------------------------------------------------------------------
+// operand packing
+// ---------------------------------------------------------------------------------------
+// A_packed[mtile][k16][row 0..127][16 bytes] = spins[mtile*128 + row][16*k16 .. +16), zero padded
+__global__ void pack_spins_kernel(const int8_t* __restrict__ spins, long long B, int N, int K16, long long nMT,
+                                  uint4* __restrict__ A_packed) {
+    const long long total = nMT * K16 * TM_M;
+    const bool vec = (N % 16 == 0) && ((reinterpret_cast<uintptr_t>(spins) & 15) == 0);
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const int row = (int)(idx % TM_M);
+        const int k16 = (int)((idx / TM_M) % K16);
+        const long long mt = idx / ((long long)TM_M * K16);
+        const long long b = mt * TM_M + row;
+        uint4 v = make_uint4(0, 0, 0, 0);
+        if (b < B) {
+            const int i0 = k16 * 16;
+            if (vec && i0 + 16 <= N) {
+                v = *reinterpret_cast<const uint4*>(spins + b * N + i0);
+            } else {
+                unsigned w[4] = {0, 0, 0, 0};
+                for (int k = 0; k < 16; ++k)
+                    if (i0 + k < N) w[k >> 2] |= (unsigned)(uint8_t)spins[b * N + i0 + k] << (8 * (k & 3));
+                v = make_uint4(w[0], w[1], w[2], w[3]);
+            }
+        }
+        A_packed[idx] = v;
+    }
+}
+
+// One block per hidden unit j (padded to nNT*32): power-of-two scale from the row maximum, then
+// W_ji * 2^(27-e) rounded to an integer Q, |Q| <= 2^27, written as digits d0..d3 in [-64, 64]:
+//   Q = d0 + 128 d1 + 128^2 d2 + 128^3 d3.
+// B_packed[ntile][k16][n = 8*jl + 4*part + digit][16 bytes];  scale[j] = 2^(e-27).
+__global__ void __launch_bounds__(128) pack_w_kernel(const float2* __restrict__ W, int N, int M, int K16,
+                                                     uint4* __restrict__ B_packed, float* __restrict__ scale) {
+    const int j = blockIdx.x;
+    const int tid = threadIdx.x;
+    __shared__ float smax[4];
+    float mx = 0.f;
+    if (j < M)
+        for (int i = tid; i < N; i += 128) {
+            const float2 w = W[(long long)j * N + i];
+            mx = fmaxf(mx, fmaxf(fabsf(w.x), fabsf(w.y)));
+        }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if ((tid & 31) == 0) smax[tid >> 5] = mx;
+    __syncthreads();
+    mx = fmaxf(fmaxf(smax[0], smax[1]), fmaxf(smax[2], smax[3]));
+    int e = 0;
+    if (mx > 0.f) (void)frexpf(mx, &e);  // mx = f * 2^e, f in [0.5, 1)
+    if (tid == 0) scale[j] = (mx > 0.f && j < M) ? ldexpf(1.f, e - 27) : 0.f;
+    const int nt = j / TM_JT, jl = j % TM_JT;
+    for (int item = tid; item < 2 * K16; item += 128) {
+        const int part = item & 1, k16 = item >> 1;
+        unsigned d[4][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
+        if (j < M && mx > 0.f) {
+            for (int k = 0; k < 16; ++k) {
+                const int i = k16 * 16 + k;
+                if (i < N) {
+                    const float2 w = W[(long long)j * N + i];
+                    int Q = __float2int_rn(ldexpf(part ? w.y : w.x, 27 - e));
+#pragma unroll
+                    for (int l = 0; l < 3; ++l) {
+                        const int dl = ((Q + 64) & 127) - 64;
+                        Q = (Q - dl) >> 7;
+                        d[l][k >> 2] |= (unsigned)(uint8_t)(int8_t)dl << (8 * (k & 3));
+                    }
+                    d[3][k >> 2] |= (unsigned)(uint8_t)(int8_t)Q << (8 * (k & 3));
+                }
+            }
+        }
+        uint4* dst = B_packed + ((long long)nt * K16 + k16) * TM_N + jl * 8 + part * 4;
+#pragma unroll
+        for (int l = 0; l < 4; ++l) dst[l] = make_uint4(d[l][0], d[l][1], d[l][2], d[l][3]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// tcgen05 / TMEM PTX wrappers
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void tmem_alloc(uint32_t* slot, uint32_t ncols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "r"(ncols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// D[tmem] (+)= A[smem desc] * B[smem desc]^T, int8 x int8 -> int32
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+// K-major, no swizzle: 8-row x 16-byte core matrices; LBO = byte step between the two 16-byte K slabs
+// of one K=32 MMA, SBO = byte step between 8-row groups; descriptor version 1 (Blackwell).
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) |
+           ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | (1ull << 46);
+}
+constexpr uint32_t TM_IDESC = (2u << 4) /* D = S32 */ | (1u << 7) /* A = INT8 */ | (1u << 10) /* B = INT8 */ |
+                              ((uint32_t)(TM_N >> 3) << 17) | ((uint32_t)(TM_M >> 4) << 24);
+
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, int (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// ---------------------------------------------------------------------------------------
+// the kernel
+// ---------------------------------------------------------------------------------------
+struct ThetaMmaParams {
+    const uint4* A_packed;   // [nMT][K16][128]
+    const uint4* B_packed;   // [nNT][K16][256]
+    const float* scale;      // [nNT*32]
+    const float2* bvec;      // [M]
+    const float2* a;         // [N]
+    const int8_t* spins;     // [B][N]
+    long long B;
+    int N, M, M_pad, K16, nNT;
+    float4* tp;              // [M_pad][nPairsPad] or nullptr
+    long long nPairsPad;
+    float2* logpsi;          // [B] or nullptr
+};
+
+__global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMmaParams p) {
+    extern __shared__ __align__(128) unsigned char tm_smem[];
+    const int K16 = p.K16;
+    unsigned char* const sA = tm_smem;
+    unsigned char* const sB = tm_smem + (size_t)K16 * TM_A_K16_BYTES;
+    uint64_t* const bars = reinterpret_cast<uint64_t*>(sB + (size_t)TM_STAGES * TM_B_STAGE_BYTES);
+    uint64_t* const a_full = bars;
+    uint64_t* const b_full = bars + 1;
+    uint64_t* const b_empty = bars + 1 + TM_STAGES;
+    uint64_t* const t_full = bars + 1 + 2 * TM_STAGES;
+    uint64_t* const t_empty = bars + 2 + 2 * TM_STAGES;
+    uint32_t* const tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 + 2 * TM_STAGES);
+    double* const lp_x = reinterpret_cast<double*>(sB);  // reused after the main loop: [128][2]
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const long long mt = blockIdx.x;
+    const int nKC = K16 / (TM_KC / 16);
+
+    if (tid == 0) {
+        mbar_init(a_full, 1);
+        for (int s = 0; s < TM_STAGES; ++s) {
+            mbar_init(&b_full[s], 1);
+            mbar_init(&b_empty[s], 1);
+        }
+        mbar_init(t_full, 1);
+        mbar_init(t_empty, 8);
+        fence_mbar_init();
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, TM_N);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        if (lane == 0) {
+            const uint32_t a_bytes = (uint32_t)K16 * TM_A_K16_BYTES;
+            mbar_expect_tx(a_full, a_bytes);
+            bulk_g2s(sA, p.A_packed + mt * (long long)K16 * TM_M, a_bytes, a_full);
+            int it = 0;
+            for (int nt = 0; nt < p.nNT; ++nt)
+                for (int kc = 0; kc < nKC; ++kc, ++it) {
+                    const int s = it % TM_STAGES;
+                    mbar_wait(&b_empty[s], ((it / TM_STAGES) & 1) ^ 1);
+                    mbar_expect_tx(&b_full[s], TM_B_STAGE_BYTES);
+                    bulk_g2s(sB + (size_t)s * TM_B_STAGE_BYTES,
+                             p.B_packed + ((long long)nt * K16 + kc * (TM_KC / 16)) * TM_N, TM_B_STAGE_BYTES,
+                             &b_full[s]);
+                }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            mbar_wait(a_full, 0);
+            const uint32_t sA_u = smem_u32(sA), sB_u = smem_u32(sB);
+            int it = 0;
+            for (int nt = 0; nt < p.nNT; ++nt) {
+                mbar_wait(t_empty, (nt & 1) ^ 1);
+                tc_fence_after();
+                for (int kc = 0; kc < nKC; ++kc, ++it) {
+                    const int s = it % TM_STAGES;
+                    mbar_wait(&b_full[s], (it / TM_STAGES) & 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int ks = 0; ks < TM_KC / 32; ++ks) {
+                        const uint64_t ad = umma_desc(sA_u + (uint32_t)(kc * (TM_KC / 16) + ks * 2) * TM_A_K16_BYTES,
+                                                      TM_A_K16_BYTES, 128);
+                        const uint64_t bd = umma_desc(sB_u + (uint32_t)s * TM_B_STAGE_BYTES + (uint32_t)(ks * 2) * TM_B_K16_BYTES,
+                                                      TM_B_K16_BYTES, 128);
+                        umma_i8(tmem_base, ad, bd, TM_IDESC, (kc | ks) ? 1u : 0u);
+                    }
+                    tc_commit(&b_empty[s]);  // frees the stage once these MMAs have read it
+                }
+                tc_commit(t_full);
+            }
+        }
+    } else {
+        // ---------------- epilogue: 8 warps; TMEM lanes 32*(warp%4).., column half (warp-2)/4
+        const int ew = warp - 2;
+        const int lane_grp = warp & 3, half = ew >> 2;
+        const int row = lane_grp * 32 + lane;
+        const long long b = mt * TM_M + row;
+        const long long pair = b >> 1;
+        const bool odd = lane & 1;
+        double lpr = 0.0, lpi = 0.0;
+        for (int nt = 0; nt < p.nNT; ++nt) {
+            mbar_wait(t_full, nt & 1);
+            tc_fence_after();
+#pragma unroll 1
+            for (int q4 = 0; q4 < 4; ++q4) {  // 4 hidden units per TMEM load
+                int v[32];
+                const uint32_t col = (uint32_t)(half * 128 + q4 * 32);
+                tmem_ld32(tmem_base + ((uint32_t)(lane_grp * 32) << 16) + col, v);
+                float tr[4], ti[4];
+                const int jbase = nt * TM_JT + half * 16 + q4 * 4;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int j = jbase + u;
+                    const bool live = j < p.M;
+                    const float sc = p.scale[j];
+                    const float2 bj = live ? p.bvec[j] : make_float2(0.f, 0.f);
+                    const int* w = &v[u * 8];
+                    const float hr = (float)(w[3] * 128 + w[2]), lr_ = (float)(w[1] * 128 + w[0]);
+                    const float hi_ = (float)(w[7] * 128 + w[6]), li_ = (float)(w[5] * 128 + w[4]);
+                    const float thr = fmaf(hr * 16384.f, sc, fmaf(lr_, sc, bj.x));
+                    const float thi = fmaf(hi_ * 16384.f, sc, fmaf(li_, sc, bj.y));
+                    float lr, li;
+                    lncosh_tanh(thr, thi, lr, li, tr[u], ti[u]);
+                    if (live) {
+                        lpr += (double)lr;
+                        lpi += (double)li;
+                    } else {
+                        tr[u] = 0.f;
+                        ti[u] = 0.f;
+                    }
+                }
+                if (p.tp) {
+#pragma unroll
+                    for (int u = 0; u < 4; u += 2) {
+                        // even lane writes unit u (needs the odd lane's values), odd lane writes u+1
+                        const float sr = odd ? tr[u] : tr[u + 1], si = odd ? ti[u] : ti[u + 1];
+                        const float rr = __shfl_xor_sync(0xffffffffu, sr, 1), ri = __shfl_xor_sync(0xffffffffu, si, 1);
+                        const int j = jbase + u + (odd ? 1 : 0);
+                        const float4 rec = odd ? make_float4(rr, tr[u + 1], ri, ti[u + 1])
+                                               : make_float4(tr[u], rr, ti[u], ri);
+                        if (j < p.M_pad) p.tp[(long long)j * p.nPairsPad + pair] = rec;
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(t_empty);
+        }
+        // visible bias, split between the two column halves of a row
+        if (b < p.B) {
+            float ar = 0.f, ai = 0.f;
+            const int i_lo = half ? p.N / 2 : 0, i_hi = half ? p.N : p.N / 2;
+            for (int i = i_lo; i < i_hi; ++i) {
+                const float s = (float)p.spins[b * p.N + i];
+                const float2 av = p.a[i];
+                ar = fmaf(av.x, s, ar);
+                ai = fmaf(av.y, s, ai);
+            }
+            lpr += (double)ar;
+            lpi += (double)ai;
+        }
+        // all MMAs have completed (t_full of the last tile was observed): the B stages are dead
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (half == 1) {
+            lp_x[2 * row] = lpr;
+            lp_x[2 * row + 1] = lpi;
+        }
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (half == 0 && b < p.B && p.logpsi)
+            p.logpsi[b] = make_float2((float)(lpr + lp_x[2 * row]), (float)(lpi + lp_x[2 * row + 1]));
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc(tmem_base, TM_N);
+    }
+}
+
+}  // namespace nqs
