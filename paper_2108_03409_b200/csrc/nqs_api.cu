@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <list>
 #include <mutex>
@@ -12,6 +13,7 @@
 #include "../../include/nqs.h"
 #include "nqs_hamiltonian.h"
 #include "nqs_kernels.cuh"
+#include "nqs_theta_mma.cuh"
 
 using namespace nqs;
 
@@ -293,9 +295,9 @@ static int check_device() {
 
 static inline long long round_up(long long x, long long m) { return (x + m - 1) / m * m; }
 
-static int launch_theta(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
-                        const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad, nqs_c64* d_logpsi,
-                        cudaStream_t st) {
+static int launch_theta_simt(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
+                             const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad,
+                             nqs_c64* d_logpsi, cudaStream_t st) {
     const long long rows = tp ? nPairsPad * 2 : B;
     const unsigned grid = (unsigned)((rows + 63) / 64);
     static bool attr_set = false;
@@ -307,6 +309,72 @@ static int launch_theta(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, 
                                        (const float2*)d_W, tp, nPairsPad, (float2*)d_logpsi);
     NQS_CUDA(cudaGetLastError());
     return NQS_OK;
+}
+
+// a2 on the tensor cores: pack spins and the int8 digits of W, then theta_mma_kernel (tcgen05).
+static int launch_theta_mma(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
+                            const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad,
+                            nqs_c64* d_logpsi, cudaStream_t st) {
+    const long long rows = tp ? nPairsPad * 2 : B;
+    const long long nMT = (rows + TM_M - 1) / TM_M;
+    const int K_pad = (int)round_up(N, TM_KC), K16 = K_pad / 16;
+    const int nNT = (M_pad + TM_JT - 1) / TM_JT;
+    uint4 *A_packed = nullptr, *B_packed = nullptr;
+    float* scale = nullptr;
+    NQS_CUDA(cudaMallocAsync(&A_packed, sizeof(uint4) * (size_t)nMT * K16 * TM_M, st));
+    NQS_CUDA(cudaMallocAsync(&B_packed, sizeof(uint4) * (size_t)nNT * K16 * TM_N, st));
+    NQS_CUDA(cudaMallocAsync(&scale, sizeof(float) * (size_t)nNT * TM_JT, st));
+    const long long a_items = nMT * K16 * TM_M;
+    const unsigned agrid = (unsigned)((a_items + 255) / 256 < 148 * 16 ? (a_items + 255) / 256 : 148 * 16);
+    pack_spins_kernel<<<agrid, 256, 0, st>>>(d_spins, (long long)B, N, K16, nMT, A_packed);
+    NQS_CUDA(cudaGetLastError());
+    pack_w_kernel<<<(unsigned)(nNT * TM_JT), 128, 0, st>>>((const float2*)d_W, N, M, K16, B_packed, scale);
+    NQS_CUDA(cudaGetLastError());
+    const size_t smem = theta_mma_smem_bytes(K_pad);
+    static size_t attr_smem = 0;
+    if (smem > attr_smem) {
+        NQS_CUDA(cudaFuncSetAttribute(theta_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_smem = smem;
+    }
+    ThetaMmaParams p;
+    p.A_packed = A_packed;
+    p.B_packed = B_packed;
+    p.scale = scale;
+    p.bvec = (const float2*)d_b;
+    p.a = (const float2*)d_a;
+    p.spins = d_spins;
+    p.B = B;
+    p.N = N;
+    p.M = M;
+    p.M_pad = M_pad;
+    p.K16 = K16;
+    p.nNT = nNT;
+    p.tp = tp;
+    p.nPairsPad = nPairsPad;
+    p.logpsi = (float2*)d_logpsi;
+    theta_mma_kernel<<<(unsigned)nMT, TM_THREADS, smem, st>>>(p);
+    NQS_CUDA(cudaGetLastError());
+    NQS_CUDA(cudaFreeAsync(A_packed, st));
+    NQS_CUDA(cudaFreeAsync(B_packed, st));
+    NQS_CUDA(cudaFreeAsync(scale, st));
+    return NQS_OK;
+}
+
+// NQS_THETA=simt forces the FP32 SIMT kernel (A/B comparisons); the tensor-core kernel covers N <= 512.
+static bool theta_use_mma(int32_t N) {
+    static const bool force_simt = [] {
+        const char* e = getenv("NQS_THETA");
+        return e && strcmp(e, "simt") == 0;
+    }();
+    return !force_simt && round_up(N, TM_KC) <= TM_MAX_KPAD;
+}
+
+static int launch_theta(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
+                        const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad, nqs_c64* d_logpsi,
+                        cudaStream_t st) {
+    if (theta_use_mma(N))
+        return launch_theta_mma(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st);
+    return launch_theta_simt(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st);
 }
 
 template <int WC, int WS>
