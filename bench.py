@@ -33,7 +33,7 @@ FP32_LANES_PER_SM = 128
 L2_FLUSH_BYTES = 256 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum of one eloc_kernel launch at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-ELOC_KERNEL_DRAM_TRAFFIC_BYTES = None
+ELOC_KERNEL_DRAM_TRAFFIC_BYTES = 891_420_160  # profiles/r1_v2_ncu_summary.md
 
 
 def shard_plan(n_ranks: int, rank: int, config: int) -> dict:
@@ -291,7 +291,7 @@ def run_ours(args) -> None:
             "clocks": {k: clocks[k] for k in ("sm_mhz", "sm_max_mhz", "reasons")},
             "e2e": {"value": plan["global_batch"] / e2e_s, "unit": "samples/s", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
-            "gpu_launches": 4 * args.steps,
+            "gpu_launches": 6 * args.steps,  # table, pack_spins, pack_w, theta_mma, eloc, finalize
         }
         if world == 1 and not args.no_cpu_baseline:
             cb, _, _ = cpu_baseline(w)
