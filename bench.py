@@ -293,6 +293,15 @@ def run_ours(args) -> None:
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": 6 * args.steps,  # table, pack_spins, pack_w, theta_mma, eloc, finalize
         }
+        # pipe rates measured on this box (nqs_microbench; register-only kernels, after the timed region)
+        mb = {k: nqs.microbench(k)["lane_ops_per_s"] for k in nqs.MICROBENCH_KINDS}
+        line["measured_peaks"] = {
+            "ffma_tflops": 2 * mb["ffma"] / 1e12, "ffma2_tflops": 2 * mb["ffma2"] / 1e12,
+            "a5_body_packed_tflops": 2 * mb["a5_body_packed"] / 1e12,
+            "a5_body_scalar_tflops": 2 * mb["a5_body_scalar"] / 1e12,
+            "mufu_ex2_gops": mb["mufu_ex2"] / 1e9,
+            "how": "nqs_microbench: 2 x 320 threads per SM, operands in registers, best of 3; FMA = 2 flop"}
+        line["roofline"]["frac_of_measured_ffma"] = achieved / (2 * max(mb["ffma"], mb["ffma2"]) / 1e12)
         if world == 1 and not args.no_cpu_baseline:
             cb, _, _ = cpu_baseline(w)
             line["cpu_baseline"] = cb

@@ -141,6 +141,19 @@ int nqs_enumerate_connected(const nqs_hamiltonian *h, const int8_t *d_spins, int
 int nqs_profile_enable(int on);
 int nqs_profile_last(float ms[4]);
 
+/* Pipe-rate micro-benchmark (the roofline is quoted against the nominal peak
+ * AND a peak measured on the box).  Runs a register-only kernel (2 blocks of 320 threads per SM,
+ * no memory traffic in the loop) `iters` iterations, best of 3 after one warm-up, on a private
+ * stream; synchronous.  kind:
+ *   0 scalar FFMA              (16 lane-FMAs per thread-iteration)
+ *   1 FFMA2 (fma.rn.f32x2)     (16 lane-FMAs)
+ *   2 the a5 inner-loop body, packed FFMA2 form, operands in registers (64 lane-FMAs)
+ *   3 the same body as scalar FFMA (64 lane-FMAs)
+ *   4 MUFU.EX2                 (8 lane-ops)
+ * *lane_ops_per_s receives thread-level operations per second summed over the GPU (one FMA = one
+ * operation); ms_out (may be NULL) the kernel time. */
+int nqs_microbench(int32_t kind, int32_t iters, double *lane_ops_per_s, float *ms_out);
+
 /* Thread-local message of the last error on this thread ("" if none). */
 const char *nqs_last_error(void);
 

@@ -7,6 +7,7 @@ CUDA device the calls raise.
 """
 from .binding import (  # noqa: F401
     Hamiltonian,
+    MICROBENCH_KINDS,
     NqsError,
     enumerate_connected,
     hamiltonian_info_host,
@@ -17,6 +18,7 @@ from .binding import (  # noqa: F401
     local_energy_host,
     log_psi,
     log_psi_host,
+    microbench,
     profile_enable,
     profile_last,
     release,

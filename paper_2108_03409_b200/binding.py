@@ -54,7 +54,7 @@ def load_library() -> ctypes.CDLL:
             for name in ("nqs_log_psi", "nqs_local_energy", "nqs_local_energy_host", "nqs_log_psi_host",
                          "nqs_hamiltonian_create", "nqs_hamiltonian_compile_host", "nqs_hamiltonian_destroy",
                          "nqs_hamiltonian_info", "nqs_local_energy_h", "nqs_enumerate_connected", "nqs_release",
-                         "nqs_profile_enable", "nqs_profile_last"):
+                         "nqs_profile_enable", "nqs_profile_last", "nqs_microbench"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -81,6 +81,16 @@ def profile_last() -> dict:
     ms = (ctypes.c_float * 4)()
     _check(load_library().nqs_profile_last(ms))
     return dict(table=ms[0], theta=ms[1], eloc=ms[2], finalize=ms[3])
+
+
+MICROBENCH_KINDS = {"ffma": 0, "ffma2": 1, "a5_body_packed": 2, "a5_body_scalar": 3, "mufu_ex2": 4}
+
+
+def microbench(kind: str, iters: int = 20000) -> dict:
+    """nqs_microbench: measured pipe rate (lane-operations per second over the whole GPU)."""
+    rate, ms = ctypes.c_double(), ctypes.c_float()
+    _check(load_library().nqs_microbench(MICROBENCH_KINDS[kind], iters, ctypes.byref(rate), ctypes.byref(ms)))
+    return dict(kind=kind, lane_ops_per_s=rate.value, ms=ms.value)
 
 
 def _check(rc: int) -> None:

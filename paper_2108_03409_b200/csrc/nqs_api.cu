@@ -13,6 +13,7 @@
 #include "../../include/nqs.h"
 #include "nqs_hamiltonian.h"
 #include "nqs_kernels.cuh"
+#include "nqs_microbench.cuh"
 #include "nqs_theta_mma.cuh"
 
 using namespace nqs;
@@ -604,5 +605,55 @@ extern "C" int nqs_log_psi_host(const int8_t* h_spins, int64_t B, int32_t N, int
     if (rc) return rc;
     NQS_CUDA(cudaMemcpyAsync(h_logpsi, dl, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
     NQS_CUDA(cudaStreamSynchronize(S.st));
+    return NQS_OK;
+}
+
+// ----------------------------------------------------------------------------------------
+// pipe-rate micro-benchmarks (measured peaks for the roofline)
+// ----------------------------------------------------------------------------------------
+template <int KIND>
+static void launch_microbench(float* out, unsigned grid, int iters, cudaStream_t st) {
+    microbench_kernel<KIND><<<grid, 320, 0, st>>>(out, iters, 1e-3f, 0.999f);
+}
+
+extern "C" int nqs_microbench(int32_t kind, int32_t iters, double* lane_ops_per_s, float* ms_out) {
+    if (kind < 0 || kind >= MB_KINDS || iters <= 0 || !lane_ops_per_s)
+        return fail(NQS_ERR_INVALID_ARG, "nqs_microbench: bad kind / iters / NULL output");
+    int rc = check_device();
+    if (rc) return rc;
+    int dev = 0, sms = 0;
+    NQS_CUDA(cudaGetDevice(&dev));
+    NQS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const unsigned grid = 2u * (unsigned)sms;
+    float* out = nullptr;
+    cudaStream_t st = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    NQS_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    NQS_CUDA(cudaMalloc(&out, sizeof(float) * (size_t)grid * 320));
+    NQS_CUDA(cudaEventCreate(&e0));
+    NQS_CUDA(cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {  // first repetition warms up; best of the rest
+        NQS_CUDA(cudaEventRecord(e0, st));
+        switch (kind) {
+            case MB_FFMA: launch_microbench<MB_FFMA>(out, grid, iters, st); break;
+            case MB_FFMA2: launch_microbench<MB_FFMA2>(out, grid, iters, st); break;
+            case MB_BODY_PACKED: launch_microbench<MB_BODY_PACKED>(out, grid, iters, st); break;
+            case MB_BODY_SCALAR: launch_microbench<MB_BODY_SCALAR>(out, grid, iters, st); break;
+            default: launch_microbench<MB_MUFU_EX2>(out, grid, iters, st); break;
+        }
+        NQS_CUDA(cudaGetLastError());
+        NQS_CUDA(cudaEventRecord(e1, st));
+        NQS_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        NQS_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    cudaStreamDestroy(st);
+    *lane_ops_per_s = (double)grid * 320.0 * iters * mb_ops_per_iter(kind) / (best * 1e-3);
+    if (ms_out) *ms_out = best;
     return NQS_OK;
 }
