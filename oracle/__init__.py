@@ -7,10 +7,13 @@ imports the product.  See oracle/nqs_oracle.c for what is computed and the citat
 from .oracle import (  # noqa: F401
     build,
     connected,
+    forces,
     lncosh,
     local_energy_definition,
     local_energy_fast,
+    log_derivatives,
     log_psi,
+    mean_variance,
     num_threads,
     set_num_threads,
 )

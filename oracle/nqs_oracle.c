@@ -30,7 +30,9 @@
  * Parity pins: see tests/test_oracle_pins.py (P1 dense H brute force, P2 Eq. 2-3 identity,
  * P3 zero parameters closed form, P4 product eigenstate, P5 singlet, P6 spin-flip symmetry,
  * P7 Pfeuty closed form for the dense-H builder, P8 definition<->fast, P9 log cosh special
- * cases).  No function here is "parity unpinned".
+ * cases; PF1 log-derivatives against finite differences of log psi, PF2 force vector against
+ * finite differences of the dense <H>, PF3 mean / variance against numpy and Eq. 3).
+ * No function here is "parity unpinned".
  */
 #include <complex.h>
 #include <math.h>
@@ -284,6 +286,121 @@ void oracle_connected(const int8_t *spins, int64_t B, int N, int T, const int32_
             mel[2 * (n * T + t) + 1] = cimag(m);
         }
     }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * batch statistics, logarithmic derivatives, force vector.
+ * Parameter order k = 0..K-1, K = N + M + M*N:  a_i (k = i), b_j (k = N + j),
+ * W_ji (k = N + M + j*N + i).  Weights w_b >= 0 are optional (NULL = uniform): with
+ * w_b = p(s_b) over the full basis they turn the sample mean of Eq. 5 into the exact
+ * expectation of Eq. 3.  They are normalised by their own sum.
+ * ------------------------------------------------------------------------------------- */
+
+/* Eq. 5 (:70-73) / Eq. 3: mean = sum_b w_b x_b / sum_b w_b and the variance
+ * <<|x - mean|^2>> (:511-515 get_global_mean / get_global_variance).
+ * x [B] complex128; out = {Re mean, Im mean, variance, sum of weights}. */
+void oracle_mean_variance(const double *x_re_im, const double *w, int64_t B, double out[4]) {
+    double sw = 0.0;
+    cplx sx = 0.0;
+    for (int64_t n = 0; n < B; ++n) {
+        const double wn = w ? w[n] : 1.0;
+        sw += wn;
+        sx += wn * (x_re_im[2 * n] + I * x_re_im[2 * n + 1]);
+    }
+    const cplx mean = sx / sw;
+    double var = 0.0;
+    for (int64_t n = 0; n < B; ++n) {
+        const double wn = w ? w[n] : 1.0;
+        const cplx d = (x_re_im[2 * n] + I * x_re_im[2 * n + 1]) - mean;
+        var += wn * (creal(d) * creal(d) + cimag(d) * cimag(d));
+    }
+    out[0] = creal(mean);
+    out[1] = cimag(mean);
+    out[2] = var / sw;
+    out[3] = sw;
+}
+
+/* Eq. 8 (:93): O_k(s) = d log psi(s) / d theta_k for the RBM of Eq. 38 (complex derivative,
+ * holomorphic ansatz :126, :299):  O_{a_i} = s_i,  O_{b_j} = tanh(theta_j),
+ * O_{W_ji} = tanh(theta_j) s_i,  theta_j = b_j + sum_i W_ji s_i.  tanh from libm (ctanh). */
+static void log_derivatives_one(const int8_t *s, int N, int M, const float *b, const float *W, cplx *O) {
+    for (int i = 0; i < N; ++i) O[i] = (double)s[i];
+    for (int j = 0; j < M; ++j) {
+        cplx theta = c64(b, j);
+        for (int i = 0; i < N; ++i) theta += c64(W, (int64_t)j * N + i) * (double)s[i];
+        const cplx t = ctanh(theta);
+        O[N + j] = t;
+        for (int i = 0; i < N; ++i) O[N + M + (int64_t)j * N + i] = t * (double)s[i];
+    }
+}
+
+/* out_O [B,K] complex128 (small inputs only: B*K*16 bytes) */
+void oracle_log_derivatives(const int8_t *spins, int64_t B, int N, int M, const float *a, const float *b,
+                            const float *W, double *out_O) {
+    (void)a;
+    const int64_t K = (int64_t)N + M + (int64_t)M * N;
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < B; ++n) log_derivatives_one(spins + n * N, N, M, b, W, (cplx *)(out_O + 2 * n * K));
+}
+
+/* Eq. 16 (:134-138), Eq. 7 (:81-89): F_k = <<E_loc O_k^*>>^c = <<O_k^* E_loc>> - <<O_k^*>> <<E_loc>>,
+ * the connected correlation written out as its two terms.  eloc [B] complex128 is an INPUT
+ * (any estimator values).  out_F [K] complex128.  Never materialises O [B,K]. */
+void oracle_forces(const int8_t *spins, int64_t B, int N, int M, const float *a, const float *b, const float *W,
+                   const double *eloc_re_im, const double *w, double *out_F) {
+    (void)a;
+    const int64_t K = (int64_t)N + M + (int64_t)M * N;
+    int nthreads = 1;
+#ifdef _OPENMP
+    nthreads = omp_get_max_threads();
+#endif
+    cplx *OE = calloc((size_t)K * nthreads, sizeof(cplx)); /* per-thread sum_b w_b O_k^* E_b */
+    cplx *Oc = calloc((size_t)K * nthreads, sizeof(cplx)); /* per-thread sum_b w_b O_k^*     */
+    cplx *Ebar = calloc((size_t)nthreads, sizeof(cplx));
+    double *Wsum = calloc((size_t)nthreads, sizeof(double));
+#pragma omp parallel
+    {
+        int tid = 0;
+#ifdef _OPENMP
+        tid = omp_get_thread_num();
+#endif
+        cplx *O = malloc((size_t)K * sizeof(cplx));
+        cplx *oe = OE + (size_t)tid * K, *oc = Oc + (size_t)tid * K;
+#pragma omp for schedule(static)
+        for (int64_t n = 0; n < B; ++n) {
+            const double wn = w ? w[n] : 1.0;
+            const cplx E = eloc_re_im[2 * n] + I * eloc_re_im[2 * n + 1];
+            log_derivatives_one(spins + n * N, N, M, b, W, O);
+            for (int64_t k = 0; k < K; ++k) {
+                oe[k] += wn * conj(O[k]) * E;
+                oc[k] += wn * conj(O[k]);
+            }
+            Ebar[tid] += wn * E;
+            Wsum[tid] += wn;
+        }
+        free(O);
+    }
+    cplx E = 0.0;
+    double sw = 0.0;
+    for (int t = 0; t < nthreads; ++t) {
+        E += Ebar[t];
+        sw += Wsum[t];
+    }
+    E /= sw;
+    for (int64_t k = 0; k < K; ++k) {
+        cplx oe = 0.0, oc = 0.0;
+        for (int t = 0; t < nthreads; ++t) {
+            oe += OE[(size_t)t * K + k];
+            oc += Oc[(size_t)t * K + k];
+        }
+        const cplx F = oe / sw - (oc / sw) * E;
+        out_F[2 * k] = creal(F);
+        out_F[2 * k + 1] = cimag(F);
+    }
+    free(OE);
+    free(Oc);
+    free(Ebar);
+    free(Wsum);
 }
 
 int oracle_num_threads(void) {

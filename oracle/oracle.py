@@ -47,6 +47,12 @@ def _load():
             fn.restype = None
         lib.oracle_connected.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp]
         lib.oracle_connected.restype = None
+        lib.oracle_mean_variance.argtypes = [vp, vp, i64, vp]
+        lib.oracle_mean_variance.restype = None
+        lib.oracle_log_derivatives.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp]
+        lib.oracle_log_derivatives.restype = None
+        lib.oracle_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp]
+        lib.oracle_forces.restype = None
         lib.oracle_num_threads.restype = i32
         lib.oracle_set_num_threads.argtypes = [i32]
         _lib = lib
@@ -130,3 +136,39 @@ def connected(spins, sites, paulis, coeffs):
     mel = np.empty((B, T), dtype=np.complex128)
     _load().oracle_connected(_p(spins), B, N, T, _p(sites), _p(paulis), _p(coeffs), _p(sp), _p(mel))
     return sp, mel
+
+
+def _weights(weights, B):
+    if weights is None:
+        return None
+    w = _c(weights, np.float64)
+    assert w.shape == (B,)
+    return w
+
+
+def mean_variance(x, weights=None):
+    """Eq. 5 / Eq. 3: (mean complex, variance, sum of weights) of x [B] complex."""
+    x = _c(x, np.complex128)
+    w = _weights(weights, x.shape[0])
+    out = np.empty(4, dtype=np.float64)
+    _load().oracle_mean_variance(_p(x), _p(w) if w is not None else None, x.shape[0], _p(out))
+    return complex(out[0], out[1]), float(out[2]), float(out[3])
+
+
+def log_derivatives(spins, a, b, W) -> np.ndarray:
+    """Eq. 8: O [B,K] complex128, K = N + M + M*N in the order a, b, W (row-major)."""
+    spins, a, b, W, B, N, M = _params(spins, a, b, W)
+    out = np.empty((B, N + M + M * N), dtype=np.complex128)
+    _load().oracle_log_derivatives(_p(spins), B, N, M, _p(a), _p(b), _p(W), _p(out))
+    return out
+
+
+def forces(spins, a, b, W, eloc, weights=None) -> np.ndarray:
+    """Eq. 16 (PAPER.md:134-138): F [K] complex128 = <<O_k^* E_loc>> - <<O_k^*>><<E_loc>>."""
+    spins, a, b, W, B, N, M = _params(spins, a, b, W)
+    eloc = _c(eloc, np.complex128)
+    assert eloc.shape == (B,)
+    w = _weights(weights, B)
+    out = np.empty(N + M + M * N, dtype=np.complex128)
+    _load().oracle_forces(_p(spins), B, N, M, _p(a), _p(b), _p(W), _p(eloc), _p(w) if w is not None else None, _p(out))
+    return out
