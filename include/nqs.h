@@ -141,6 +141,31 @@ int nqs_enumerate_connected(const nqs_hamiltonian *h, const int8_t *d_spins, int
 int nqs_profile_enable(int on);
 int nqs_profile_last(float ms[4]);
 
+/* ---------------------------------------------------------------------------------------
+ * Batch statistics (Eq. 5; get_global_mean / get_global_variance, :511-515).
+ *   d_x [B] complex64 (any local estimator, e.g. E_loc);  d_weights [B] float32 or NULL (= uniform;
+ *   with w_b = p(s_b) over a full basis the mean is the exact expectation of Eq. 3).
+ *   d_stats [4] float64 DEVICE out: Re mean, Im mean, variance <<|x - mean|^2>>, sum of weights.
+ * Sums are accumulated in float64 in a fixed order (deterministic).  Asynchronous on `stream`.
+ * ------------------------------------------------------------------------------------- */
+int nqs_energy_stats(const nqs_c64 *d_x, const float *d_weights, int64_t B, double *d_stats, void *stream);
+
+/* ---------------------------------------------------------------------------------------
+ * Force vector of the RBM (Eq. 16; energy gradient Eq. 7, :81-89):
+ *   F_k = <<E_loc O_k^*>>^c = <<O_k^* E_loc>> - <<O_k^*>> <<E_loc>>,
+ *   O_k(s) = d log psi(s) / d theta_k (Eq. 8, :93):  O_{a_i} = s_i, O_{b_j} = tanh theta_j,
+ *   O_{W_ji} = tanh theta_j s_i  with theta_j = b_j + sum_i W_ji s_i.
+ *   d_eloc [B] complex64 in (the local energies of the same batch); d_weights [B] float32 or NULL.
+ *   d_F [N + M + M*N] complex64 out, ordered a (i), b (j), W (row-major j*N + i) like the inputs.
+ *   d_stats [4] float64 device out or NULL: as nqs_energy_stats of d_eloc.
+ * The contraction over the samples runs on the tensor cores as an exact int8 GEMM (28-bit
+ * fixed-point split of conj(tanh theta) (E - mean) per hidden unit), so the result does not depend
+ * on the summation order.  B <= 2^25.  Asynchronous on `stream`.
+ * ------------------------------------------------------------------------------------- */
+int nqs_forces(const int8_t *d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64 *d_a,
+               const nqs_c64 *d_b, const nqs_c64 *d_W, const nqs_c64 *d_eloc, const float *d_weights,
+               nqs_c64 *d_F, double *d_stats, void *stream);
+
 /* Pipe-rate micro-benchmark (the roofline is quoted against the nominal peak
  * AND a peak measured on the box).  Runs a register-only kernel (2 blocks of 320 threads per SM,
  * no memory traffic in the loop) `iters` iterations, best of 3 after one warm-up, on a private

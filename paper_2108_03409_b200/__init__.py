@@ -9,7 +9,9 @@ from .binding import (  # noqa: F401
     Hamiltonian,
     MICROBENCH_KINDS,
     NqsError,
+    energy_stats,
     enumerate_connected,
+    forces,
     hamiltonian_info_host,
     last_error,
     lib_path,

@@ -47,6 +47,9 @@ def load_library() -> ctypes.CDLL:
             lib.nqs_hamiltonian_info.argtypes = [vp, vp, vp]
             lib.nqs_local_energy_h.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, vp]
             lib.nqs_enumerate_connected.argtypes = [vp, vp, i64, vp, vp, vp]
+            lib.nqs_energy_stats.argtypes = [vp, vp, i64, vp, vp]
+            lib.nqs_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+            lib.nqs_microbench.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float)]
             lib.nqs_profile_enable.argtypes = [i32]
             lib.nqs_profile_last.argtypes = [vp]
             lib.nqs_last_error.restype = ctypes.c_char_p
@@ -54,7 +57,8 @@ def load_library() -> ctypes.CDLL:
             for name in ("nqs_log_psi", "nqs_local_energy", "nqs_local_energy_host", "nqs_log_psi_host",
                          "nqs_hamiltonian_create", "nqs_hamiltonian_compile_host", "nqs_hamiltonian_destroy",
                          "nqs_hamiltonian_info", "nqs_local_energy_h", "nqs_enumerate_connected", "nqs_release",
-                         "nqs_profile_enable", "nqs_profile_last", "nqs_microbench"):
+                         "nqs_profile_enable", "nqs_profile_last", "nqs_microbench", "nqs_energy_stats",
+                         "nqs_forces"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -187,6 +191,36 @@ class Hamiltonian:
                 _dev(b, torch.complex64, "b"), _dev(W, torch.complex64, "W"), ctypes.c_void_p(eloc.data_ptr()),
                 ctypes.c_void_p(logpsi.data_ptr()) if want_logpsi else None, _stream()))
         return (eloc, logpsi) if want_logpsi else eloc
+
+
+def energy_stats(x, weights=None):
+    """nqs_energy_stats: float64 CUDA tensor [4] = (Re mean, Im mean, variance, sum of weights) of x [B]."""
+    import torch
+
+    stats = torch.empty(4, dtype=torch.float64, device=x.device)
+    with torch.cuda.device(x.device):
+        _check(load_library().nqs_energy_stats(
+            _dev(x, torch.complex64, "x"), _dev(weights, torch.float32, "weights") if weights is not None else None,
+            x.shape[0], ctypes.c_void_p(stats.data_ptr()), _stream()))
+    return stats
+
+
+def forces(spins, a, b, W, eloc, weights=None, want_stats: bool = False):
+    """nqs_forces: complex64 CUDA tensor [N + M + M*N] (order a, b, W row-major); optionally the stats of eloc."""
+    import torch
+
+    B, N, M = _shapes(spins, a, b, W)
+    if tuple(eloc.shape) != (B,) or (weights is not None and tuple(weights.shape) != (B,)):
+        raise ValueError("eloc / weights must have shape [B]")
+    F = torch.empty(N + M + M * N, dtype=torch.complex64, device=spins.device)
+    stats = torch.empty(4, dtype=torch.float64, device=spins.device) if want_stats else None
+    with torch.cuda.device(spins.device):
+        _check(load_library().nqs_forces(
+            _dev(spins, torch.int8, "spins"), B, N, M, _dev(a, torch.complex64, "a"), _dev(b, torch.complex64, "b"),
+            _dev(W, torch.complex64, "W"), _dev(eloc, torch.complex64, "eloc"),
+            _dev(weights, torch.float32, "weights") if weights is not None else None, ctypes.c_void_p(F.data_ptr()),
+            ctypes.c_void_p(stats.data_ptr()) if want_stats else None, _stream()))
+    return (F, stats) if want_stats else F
 
 
 def hamiltonian_info_host(N: int, sites, paulis, coeffs) -> dict:

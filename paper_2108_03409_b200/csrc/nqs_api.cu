@@ -13,6 +13,7 @@
 #include "../../include/nqs.h"
 #include "nqs_hamiltonian.h"
 #include "nqs_kernels.cuh"
+#include "nqs_forces.cuh"
 #include "nqs_microbench.cuh"
 #include "nqs_theta_mma.cuh"
 
@@ -655,5 +656,91 @@ extern "C" int nqs_microbench(int32_t kind, int32_t iters, double* lane_ops_per_
     cudaStreamDestroy(st);
     *lane_ops_per_s = (double)grid * 320.0 * iters * mb_ops_per_iter(kind) / (best * 1e-3);
     if (ms_out) *ms_out = best;
+    return NQS_OK;
+}
+
+// ----------------------------------------------------------------------------------------
+// batch statistics and the force vector
+// ----------------------------------------------------------------------------------------
+static int launch_stats(const nqs_c64* d_x, const float* d_w, int64_t B, double* d_stats, cudaStream_t st) {
+    double* partial = nullptr;
+    const int nblk = (int)((B + 255) / 256 < ST_BLOCKS ? (B + 255) / 256 : ST_BLOCKS);
+    NQS_CUDA(cudaMallocAsync(&partial, sizeof(double) * 4 * ST_BLOCKS, st));
+    stats_partial_kernel<<<nblk, 256, 0, st>>>((const float2*)d_x, d_w, (long long)B, partial);
+    NQS_CUDA(cudaGetLastError());
+    stats_final_kernel<<<1, 32, 0, st>>>(partial, nblk, d_stats);
+    NQS_CUDA(cudaGetLastError());
+    NQS_CUDA(cudaFreeAsync(partial, st));
+    return NQS_OK;
+}
+
+extern "C" int nqs_energy_stats(const nqs_c64* d_x, const float* d_weights, int64_t B, double* d_stats,
+                                void* stream) {
+    if (B <= 0 || !d_x || !d_stats) return fail(NQS_ERR_INVALID_ARG, "nqs_energy_stats: B <= 0 or NULL pointer");
+    int rc = check_device();
+    if (rc) return rc;
+    return launch_stats(d_x, d_weights, B, d_stats, (cudaStream_t)stream);
+}
+
+extern "C" int nqs_forces(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
+                          const nqs_c64* d_b, const nqs_c64* d_W, const nqs_c64* d_eloc, const float* d_weights,
+                          nqs_c64* d_F, double* d_stats, void* stream) {
+    int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
+    if (rc) return rc;
+    if (B <= 0 || !d_eloc || !d_F) return fail(NQS_ERR_INVALID_ARG, "nqs_forces: B <= 0 or NULL d_eloc / d_F");
+    if (B > (1ll << 25)) return fail(NQS_ERR_UNSUPPORTED, "nqs_forces: B > 2^25 (int32 accumulation range)");
+    if ((rc = check_device())) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M_pad = (int)round_up(M, KJ);
+    const long long B_pad = round_up(B, 256);
+    const long long nPairsPad = B_pad / 2;
+    const int K16 = (int)(B_pad / 16);
+    const int nIT = (N + 1 + TM_M - 1) / TM_M, nJT = (M + 1 + TM_JT - 1) / TM_JT;
+
+    float4* tp = nullptr;
+    float2* cb = nullptr;
+    double* stats = nullptr;
+    int* gexp = nullptr;
+    uint4 *A_packed = nullptr, *B_packed = nullptr;
+    NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
+    NQS_CUDA(cudaMallocAsync(&cb, sizeof(float2) * (size_t)B_pad, st));
+    NQS_CUDA(cudaMallocAsync(&stats, sizeof(double) * 4, st));
+    NQS_CUDA(cudaMallocAsync(&gexp, sizeof(int) * (size_t)nJT * TM_JT, st));
+    NQS_CUDA(cudaMallocAsync(&A_packed, sizeof(uint4) * (size_t)nIT * K16 * TM_M, st));
+    NQS_CUDA(cudaMallocAsync(&B_packed, sizeof(uint4) * (size_t)nJT * K16 * TM_N, st));
+
+    if ((rc = launch_stats(d_eloc, d_weights, B, stats, st))) return rc;
+    if (d_stats) NQS_CUDA(cudaMemcpyAsync(d_stats, stats, sizeof(double) * 4, cudaMemcpyDeviceToDevice, st));
+    force_coef_kernel<<<(unsigned)((B_pad + 255) / 256), 256, 0, st>>>((const float2*)d_eloc, d_weights, (long long)B,
+                                                                       B_pad, stats, cb);
+    NQS_CUDA(cudaGetLastError());
+    if ((rc = launch_theta(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st))) return rc;
+    force_gscale_kernel<<<(unsigned)(nJT * TM_JT), 256, 0, st>>>(tp, nPairsPad, cb, M, gexp);
+    NQS_CUDA(cudaGetLastError());
+    force_pack_g_kernel<<<148 * 8, 256, 0, st>>>(tp, nPairsPad, cb, M, K16, nJT, gexp, B_packed);
+    NQS_CUDA(cudaGetLastError());
+    force_pack_spins_kernel<<<148 * 8, 256, 0, st>>>(d_spins, (long long)B, N, K16, nIT, A_packed);
+    NQS_CUDA(cudaGetLastError());
+    static bool attr_set = false;
+    if (!attr_set) {
+        NQS_CUDA(cudaFuncSetAttribute(force_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FM_SMEM));
+        attr_set = true;
+    }
+    ForceMmaParams p;
+    p.A_packed = A_packed;
+    p.B_packed = B_packed;
+    p.gexp = gexp;
+    p.N = N;
+    p.M = M;
+    p.K16 = K16;
+    p.F = (float2*)d_F;
+    force_mma_kernel<<<dim3((unsigned)nIT, (unsigned)nJT), FM_THREADS, FM_SMEM, st>>>(p);
+    NQS_CUDA(cudaGetLastError());
+    NQS_CUDA(cudaFreeAsync(tp, st));
+    NQS_CUDA(cudaFreeAsync(cb, st));
+    NQS_CUDA(cudaFreeAsync(stats, st));
+    NQS_CUDA(cudaFreeAsync(gexp, st));
+    NQS_CUDA(cudaFreeAsync(A_packed, st));
+    NQS_CUDA(cudaFreeAsync(B_packed, st));
     return NQS_OK;
 }
