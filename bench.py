@@ -293,6 +293,20 @@ def run_ours(args) -> None:
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": 6 * args.steps,  # table, pack_spins, pack_w, theta_mma, eloc, finalize
         }
+        # SURVEY.md 8(f) items 1 + 3, reported beside the headline (not part of `value`): the force
+        # vector of the same batch from the E_loc just computed (nqs_forces: stats, theta, pack, int8 GEMM)
+        f_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+        for k in range(7):
+            if k >= 2:
+                flush.fill_(k)
+                f_ev[k - 2][0].record()
+            nqs.forces(spins, a, b, W, e)
+            if k >= 2:
+                f_ev[k - 2][1].record()
+        torch.cuda.synchronize()
+        f_ms = float(np.median([s0.elapsed_time(s1) for s0, s1 in f_ev]))
+        line["forces"] = {"ms_per_call": f_ms, "samples_per_s": w.B / (f_ms * 1e-3), "parameters": w.N + w.M + w.M * w.N,
+                          "what": "nqs_forces (Eq. 16) on the same batch, device-resident, median of 5, L2 flushed"}
         # pipe rates measured on this box (nqs_microbench; register-only kernels, after the timed region)
         mb = {k: nqs.microbench(k)["lane_ops_per_s"] for k in nqs.MICROBENCH_KINDS}
         line["measured_peaks"] = {
