@@ -14,6 +14,7 @@ from .oracle import (  # noqa: F401
     log_derivatives,
     log_psi,
     mean_variance,
+    metropolis,
     num_threads,
     set_num_threads,
 )

@@ -31,7 +31,8 @@
  * P3 zero parameters closed form, P4 product eigenstate, P5 singlet, P6 spin-flip symmetry,
  * P7 Pfeuty closed form for the dense-H builder, P8 definition<->fast, P9 log cosh special
  * cases; PF1 log-derivatives against finite differences of log psi, PF2 force vector against
- * finite differences of the dense <H>, PF3 mean / variance against numpy and Eq. 3).
+ * finite differences of the dense <H>, PF3 mean / variance against numpy and Eq. 3; PM1 the
+ * Metropolis rule against the dense psi, PM2 its stationary distribution |psi|^2).
  * No function here is "parity unpinned".
  */
 #include <complex.h>
@@ -401,6 +402,51 @@ void oracle_forces(const int8_t *spins, int64_t B, int N, int M, const float *a,
     free(Oc);
     free(Ebar);
     free(Wsum);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Metropolis sampling of p(s) = |psi(s)|^2 / <psi|psi> with single-spin-flip
+ * proposals, many independent chains (PAPER.md:70 Metropolis-Hastings; :341 one sweep = one
+ * proposal per degree of freedom; :490-494 chains run in sync).  The random numbers are INPUTS
+ * (proposal site and a uniform number per chain and step), so this function is deterministic.
+ *
+ * For chain c and step t:  s' = s with site sites[t,c] flipped;  the move is accepted iff
+ *     u[t,c] < |psi(s') / psi(s)|^2          (Metropolis: min(1, p(s')/p(s)), symmetric proposal)
+ * evaluated in logarithms, log u < 2 Re(log psi(s') - log psi(s)), with log psi(s') recomputed FROM
+ * SCRATCH by Eq. 38 at every proposal (no incremental update).  u = 0 always accepts.
+ *
+ * spins [C,N] int8 in/out; sites [S,C] int32; u [S,C] float32 in [0,1); accepted [C] int32 out;
+ * min_margin [C] float64 out = min over the steps of |2 Re dlogpsi - log u|: how far the closest
+ * decision of the chain was from a tie (a float32 implementation can only be asked to reproduce
+ * chains whose margin exceeds its rounding error).
+ * ------------------------------------------------------------------------------------- */
+void oracle_metropolis(int8_t *spins, int64_t C, int N, int M, const float *a, const float *b, const float *W,
+                       int S, const int32_t *sites, const float *u, int32_t *accepted, double *min_margin) {
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t c = 0; c < C; ++c) {
+        int8_t *s = spins + c * N;
+        cplx lp = log_psi_one(s, N, M, a, b, W, 1);
+        int acc = 0;
+        double mm = INFINITY;
+        for (int t = 0; t < S; ++t) {
+            const int site = sites[(int64_t)t * C + c];
+            const double ut = (double)u[(int64_t)t * C + c];
+            s[site] = (int8_t)(-s[site]);
+            const cplx lp_new = log_psi_one(s, N, M, a, b, W, 1);
+            const double log_ratio = 2.0 * creal(lp_new - lp);
+            const double log_u = ut > 0.0 ? log(ut) : -INFINITY;
+            const double margin = fabs(log_ratio - log_u);
+            if (margin < mm) mm = margin;
+            if (log_u < log_ratio) {
+                lp = lp_new;
+                ++acc;
+            } else {
+                s[site] = (int8_t)(-s[site]);
+            }
+        }
+        accepted[c] = acc;
+        min_margin[c] = mm;
+    }
 }
 
 int oracle_num_threads(void) {

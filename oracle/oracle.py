@@ -53,6 +53,8 @@ def _load():
         lib.oracle_log_derivatives.restype = None
         lib.oracle_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp]
         lib.oracle_forces.restype = None
+        lib.oracle_metropolis.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp]
+        lib.oracle_metropolis.restype = None
         lib.oracle_num_threads.restype = i32
         lib.oracle_set_num_threads.argtypes = [i32]
         _lib = lib
@@ -172,3 +174,18 @@ def forces(spins, a, b, W, eloc, weights=None) -> np.ndarray:
     out = np.empty(N + M + M * N, dtype=np.complex128)
     _load().oracle_forces(_p(spins), B, N, M, _p(a), _p(b), _p(W), _p(eloc), _p(w) if w is not None else None, _p(out))
     return out
+
+
+def metropolis(spins, a, b, W, sites, u):
+    """Single-spin-flip Metropolis chains driven by the given proposals (sites [S,C] int32) and
+    uniforms (u [S,C] float32).  Returns (final spins int8 [C,N], accepted int32 [C], min_margin f64 [C])."""
+    spins, a, b, W, C, N, M = _params(spins, a, b, W)
+    spins = spins.copy()
+    sites, u = _c(sites, np.int32), _c(u, np.float32)
+    S = sites.shape[0]
+    assert sites.shape == (S, C) and u.shape == (S, C)
+    assert sites.min(initial=0) >= 0 and sites.max(initial=0) < N
+    acc = np.empty(C, dtype=np.int32)
+    mm = np.empty(C, dtype=np.float64)
+    _load().oracle_metropolis(_p(spins), C, N, M, _p(a), _p(b), _p(W), S, _p(sites), _p(u), _p(acc), _p(mm))
+    return spins, acc, mm
