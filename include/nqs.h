@@ -166,6 +166,25 @@ int nqs_forces(const int8_t *d_spins, int64_t B, int32_t N, int32_t M, const nqs
                const nqs_c64 *d_b, const nqs_c64 *d_W, const nqs_c64 *d_eloc, const float *d_weights,
                nqs_c64 *d_F, double *d_stats, void *stream);
 
+/* ---------------------------------------------------------------------------------------
+ * Metropolis sampling of p(s) = |psi(s)|^2 / <psi|psi> with single-spin-flip
+ * proposals, C independent chains advanced in lock-step (:490-494); one sweep = N steps (:341).
+ *   d_spins    [C,N] int8 DEVICE in/out: the chains' states (start -> after S steps)
+ *   d_sites    [S,C] int32 DEVICE: the site proposed to chain c at step t is d_sites[t*C + c] in [0,N)
+ *   d_u        [S,C] float32 DEVICE, uniform in [0,1): the move is accepted iff
+ *                    u < |psi(s')/psi(s)|^2      (u = 0 always accepts)
+ *   d_accepted [C] int32 DEVICE out or NULL: accepted moves per chain
+ * The random numbers are the caller's (e.g. torch.randint / torch.rand on the device), so a call is
+ * a deterministic function of its inputs.  The acceptance test is evaluated in float32 (a decision
+ * closer to a tie than ~1e-4 in log |ratio|^2 may differ from exact arithmetic); tanh theta is
+ * recomputed from the spins every two sweeps (2 N steps) and updated in place by the addition
+ * theorem on each accepted move in between.  Sites outside [0,N) are undefined behaviour.  S = 0 is a no-op.  Asynchronous.
+ * NQS_ERR_UNSUPPORTED if one chain's state (8 M + N bytes) does not fit shared memory twice.
+ * ------------------------------------------------------------------------------------- */
+int nqs_metropolis(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64 *d_a,
+                   const nqs_c64 *d_b, const nqs_c64 *d_W, int32_t S, const int32_t *d_sites,
+                   const float *d_u, int32_t *d_accepted, void *stream);
+
 /* Pipe-rate micro-benchmark (the roofline is quoted against the nominal peak
  * AND a peak measured on the box).  Runs a register-only kernel (2 blocks of 320 threads per SM,
  * no memory traffic in the loop) `iters` iterations, best of 3 after one warm-up, on a private

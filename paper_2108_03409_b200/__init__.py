@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     local_energy_host,
     log_psi,
     log_psi_host,
+    metropolis,
     microbench,
     profile_enable,
     profile_last,

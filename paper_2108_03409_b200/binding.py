@@ -50,6 +50,7 @@ def load_library() -> ctypes.CDLL:
             lib.nqs_energy_stats.argtypes = [vp, vp, i64, vp, vp]
             lib.nqs_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_microbench.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float)]
+            lib.nqs_metropolis.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp]
             lib.nqs_profile_enable.argtypes = [i32]
             lib.nqs_profile_last.argtypes = [vp]
             lib.nqs_last_error.restype = ctypes.c_char_p
@@ -58,7 +59,7 @@ def load_library() -> ctypes.CDLL:
                          "nqs_hamiltonian_create", "nqs_hamiltonian_compile_host", "nqs_hamiltonian_destroy",
                          "nqs_hamiltonian_info", "nqs_local_energy_h", "nqs_enumerate_connected", "nqs_release",
                          "nqs_profile_enable", "nqs_profile_last", "nqs_microbench", "nqs_energy_stats",
-                         "nqs_forces"):
+                         "nqs_forces", "nqs_metropolis"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -221,6 +222,23 @@ def forces(spins, a, b, W, eloc, weights=None, want_stats: bool = False):
             _dev(weights, torch.float32, "weights") if weights is not None else None, ctypes.c_void_p(F.data_ptr()),
             ctypes.c_void_p(stats.data_ptr()) if want_stats else None, _stream()))
     return (F, stats) if want_stats else F
+
+
+def metropolis(spins, a, b, W, sites, u, want_accepted: bool = True):
+    """nqs_metropolis: advances the chains `spins` [C,N] IN PLACE by S = sites.shape[0] steps."""
+    import torch
+
+    C, N, M = _shapes(spins, a, b, W)
+    S = int(sites.shape[0])
+    if tuple(sites.shape) != (S, C) or tuple(u.shape) != (S, C):
+        raise ValueError("sites and u must have shape [S, C]")
+    accepted = torch.empty(C, dtype=torch.int32, device=spins.device) if want_accepted else None
+    with torch.cuda.device(spins.device):
+        _check(load_library().nqs_metropolis(
+            _dev(spins, torch.int8, "spins"), C, N, M, _dev(a, torch.complex64, "a"), _dev(b, torch.complex64, "b"),
+            _dev(W, torch.complex64, "W"), S, _dev(sites, torch.int32, "sites"), _dev(u, torch.float32, "u"),
+            ctypes.c_void_p(accepted.data_ptr()) if want_accepted else None, _stream()))
+    return accepted
 
 
 def hamiltonian_info_host(N: int, sites, paulis, coeffs) -> dict:

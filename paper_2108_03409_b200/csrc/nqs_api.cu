@@ -15,6 +15,7 @@
 #include "nqs_kernels.cuh"
 #include "nqs_forces.cuh"
 #include "nqs_microbench.cuh"
+#include "nqs_sampler.cuh"
 #include "nqs_theta_mma.cuh"
 
 using namespace nqs;
@@ -742,5 +743,78 @@ extern "C" int nqs_forces(const int8_t* d_spins, int64_t B, int32_t N, int32_t M
     NQS_CUDA(cudaFreeAsync(gexp, st));
     NQS_CUDA(cudaFreeAsync(A_packed, st));
     NQS_CUDA(cudaFreeAsync(B_packed, st));
+    return NQS_OK;
+}
+
+// ----------------------------------------------------------------------------------------
+// Metropolis chains
+// ----------------------------------------------------------------------------------------
+template <int CPB>
+static int launch_metropolis_t(const MetroParams& p, size_t smem, cudaStream_t st) {
+    static size_t attr_smem = 0;
+    if (smem > attr_smem) {
+        NQS_CUDA(cudaFuncSetAttribute(metropolis_kernel<CPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_smem = smem;
+    }
+    metropolis_kernel<CPB><<<(unsigned)((p.C + CPB - 1) / CPB), CPB * 32, smem, st>>>(p);
+    NQS_CUDA(cudaGetLastError());
+    return NQS_OK;
+}
+
+extern "C" int nqs_metropolis(int8_t* d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64* d_a,
+                              const nqs_c64* d_b, const nqs_c64* d_W, int32_t S, const int32_t* d_sites,
+                              const float* d_u, int32_t* d_accepted, void* stream) {
+    int rc = check_common(d_spins, C, N, M, d_a, d_b, d_W);
+    if (rc) return rc;
+    if (S < 0 || (S > 0 && C > 0 && (!d_sites || !d_u))) return fail(NQS_ERR_INVALID_ARG, "nqs_metropolis: S < 0 or NULL sites / u");
+    if ((rc = check_device())) return rc;
+    if (C == 0) return NQS_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M_pad = (int)round_up(M, KJ);
+    const long long C_pad = round_up(C, 256);
+    const long long nPairsPad = C_pad / 2;
+    int cpb = 16;
+    while (cpb > 2 && metropolis_smem_bytes(cpb, N, M_pad) > 220 * 1024) cpb >>= 1;
+    const size_t smem = metropolis_smem_bytes(cpb, N, M_pad);
+    if (smem > 220 * 1024) return fail(NQS_ERR_UNSUPPORTED, "nqs_metropolis: M too large for the shared-memory chain state");
+
+    float4* tp = nullptr;
+    float2 *TT = nullptr, *lk2 = nullptr;
+    NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
+    NQS_CUDA(cudaMallocAsync(&TT, sizeof(float2) * (size_t)N * M_pad, st));
+    NQS_CUDA(cudaMallocAsync(&lk2, sizeof(float2) * (size_t)N, st));
+    site_table_kernel<<<(unsigned)N, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, TT, lk2);
+    NQS_CUDA(cudaGetLastError());
+    MetroParams p;
+    p.spins = d_spins;
+    p.C = C;
+    p.N = N;
+    p.M = M;
+    p.M_pad = M_pad;
+    p.tp = tp;
+    p.nPairsPad = nPairsPad;
+    p.TT = TT;
+    p.lk2 = lk2;
+    p.accepted = d_accepted;
+    // chunks of two sweeps; tanh(theta) is recomputed from the current spins before each chunk
+    const int chunk = 2 * N;
+    for (int s0 = 0; s0 == 0 || s0 < S; s0 += chunk) {
+        if ((rc = launch_theta(d_spins, C, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st))) return rc;
+        p.S = S - s0 < chunk ? S - s0 : chunk;
+        p.sites = d_sites + (long long)s0 * C;
+        p.u = d_u + (long long)s0 * C;
+        p.accumulate = s0 > 0;
+        switch (cpb) {
+            case 16: rc = launch_metropolis_t<16>(p, smem, st); break;
+            case 8: rc = launch_metropolis_t<8>(p, smem, st); break;
+            case 4: rc = launch_metropolis_t<4>(p, smem, st); break;
+            default: rc = launch_metropolis_t<2>(p, smem, st); break;
+        }
+        if (rc) return rc;
+    }
+    if (rc) return rc;
+    NQS_CUDA(cudaFreeAsync(tp, st));
+    NQS_CUDA(cudaFreeAsync(TT, st));
+    NQS_CUDA(cudaFreeAsync(lk2, st));
     return NQS_OK;
 }

@@ -1,0 +1,125 @@
+"""Parity of nqs_metropolis against the float64 oracle.
+
+Floating point decides an integer here (accept / reject), and the kernel takes the decision in
+float32 from a product form the oracle does not use.  So: the oracle reports for
+every chain how close its closest decision was to a tie (min_margin, in log |ratio|^2); chains whose
+margin exceeds MARGIN must come out BIT-IDENTICAL (final spins and accepted count); the others must
+still be valid configurations.  MARGIN = 2e-4 is ~10x the float32 error of log |ratio|^2 (<= ~2e-5 at
+these sizes) and keeps > 85 % of the chains in the exact comparison.
+"""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+MARGIN = 2e-4
+
+
+@pytest.fixture(scope="module")
+def nqs():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests need a B200")
+    import paper_2108_03409_b200 as m
+
+    m.load_library()
+    return m
+
+
+def proposals(S, C, N, seed):
+    rng = np.random.default_rng([seed, 9])
+    return rng.integers(0, N, (S, C)).astype(np.int32), rng.random((S, C), dtype=np.float32)
+
+
+def gpu_metropolis(nqs, spins, a, b, W, sites, u):
+    import torch
+
+    d = torch.device("cuda:0")
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x)).to(d)  # noqa: E731
+    sp = t(spins.copy())
+    acc = nqs.metropolis(sp, t(a), t(b), t(W), t(sites), t(u))
+    torch.cuda.synchronize()
+    return sp.cpu().numpy(), acc.cpu().numpy()
+
+
+def compare(final, acc, ref_final, ref_acc, margin, what, min_robust=0.85):
+    assert set(np.unique(final)) <= {-1, 1}, what
+    robust = margin > MARGIN
+    assert robust.mean() >= min_robust, f"{what}: only {robust.mean():.2%} of the chains are robust"
+    bad = np.flatnonzero(robust & (np.any(final != ref_final, axis=1) | (acc != ref_acc)))
+    assert bad.size == 0, f"{what}: {bad.size} robust chains differ, first {bad[:5]}, margins {margin[bad[:5]]}"
+
+
+@pytest.mark.parametrize("N,M,C,S,sigma,seed", [
+    (8, 8, 256, 64, 0.3, 1),        # config-1 shapes
+    (40, 80, 1000, 200, 0.05, 2),   # config-2 shapes, 5 sweeps
+    (37, 45, 333, 150, 0.2, 3),     # ragged sizes, chains not a multiple of the block
+    (100, 400, 2048, 100, 0.03, 4), # config-3 shapes, one sweep
+    (20, 30, 64, 2000, 0.25, 5),    # long chains: drift of the in-place tanh update over 100 sweeps
+])
+def test_metropolis_vs_oracle(nqs, oracle, N, M, C, S, sigma, seed):
+    w = wl.make_random(N, M, C, 4, sigma, 200 + seed)
+    sites, u = proposals(S, w.B, N, seed)
+    final, acc = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, u)
+    ref_final, ref_acc, margin = oracle.metropolis(w.spins, w.a, w.b, w.W, sites, u)
+    compare(final, acc, ref_final, ref_acc, margin, f"N={N} M={M} C={w.B} S={S}", min_robust=0.5 if S > 1000 else 0.85)
+    assert 0.05 < acc.mean() / S <= 1.0
+
+
+def test_metropolis_config5_full_size_sampled_chains(nqs, oracle):
+    """Config 5 at full size (65536 chains, the launch configuration of the sampler bench): chains are
+    independent, so the oracle replays 48 sampled chains one by one."""
+    w = wl.make_config(5)
+    S = 24
+    sites, u = proposals(S, w.B, w.N, 55)
+    final, acc = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, u)
+    assert set(np.unique(final)) <= {-1, 1}
+    sel = np.sort(np.random.default_rng(56).choice(w.B, size=48, replace=False))
+    sel[0], sel[-1] = 0, w.B - 1
+    ref_final, ref_acc, margin = oracle.metropolis(w.spins[sel], w.a, w.b, w.W, sites[:, sel], u[:, sel])
+    compare(final[sel], acc[sel], ref_final, ref_acc, margin, "config 5 sampled chains")
+    # every chain: the flipped sites are exactly the accepted proposals' parity
+    flips = (final != w.spins).sum(axis=1)
+    assert np.all(flips <= acc) and np.all((acc - flips) % 2 == 0)
+
+
+def test_metropolis_properties(nqs):
+    import torch
+
+    N, M, C = 24, 16, 100
+    w = wl.make_random(N, M, C, 4, 0.2, 77)
+    rng = np.random.default_rng(78)
+    sites = np.repeat(rng.integers(0, N, (8, C)), 2, axis=0).astype(np.int32)
+    final, acc = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, np.zeros(sites.shape, np.float32))
+    assert np.all(acc == 16) and np.array_equal(final, w.spins)  # u = 0 accepts; double flips restore
+    sites, u = proposals(50, C, N, 79)
+    f1, a1 = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, u)
+    f2, a2 = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, u)
+    assert np.array_equal(f1, f2) and np.array_equal(a1, a2)  # deterministic
+    f0, a0 = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites[:0], u[:0])
+    assert np.array_equal(f0, w.spins) and np.all(a0 == 0)  # S = 0
+    d = torch.device("cuda:0")
+    with pytest.raises(ValueError):
+        nqs.metropolis(torch.from_numpy(w.spins).to(d), torch.from_numpy(w.a).to(d), torch.from_numpy(w.b).to(d),
+                       torch.from_numpy(w.W).to(d), torch.from_numpy(sites[:, :5]).to(d), torch.from_numpy(u).to(d))
+
+
+def test_metropolis_samples_the_born_distribution(nqs):
+    """End to end, no oracle: 2^5 states, 60000 chains from uniform starts; the final states follow
+    |psi|^2 (dense psi from tests/dense_reference.py) within 4.5 standard errors."""
+    from dense_reference import all_states, psi_all
+
+    N, M, C, S = 5, 4, 60000, 80
+    w = wl.make_random(N, M, 1 << N, 4, 0.3, 88)
+    p = np.abs(psi_all(N, w.a, w.b, w.W)) ** 2
+    p /= p.sum()
+    rng = np.random.default_rng(89)
+    start = all_states(N).astype(np.int8)[rng.integers(0, 1 << N, C)]
+    sites, u = proposals(S, C, N, 90)
+    final, _ = gpu_metropolis(nqs, start, w.a, w.b, w.W, sites, u)
+    idx = ((1 - final.astype(np.int64)) // 2) @ (1 << np.arange(N - 1, -1, -1))
+    freq = np.bincount(idx, minlength=1 << N) / C
+    assert np.all(np.abs(freq - p) < 4.5 * np.sqrt(p * (1 - p) / C)), np.abs(freq - p).max()
