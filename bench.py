@@ -307,6 +307,28 @@ def run_ours(args) -> None:
         f_ms = float(np.median([s0.elapsed_time(s1) for s0, s1 in f_ev]))
         line["forces"] = {"ms_per_call": f_ms, "samples_per_s": w.B / (f_ms * 1e-3), "parameters": w.N + w.M + w.M * w.N,
                           "what": "nqs_forces (Eq. 16) on the same batch, device-resident, median of 5, L2 flushed"}
+        # one Metropolis sweep (N proposals per chain) of B chains, proposals and
+        # uniforms drawn on the device beforehand (not timed), chains continue from the batch
+        gen = torch.Generator(device=dev)
+        gen.manual_seed(1234)
+        m_sites = torch.randint(0, w.N, (w.N, w.B), device=dev, dtype=torch.int32, generator=gen)
+        m_u = torch.rand((w.N, w.B), device=dev, dtype=torch.float32, generator=gen)
+        chains = spins.clone()
+        m_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)]
+        acc = None
+        for k in range(4):
+            if k >= 1:
+                m_ev[k - 1][0].record()
+            acc = nqs.metropolis(chains, a, b, W, m_sites, m_u)
+            if k >= 1:
+                m_ev[k - 1][1].record()
+        torch.cuda.synchronize()
+        m_ms = float(np.median([s0.elapsed_time(s1) for s0, s1 in m_ev]))
+        line["metropolis"] = {"ms_per_sweep": m_ms, "chains": w.B, "steps_per_sweep": w.N,
+                              "proposals_per_s": w.B * w.N / (m_ms * 1e-3),
+                              "acceptance": float(acc.float().mean().item()) / w.N,
+                              "what": "nqs_metropolis, one sweep of all chains, median of 3"}
+        del m_sites, m_u, chains
         # pipe rates measured on this box (nqs_microbench; register-only kernels, after the timed region)
         mb = {k: nqs.microbench(k)["lane_ops_per_s"] for k in nqs.MICROBENCH_KINDS}
         line["measured_peaks"] = {

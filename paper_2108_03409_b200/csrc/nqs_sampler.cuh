@@ -68,6 +68,8 @@ __host__ __device__ inline size_t metropolis_smem_bytes(int cpb, int N, int M_pa
     return (size_t)cpb * ((size_t)M_pad * sizeof(float2) + (size_t)((N + 15) / 16 * 16));
 }
 
+constexpr int MT_UNROLL = 8;
+
 template <int CPB>
 __global__ void __launch_bounds__(CPB * 32) metropolis_kernel(const MetroParams p) {
     extern __shared__ __align__(16) unsigned char mt_smem[];
@@ -106,36 +108,50 @@ __global__ void __launch_bounds__(CPB * 32) metropolis_kernel(const MetroParams 
         ul = __shfl_sync(0xffffffffu, ul, 0);
         const float sg = (float)s_s[site];
         const float2* const Trow = p.TT + (long long)site * p.M_pad;
-        // pass 1: log2 prod_j |D_j|^2
-        float lg = 0.f, q = 1.f;
-        int cnt = 0;
-#pragma unroll 4
-        for (int j = lane; j < p.M; j += 32) {
-            const float2 t = t_s[j], T = Trow[j];
-            const float xr = fmaf(t.x, T.x, -t.y * T.y), xi = fmaf(t.x, T.y, t.y * T.x);
-            const float Dr = fmaf(-sg, xr, 1.f), Di = -sg * xi;
-            q *= fmaf(Dr, Dr, Di * Di);
-            if (++cnt == 8) {
-                lg += log2f(q);
-                q = 1.f;
-                cnt = 0;
+        // pass 1: log2 prod_j |D_j|^2, eight hidden units per lane at a time (loads issued together)
+        float lg = 0.f;
+        for (int j0 = lane; j0 < p.M; j0 += 32 * MT_UNROLL) {
+            float2 t[MT_UNROLL], T[MT_UNROLL];
+#pragma unroll
+            for (int k = 0; k < MT_UNROLL; ++k) {
+                const int j = j0 + 32 * k;
+                const bool live = j < p.M;  // t = T = 0 gives D = 1
+                T[k] = live ? Trow[j] : make_float2(0.f, 0.f);
+                t[k] = live ? t_s[j] : make_float2(0.f, 0.f);
             }
+            float q = 1.f;
+#pragma unroll
+            for (int k = 0; k < MT_UNROLL; ++k) {
+                const float xr = fmaf(t[k].x, T[k].x, -t[k].y * T[k].y), xi = fmaf(t[k].x, T[k].y, t[k].y * T[k].x);
+                const float Dr = fmaf(-sg, xr, 1.f), Di = -sg * xi;
+                q *= fmaf(Dr, Dr, Di * Di);
+            }
+            lg += log2f(q);
         }
-        lg += log2f(q);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) lg += __shfl_xor_sync(0xffffffffu, lg, o);
         const float2 lk = p.lk2[site];
         const bool accept = log2f(ul) < 2.f * (sg > 0.f ? lk.x : lk.y) + lg;  // u == 0: -inf, always accepted
         if (accept) {
             // pass 2: t_j <- (t_j - sigma T_j) / D_j
-#pragma unroll 4
-            for (int j = lane; j < p.M; j += 32) {
-                const float2 t = t_s[j], T = Trow[j];
-                const float xr = fmaf(t.x, T.x, -t.y * T.y), xi = fmaf(t.x, T.y, t.y * T.x);
-                const float Dr = fmaf(-sg, xr, 1.f), Di = -sg * xi;
-                const float inv = 1.f / fmaf(Dr, Dr, Di * Di);
-                const float nr = fmaf(-sg, T.x, t.x), ni = fmaf(-sg, T.y, t.y);
-                t_s[j] = make_float2(fmaf(nr, Dr, ni * Di) * inv, fmaf(ni, Dr, -nr * Di) * inv);
+            for (int j0 = lane; j0 < p.M; j0 += 32 * MT_UNROLL) {
+                float2 t[MT_UNROLL], T[MT_UNROLL];
+#pragma unroll
+                for (int k = 0; k < MT_UNROLL; ++k) {
+                    const int j = j0 + 32 * k;
+                    const bool live = j < p.M;
+                    T[k] = live ? Trow[j] : make_float2(0.f, 0.f);
+                    t[k] = live ? t_s[j] : make_float2(0.f, 0.f);
+                }
+#pragma unroll
+                for (int k = 0; k < MT_UNROLL; ++k) {
+                    const float xr = fmaf(t[k].x, T[k].x, -t[k].y * T[k].y), xi = fmaf(t[k].x, T[k].y, t[k].y * T[k].x);
+                    const float Dr = fmaf(-sg, xr, 1.f), Di = -sg * xi;
+                    const float inv = __frcp_rn(fmaf(Dr, Dr, Di * Di));
+                    const float nr = fmaf(-sg, T[k].x, t[k].x), ni = fmaf(-sg, T[k].y, t[k].y);
+                    if (j0 + 32 * k < p.M)
+                        t_s[j0 + 32 * k] = make_float2(fmaf(nr, Dr, ni * Di) * inv, fmaf(ni, Dr, -nr * Di) * inv);
+                }
             }
             if (lane == 0) s_s[site] = (int8_t)(-(int)sg);
             ++acc;
