@@ -33,7 +33,7 @@ FP32_LANES_PER_SM = 128
 L2_FLUSH_BYTES = 256 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum of one eloc_kernel launch at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-ELOC_KERNEL_DRAM_TRAFFIC_BYTES = 891_420_160  # profiles/r1_v2_ncu_summary.md
+ELOC_KERNEL_DRAM_TRAFFIC_BYTES = 897_815_552  # profiles/r1_v3_ncu_summary.md: dram read + write per launch
 
 
 def shard_plan(n_ranks: int, rank: int, config: int) -> dict:
