@@ -59,16 +59,22 @@ static void plan_tiles(nqs_hamiltonian* h) {
     const int C = (int)h->hc.col_i.size();
     h->C = C;
     const int slices = C > 0 ? (C + 15) / 16 : 1;
-    // fewest padded 16-column slices; ties -> wider blocks (less re-staging of tanh(theta))
+    // least padded work divided by the measured efficiency of the block shape: a CTA has 2 WC warps, and
+    // narrow CTAs leave the SM short of warps (measured per 16-column slice on configs 3 and 4, B200)
+    static const double eff[MAX_WC + 1] = {0.0, 0.36, 0.54, 0.55, 0.68, 0.64};
     int best = 1;
     double best_cost = 1e30;
     for (int wc = 1; wc <= MAX_WC; ++wc) {
         const int tiles = (slices + wc - 1) / wc;
-        const double cost = (double)tiles * wc * (1.0 + 0.08 / wc);
-        if (cost < best_cost - 1e-9 || (cost < best_cost + 1e-9 && wc > best)) {
+        const double cost = (double)tiles * wc / eff[wc];
+        if (cost < best_cost - 1e-9) {
             best_cost = cost;
             best = wc;
         }
+    }
+    if (const char* e = getenv("NQS_WC")) {  // A/B experiments
+        const int v = atoi(e);
+        if (v >= 1 && v <= MAX_WC) best = v;
     }
     h->WC = best;
     h->WS = 2;
