@@ -784,10 +784,10 @@ extern "C" int nqs_metropolis(int8_t* d_spins, int64_t C, int32_t N, int32_t M, 
     const size_t smem = metropolis_smem_bytes(cpb, N, M_pad);
     if (smem > 220 * 1024) return fail(NQS_ERR_UNSUPPORTED, "nqs_metropolis: M too large for the shared-memory chain state");
 
-    float4* tp = nullptr;
-    float2 *TT = nullptr, *lk2 = nullptr;
+    float4 *tp = nullptr, *TT = nullptr;
+    float2* lk2 = nullptr;
     NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
-    NQS_CUDA(cudaMallocAsync(&TT, sizeof(float2) * (size_t)N * M_pad, st));
+    NQS_CUDA(cudaMallocAsync(&TT, sizeof(float4) * (size_t)N * (M_pad / 2), st));
     NQS_CUDA(cudaMallocAsync(&lk2, sizeof(float2) * (size_t)N, st));
     site_table_kernel<<<(unsigned)N, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, TT, lk2);
     NQS_CUDA(cudaGetLastError());

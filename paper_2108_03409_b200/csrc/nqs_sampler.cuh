@@ -19,24 +19,32 @@
 
 namespace nqs {
 
-// One block per site i: TT[i][j] = tanh(2 W_ji) (0 for the padding j >= M) and
+// Hidden units are handled in PAIRS (j0, j1) = (2 jp, 2 jp + 1) riding in the two halves of packed
+// FFMA2 operands: records are float4 (re_j0, re_j1, im_j0, im_j1), for t in shared memory and for
+// T^T in global memory, so one 16-byte load per operand feeds two hidden units.
+
+// One block per site i: TT[i][jp] = tanh(2 W_ji) for the pair jp (0 for the padding j >= M) and
 // lk2[i] = log2(e) * (Re L_i - 2 Re a_i, Re L_i + 2 Re a_i),  L_i = sum_j log cosh(2 W_ji):
 // log2 |exp(-2 sigma a_i) prod_j cosh 2 W_ji|^2 / 2 for sigma = +1 (x) and -1 (y).
 __global__ void __launch_bounds__(256) site_table_kernel(const float2* __restrict__ W, const float2* __restrict__ a,
-                                                         int N, int M, int M_pad, float2* __restrict__ TT,
+                                                         int N, int M, int M_pad, float4* __restrict__ TT,
                                                          float2* __restrict__ lk2) {
     const int i = blockIdx.x;
     __shared__ double sh[256];
     double acc = 0.0;
-    for (int j = threadIdx.x; j < M_pad; j += 256) {
-        float2 t = make_float2(0.f, 0.f);
-        if (j < M) {
-            const float2 w = W[(long long)j * N + i];
-            float lr, li;
-            lncosh_tanh(2.f * w.x, 2.f * w.y, lr, li, t.x, t.y);
-            acc += (double)lr;
+    for (int jp = threadIdx.x; jp < M_pad / 2; jp += 256) {
+        float tr[2] = {0.f, 0.f}, ti[2] = {0.f, 0.f};
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int j = 2 * jp + h;
+            if (j < M) {
+                const float2 w = W[(long long)j * N + i];
+                float lr, li;
+                lncosh_tanh(2.f * w.x, 2.f * w.y, lr, li, tr[h], ti[h]);
+                acc += (double)lr;
+            }
         }
-        TT[(long long)i * M_pad + j] = t;
+        TT[(long long)i * (M_pad / 2) + jp] = make_float4(tr[0], tr[1], ti[0], ti[1]);
     }
     sh[threadIdx.x] = acc;
     __syncthreads();
@@ -56,7 +64,7 @@ struct MetroParams {
     int N, M, M_pad, S;
     const float4* tp;        // [M_pad][nPairsPad]: tanh theta of the start states, two chains per record
     long long nPairsPad;
-    const float2* TT;        // [N][M_pad]
+    const float4* TT;        // [N][M_pad / 2]
     const float2* lk2;       // [N]
     const int* sites;        // [S][C]
     const float* u;          // [S][C]
@@ -68,23 +76,36 @@ __host__ __device__ inline size_t metropolis_smem_bytes(int cpb, int N, int M_pa
     return (size_t)cpb * ((size_t)M_pad * sizeof(float2) + (size_t)((N + 15) / 16 * 16));
 }
 
-constexpr int MT_UNROLL = 8;
+constexpr int MT_UNROLL = 5;  // pairs per lane whose loads are issued together (config 5: 25 = 5 x 5)
+
+// D = 1 - sigma t T for a pair of hidden units; returns |D|^2 per half
+__device__ __forceinline__ float2 metro_D(const float4 t, const float4 T, const float nsg, float2& Dr, float2& Di) {
+    const float2 tr = make_float2(t.x, t.y), ti = make_float2(t.z, t.w);
+    const float2 Tr = make_float2(T.x, T.y), Ti = make_float2(T.z, T.w);
+    const float2 xr = __ffma2_rn(neg2(ti), Ti, __fmul2_rn(tr, Tr));
+    const float2 xi = __ffma2_rn(ti, Tr, __fmul2_rn(tr, Ti));
+    Dr = __ffma2_rn(bc2(nsg), xr, bc2(1.f));
+    Di = __fmul2_rn(bc2(nsg), xi);
+    return __ffma2_rn(Dr, Dr, __fmul2_rn(Di, Di));
+}
 
 template <int CPB>
-__global__ void __launch_bounds__(CPB * 32) metropolis_kernel(const MetroParams p) {
+__global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroParams p) {
     extern __shared__ __align__(16) unsigned char mt_smem[];
-    float2* const t_all = reinterpret_cast<float2*>(mt_smem);
+    float4* const t_all = reinterpret_cast<float4*>(mt_smem);
     const int N_pad = (p.N + 15) / 16 * 16;
+    const int MP = p.M_pad / 2;  // hidden-unit pairs (padding pairs hold t = 0, T = 0: D = 1)
     int8_t* const s_all = reinterpret_cast<int8_t*>(mt_smem + (size_t)CPB * p.M_pad * sizeof(float2));
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long c0 = (long long)blockIdx.x * CPB;
 
     // the block's CPB chains are CPB/2 consecutive records of every tp row
-    for (int idx = tid; idx < p.M_pad * (CPB / 2); idx += CPB * 32) {
-        const int j = idx / (CPB / 2), pr = idx % (CPB / 2);
-        const float4 r = p.tp[(long long)j * p.nPairsPad + c0 / 2 + pr];
-        t_all[(size_t)(2 * pr) * p.M_pad + j] = make_float2(r.x, r.z);
-        t_all[(size_t)(2 * pr + 1) * p.M_pad + j] = make_float2(r.y, r.w);
+    for (int idx = tid; idx < MP * (CPB / 2); idx += CPB * 32) {
+        const int jp = idx / (CPB / 2), pr = idx % (CPB / 2);
+        const float4 r0 = p.tp[(long long)(2 * jp) * p.nPairsPad + c0 / 2 + pr];
+        const float4 r1 = p.tp[(long long)(2 * jp + 1) * p.nPairsPad + c0 / 2 + pr];
+        t_all[(size_t)(2 * pr) * MP + jp] = make_float4(r0.x, r1.x, r0.z, r1.z);
+        t_all[(size_t)(2 * pr + 1) * MP + jp] = make_float4(r0.y, r1.y, r0.w, r1.w);
     }
     for (int idx = tid; idx < CPB * p.N; idx += CPB * 32) {
         const int w = idx / p.N, i = idx % p.N;
@@ -94,8 +115,9 @@ __global__ void __launch_bounds__(CPB * 32) metropolis_kernel(const MetroParams 
 
     const long long c = c0 + warp;
     if (c >= p.C) return;
-    float2* const t_s = t_all + (size_t)warp * p.M_pad;
+    float4* const t_s = t_all + (size_t)warp * MP;
     int8_t* const s_s = s_all + warp * N_pad;
+    const int nFull = MP / (32 * MT_UNROLL);  // groups of 32 x MT_UNROLL pairs with no ragged lane
     int acc = 0;
     for (int step = 0; step < p.S; ++step) {
         int site = 0;
@@ -106,53 +128,59 @@ __global__ void __launch_bounds__(CPB * 32) metropolis_kernel(const MetroParams 
         }
         site = __shfl_sync(0xffffffffu, site, 0);
         ul = __shfl_sync(0xffffffffu, ul, 0);
-        const float sg = (float)s_s[site];
-        const float2* const Trow = p.TT + (long long)site * p.M_pad;
-        // pass 1: log2 prod_j |D_j|^2, eight hidden units per lane at a time (loads issued together)
+        const float sg = (float)s_s[site], nsg = -sg;
+        const float4* const Trow = p.TT + (long long)site * MP;
+        // pass 1: log2 prod_j |D_j|^2 (real product per lane, log2 per group, shuffle sum)
         float lg = 0.f;
-        for (int j0 = lane; j0 < p.M; j0 += 32 * MT_UNROLL) {
-            float2 t[MT_UNROLL], T[MT_UNROLL];
+        auto pass1 = [&](int jp0, bool ragged) {
+            float4 t[MT_UNROLL], T[MT_UNROLL];
 #pragma unroll
             for (int k = 0; k < MT_UNROLL; ++k) {
-                const int j = j0 + 32 * k;
-                const bool live = j < p.M;  // t = T = 0 gives D = 1
-                T[k] = live ? Trow[j] : make_float2(0.f, 0.f);
-                t[k] = live ? t_s[j] : make_float2(0.f, 0.f);
+                const int jp = jp0 + 32 * k;
+                const bool live = !ragged || jp < MP;
+                T[k] = live ? Trow[jp] : make_float4(0.f, 0.f, 0.f, 0.f);
+                t[k] = live ? t_s[jp] : make_float4(0.f, 0.f, 0.f, 0.f);
             }
-            float q = 1.f;
+            float2 q = make_float2(1.f, 1.f);
 #pragma unroll
             for (int k = 0; k < MT_UNROLL; ++k) {
-                const float xr = fmaf(t[k].x, T[k].x, -t[k].y * T[k].y), xi = fmaf(t[k].x, T[k].y, t[k].y * T[k].x);
-                const float Dr = fmaf(-sg, xr, 1.f), Di = -sg * xi;
-                q *= fmaf(Dr, Dr, Di * Di);
+                float2 Dr, Di;
+                q = __fmul2_rn(q, metro_D(t[k], T[k], nsg, Dr, Di));
             }
-            lg += log2f(q);
-        }
+            lg += log2f(q.x * q.y);
+        };
+        for (int g = 0; g < nFull; ++g) pass1(g * 32 * MT_UNROLL + lane, false);
+        if (nFull * 32 * MT_UNROLL < MP) pass1(nFull * 32 * MT_UNROLL + lane, true);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) lg += __shfl_xor_sync(0xffffffffu, lg, o);
         const float2 lk = p.lk2[site];
         const bool accept = log2f(ul) < 2.f * (sg > 0.f ? lk.x : lk.y) + lg;  // u == 0: -inf, always accepted
         if (accept) {
             // pass 2: t_j <- (t_j - sigma T_j) / D_j
-            for (int j0 = lane; j0 < p.M; j0 += 32 * MT_UNROLL) {
-                float2 t[MT_UNROLL], T[MT_UNROLL];
+            auto pass2 = [&](int jp0, bool ragged) {
+                float4 t[MT_UNROLL], T[MT_UNROLL];
 #pragma unroll
                 for (int k = 0; k < MT_UNROLL; ++k) {
-                    const int j = j0 + 32 * k;
-                    const bool live = j < p.M;
-                    T[k] = live ? Trow[j] : make_float2(0.f, 0.f);
-                    t[k] = live ? t_s[j] : make_float2(0.f, 0.f);
+                    const int jp = jp0 + 32 * k;
+                    const bool live = !ragged || jp < MP;
+                    T[k] = live ? Trow[jp] : make_float4(0.f, 0.f, 0.f, 0.f);
+                    t[k] = live ? t_s[jp] : make_float4(0.f, 0.f, 0.f, 0.f);
                 }
 #pragma unroll
                 for (int k = 0; k < MT_UNROLL; ++k) {
-                    const float xr = fmaf(t[k].x, T[k].x, -t[k].y * T[k].y), xi = fmaf(t[k].x, T[k].y, t[k].y * T[k].x);
-                    const float Dr = fmaf(-sg, xr, 1.f), Di = -sg * xi;
-                    const float inv = __frcp_rn(fmaf(Dr, Dr, Di * Di));
-                    const float nr = fmaf(-sg, T[k].x, t[k].x), ni = fmaf(-sg, T[k].y, t[k].y);
-                    if (j0 + 32 * k < p.M)
-                        t_s[j0 + 32 * k] = make_float2(fmaf(nr, Dr, ni * Di) * inv, fmaf(ni, Dr, -nr * Di) * inv);
+                    float2 Dr, Di;
+                    const float2 d2 = metro_D(t[k], T[k], nsg, Dr, Di);
+                    const float2 inv = make_float2(__frcp_rn(d2.x), __frcp_rn(d2.y));
+                    const float2 nr = __ffma2_rn(bc2(nsg), make_float2(T[k].x, T[k].y), make_float2(t[k].x, t[k].y));
+                    const float2 ni = __ffma2_rn(bc2(nsg), make_float2(T[k].z, T[k].w), make_float2(t[k].z, t[k].w));
+                    const float2 outr = __fmul2_rn(__ffma2_rn(nr, Dr, __fmul2_rn(ni, Di)), inv);
+                    const float2 outi = __fmul2_rn(__ffma2_rn(ni, Dr, __fmul2_rn(neg2(nr), Di)), inv);
+                    const int jp = jp0 + 32 * k;
+                    if (!ragged || jp < MP) t_s[jp] = make_float4(outr.x, outr.y, outi.x, outi.y);
                 }
-            }
+            };
+            for (int g = 0; g < nFull; ++g) pass2(g * 32 * MT_UNROLL + lane, false);
+            if (nFull * 32 * MT_UNROLL < MP) pass2(nFull * 32 * MT_UNROLL + lane, true);
             if (lane == 0) s_s[site] = (int8_t)(-(int)sg);
             ++acc;
         }
