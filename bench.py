@@ -307,6 +307,20 @@ def run_ours(args) -> None:
         f_ms = float(np.median([s0.elapsed_time(s1) for s0, s1 in f_ev]))
         line["forces"] = {"ms_per_call": f_ms, "samples_per_s": w.B / (f_ms * 1e-3), "parameters": w.N + w.M + w.M * w.N,
                           "what": "nqs_forces (Eq. 16) on the same batch, device-resident, median of 5, L2 flushed"}
+        # one VMC evaluation step: E_loc + statistics + forces with theta computed once
+        v_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+        for k in range(7):
+            if k >= 2:
+                flush.fill_(k)
+                v_ev[k - 2][0].record()
+            ham.local_energy_forces(spins, a, b, W)
+            if k >= 2:
+                v_ev[k - 2][1].record()
+        torch.cuda.synchronize()
+        v_ms = float(np.median([s0.elapsed_time(s1) for s0, s1 in v_ev]))
+        line["vmc_step"] = {"ms_per_call": v_ms, "samples_per_s": w.B / (v_ms * 1e-3),
+                            "what": "nqs_local_energy_forces_h: E_loc, mean/variance and force vector of one batch, "
+                                    "theta and tanh(theta) computed once; median of 5, L2 flushed"}
         # one Metropolis sweep (N proposals per chain) of B chains, proposals and
         # uniforms drawn on the device beforehand (not timed), chains continue from the batch
         gen = torch.Generator(device=dev)

@@ -166,6 +166,14 @@ int nqs_forces(const int8_t *d_spins, int64_t B, int32_t N, int32_t M, const nqs
                const nqs_c64 *d_b, const nqs_c64 *d_W, const nqs_c64 *d_eloc, const float *d_weights,
                nqs_c64 *d_F, double *d_stats, void *stream);
 
+/* One VMC evaluation step (Algorithm 1 lines 6-9): nqs_local_energy_h followed by
+ * nqs_forces on the same batch, with theta and tanh(theta) computed once and shared.  Arguments as in
+ * those two calls; d_logpsi and d_stats may be NULL.  Results are identical to the two separate calls. */
+int nqs_local_energy_forces_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t B, int32_t M,
+                              const nqs_c64 *d_a, const nqs_c64 *d_b, const nqs_c64 *d_W,
+                              const float *d_weights, nqs_c64 *d_eloc, nqs_c64 *d_logpsi, nqs_c64 *d_F,
+                              double *d_stats, void *stream);
+
 /* ---------------------------------------------------------------------------------------
  * Metropolis sampling of p(s) = |psi(s)|^2 / <psi|psi> with single-spin-flip
  * proposals, C independent chains advanced in lock-step (:490-494); one sweep = N steps (:341).

@@ -50,6 +50,7 @@ def load_library() -> ctypes.CDLL:
             lib.nqs_energy_stats.argtypes = [vp, vp, i64, vp, vp]
             lib.nqs_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_microbench.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float)]
+            lib.nqs_local_energy_forces_h.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_metropolis.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp]
             lib.nqs_profile_enable.argtypes = [i32]
             lib.nqs_profile_last.argtypes = [vp]
@@ -59,7 +60,7 @@ def load_library() -> ctypes.CDLL:
                          "nqs_hamiltonian_create", "nqs_hamiltonian_compile_host", "nqs_hamiltonian_destroy",
                          "nqs_hamiltonian_info", "nqs_local_energy_h", "nqs_enumerate_connected", "nqs_release",
                          "nqs_profile_enable", "nqs_profile_last", "nqs_microbench", "nqs_energy_stats",
-                         "nqs_forces", "nqs_metropolis"):
+                         "nqs_forces", "nqs_metropolis", "nqs_local_energy_forces_h"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -192,6 +193,27 @@ class Hamiltonian:
                 _dev(b, torch.complex64, "b"), _dev(W, torch.complex64, "W"), ctypes.c_void_p(eloc.data_ptr()),
                 ctypes.c_void_p(logpsi.data_ptr()) if want_logpsi else None, _stream()))
         return (eloc, logpsi) if want_logpsi else eloc
+
+    def local_energy_forces(self, spins, a, b, W, weights=None):
+        """nqs_local_energy_forces_h: (E_loc [B], log psi [B], F [N + M + M*N], stats [4] float64)."""
+        import torch
+
+        B, N, M = _shapes(spins, a, b, W)
+        if N != self.N:
+            raise ValueError("N mismatch with the compiled Hamiltonian")
+        dev = spins.device
+        eloc = torch.empty(B, dtype=torch.complex64, device=dev)
+        logpsi = torch.empty(B, dtype=torch.complex64, device=dev)
+        F = torch.empty(N + M + M * N, dtype=torch.complex64, device=dev)
+        stats = torch.empty(4, dtype=torch.float64, device=dev)
+        with torch.cuda.device(dev):
+            _check(load_library().nqs_local_energy_forces_h(
+                self._h, _dev(spins, torch.int8, "spins"), B, M, _dev(a, torch.complex64, "a"),
+                _dev(b, torch.complex64, "b"), _dev(W, torch.complex64, "W"),
+                _dev(weights, torch.float32, "weights") if weights is not None else None,
+                ctypes.c_void_p(eloc.data_ptr()), ctypes.c_void_p(logpsi.data_ptr()), ctypes.c_void_p(F.data_ptr()),
+                ctypes.c_void_p(stats.data_ptr()), _stream()))
+        return eloc, logpsi, F, stats
 
 
 def energy_stats(x, weights=None):

@@ -433,9 +433,11 @@ extern "C" int nqs_log_psi(const int8_t* d_spins, int64_t B, int32_t N, int32_t 
                         (cudaStream_t)stream);
 }
 
-extern "C" int nqs_local_energy_h(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int32_t M,
-                                  const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, nqs_c64* d_eloc,
-                                  nqs_c64* d_logpsi, void* stream) {
+// keep_tp != NULL: tanh(theta) ([M_pad][B_pad/2] float4, stream-ordered allocation) is handed to the
+// caller (who frees it with cudaFreeAsync) instead of being released -- nqs_local_energy_forces_h.
+static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int32_t M,
+                             const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, nqs_c64* d_eloc,
+                             nqs_c64* d_logpsi, void* stream, float4** keep_tp) {
     if (!h) return fail(NQS_ERR_INVALID_ARG, "hamiltonian handle is NULL");
     const int N = h->hc.N;
     int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
@@ -457,8 +459,8 @@ extern "C" int nqs_local_energy_h(const nqs_hamiltonian* h, const int8_t* d_spin
     float4 *tp = nullptr, *tab = nullptr, *rho = nullptr;
     float2* partial = nullptr;
     const bool have_cols = h->C > 0;
+    if (have_cols || keep_tp) NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
     if (have_cols) {
-        NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
         NQS_CUDA(cudaMallocAsync(&tab, sizeof(float4) * (size_t)nTiles * M_pad * TC, st));
         NQS_CUDA(cudaMallocAsync(&rho, sizeof(float4) * (size_t)C_pad, st));
         NQS_CUDA(cudaMallocAsync(&partial, sizeof(float2) * (size_t)B * nTiles, st));
@@ -470,7 +472,7 @@ extern "C" int nqs_local_energy_h(const nqs_hamiltonian* h, const int8_t* d_spin
         NQS_CUDA(cudaGetLastError());
     }
     if (have_cols) NQS_PROF(1, st);
-    if (have_cols || d_logpsi) {
+    if (have_cols || d_logpsi || keep_tp) {
         rc = launch_theta(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st);
         if (rc) return rc;
     }
@@ -498,12 +500,21 @@ extern "C" int nqs_local_energy_h(const nqs_hamiltonian* h, const int8_t* d_spin
     if (have_cols) {
         NQS_PROF(4, st);
         g_prof_valid = g_prof_on;
-        NQS_CUDA(cudaFreeAsync(tp, st));
         NQS_CUDA(cudaFreeAsync(tab, st));
         NQS_CUDA(cudaFreeAsync(rho, st));
         NQS_CUDA(cudaFreeAsync(partial, st));
     }
+    if (keep_tp)
+        *keep_tp = tp;
+    else if (tp)
+        NQS_CUDA(cudaFreeAsync(tp, st));
     return NQS_OK;
+}
+
+extern "C" int nqs_local_energy_h(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int32_t M,
+                                  const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, nqs_c64* d_eloc,
+                                  nqs_c64* d_logpsi, void* stream) {
+    return local_energy_impl(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream, nullptr);
 }
 
 extern "C" int nqs_local_energy(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
@@ -689,9 +700,10 @@ extern "C" int nqs_energy_stats(const nqs_c64* d_x, const float* d_weights, int6
     return launch_stats(d_x, d_weights, B, d_stats, (cudaStream_t)stream);
 }
 
-extern "C" int nqs_forces(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
-                          const nqs_c64* d_b, const nqs_c64* d_W, const nqs_c64* d_eloc, const float* d_weights,
-                          nqs_c64* d_F, double* d_stats, void* stream) {
+// tp_in != NULL: tanh(theta) of this batch from local_energy_impl (ownership passes to this function)
+static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
+                       const nqs_c64* d_b, const nqs_c64* d_W, const nqs_c64* d_eloc, const float* d_weights,
+                       nqs_c64* d_F, double* d_stats, void* stream, float4* tp_in) {
     int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
     if (rc) return rc;
     if (B <= 0 || !d_eloc || !d_F) return fail(NQS_ERR_INVALID_ARG, "nqs_forces: B <= 0 or NULL d_eloc / d_F");
@@ -704,12 +716,12 @@ extern "C" int nqs_forces(const int8_t* d_spins, int64_t B, int32_t N, int32_t M
     const int K16 = (int)(B_pad / 16);
     const int nIT = (N + 1 + TM_M - 1) / TM_M, nJT = (M + 1 + TM_JT - 1) / TM_JT;
 
-    float4* tp = nullptr;
+    float4* tp = tp_in;
     float2* cb = nullptr;
     double* stats = nullptr;
     int* gexp = nullptr;
     uint4 *A_packed = nullptr, *B_packed = nullptr;
-    NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
+    if (!tp) NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
     NQS_CUDA(cudaMallocAsync(&cb, sizeof(float2) * (size_t)B_pad, st));
     NQS_CUDA(cudaMallocAsync(&stats, sizeof(double) * 4, st));
     NQS_CUDA(cudaMallocAsync(&gexp, sizeof(int) * (size_t)nJT * TM_JT, st));
@@ -721,7 +733,7 @@ extern "C" int nqs_forces(const int8_t* d_spins, int64_t B, int32_t N, int32_t M
     force_coef_kernel<<<(unsigned)((B_pad + 255) / 256), 256, 0, st>>>((const float2*)d_eloc, d_weights, (long long)B,
                                                                        B_pad, stats, cb);
     NQS_CUDA(cudaGetLastError());
-    if ((rc = launch_theta(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st))) return rc;
+    if (!tp_in && (rc = launch_theta(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st))) return rc;
     force_gscale_kernel<<<(unsigned)(nJT * TM_JT), 256, 0, st>>>(tp, nPairsPad, cb, M, gexp);
     NQS_CUDA(cudaGetLastError());
     force_pack_g_kernel<<<148 * 8, 256, 0, st>>>(tp, nPairsPad, cb, M, K16, nJT, gexp, B_packed);
@@ -750,6 +762,25 @@ extern "C" int nqs_forces(const int8_t* d_spins, int64_t B, int32_t N, int32_t M
     NQS_CUDA(cudaFreeAsync(A_packed, st));
     NQS_CUDA(cudaFreeAsync(B_packed, st));
     return NQS_OK;
+}
+
+extern "C" int nqs_forces(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
+                          const nqs_c64* d_b, const nqs_c64* d_W, const nqs_c64* d_eloc, const float* d_weights,
+                          nqs_c64* d_F, double* d_stats, void* stream) {
+    return forces_impl(d_spins, B, N, M, d_a, d_b, d_W, d_eloc, d_weights, d_F, d_stats, stream, nullptr);
+}
+
+// One VMC evaluation step: E_loc, its statistics and the force vector of the same batch, with
+// theta / tanh(theta) computed once and shared by the two halves.
+extern "C" int nqs_local_energy_forces_h(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int32_t M,
+                                         const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W,
+                                         const float* d_weights, nqs_c64* d_eloc, nqs_c64* d_logpsi, nqs_c64* d_F,
+                                         double* d_stats, void* stream) {
+    if (B <= 0 || !d_F) return fail(NQS_ERR_INVALID_ARG, "nqs_local_energy_forces_h: B <= 0 or NULL d_F");
+    float4* tp = nullptr;
+    int rc = local_energy_impl(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream, &tp);
+    if (rc) return rc;
+    return forces_impl(d_spins, B, h->hc.N, M, d_a, d_b, d_W, d_eloc, d_weights, d_F, d_stats, stream, tp);
 }
 
 // ----------------------------------------------------------------------------------------

@@ -145,3 +145,19 @@ def test_forces_error_codes(nqs):
     lib = nqs.load_library()
     assert lib.nqs_forces(None, 4, 8, 8, None, None, None, None, None, None, None, None) == -1
     assert lib.nqs_energy_stats(None, None, 0, None, None) == -1
+
+
+def test_fused_local_energy_forces_equals_the_two_calls(nqs):
+    import torch
+
+    d = torch.device("cuda:0")
+    for k, B in ((2, 3000), (4, 1111)):
+        w = wl.make_config(k, B=B)
+        t = lambda x: torch.from_numpy(np.ascontiguousarray(x)).to(d)  # noqa: E731
+        spins, a, b, W = t(w.spins), t(w.a), t(w.b), t(w.W)
+        ham = nqs.Hamiltonian(w.N, w.ham.sites, w.ham.paulis, w.ham.coeffs)
+        e1, l1 = ham.local_energy(spins, a, b, W)
+        F1, s1 = nqs.forces(spins, a, b, W, e1, want_stats=True)
+        e2, l2, F2, s2 = ham.local_energy_forces(spins, a, b, W)
+        torch.cuda.synchronize()
+        assert torch.equal(e1, e2) and torch.equal(l1, l2) and torch.equal(F1, F2) and torch.equal(s1, s2)
