@@ -329,3 +329,23 @@ def test_error_codes(nqs):
         host.local_energy(spins, a, b, W)
     assert ei.value.code == -1
     torch.cuda.synchronize()
+
+
+def test_large_N_takes_the_simt_theta_kernel(nqs, oracle):
+    """N > 512 is outside the tensor-core theta kernel (its spins tile lives in shared memory); the
+    FP32 SIMT theta_kernel takes over.  Same tolerances; also through nqs_log_psi alone."""
+    import torch
+
+    N, M, B = 530, 48, 300
+    a, b, W = wl.rbm_parameters(N, M, 0.03, [91, 0])
+    ham = wl.tfim(wl.chain_bonds(N), N, 1.0, 0.8)
+    spins = wl.iid_spins(B, N, [91, 1])
+    w = wl.Workload("chain_N530", N, M, B, spins, a, b, W, ham)
+    e, l = gpu_eloc(nqs, w)
+    e_ref, l_ref = oracle.local_energy_fast(w.spins, w.a, w.b, w.W, w.ham.sites, w.ham.paulis, w.ham.coeffs)
+    check_eloc(e, e_ref, "N=530")
+    check_logpsi(l, l_ref, "N=530")
+    sp, ad, bd, Wd = to_dev(w)
+    l2 = nqs.log_psi(sp, ad, bd, Wd)
+    torch.cuda.synchronize()
+    check_logpsi(l2.cpu().numpy(), l_ref, "N=530 nqs_log_psi")
