@@ -144,7 +144,8 @@ int nqs_profile_last(float ms[4]);
 /* ---------------------------------------------------------------------------------------
  * Batch statistics (Eq. 5; get_global_mean / get_global_variance, :511-515).
  *   d_x [B] complex64 (any local estimator, e.g. E_loc);  d_weights [B] float32 or NULL (= uniform;
- *   with w_b = p(s_b) over a full basis the mean is the exact expectation of Eq. 3).
+ *   with w_b = p(s_b) over a full basis the mean is the exact expectation of Eq. 3).  Weights must be
+ *   non-negative with a positive sum (otherwise the outputs are NaN, no error is raised).
  *   d_stats [4] float64 DEVICE out: Re mean, Im mean, variance <<|x - mean|^2>>, sum of weights.
  * Sums are accumulated in float64 in a fixed order (deterministic).  Asynchronous on `stream`.
  * ------------------------------------------------------------------------------------- */
