@@ -185,9 +185,9 @@ int nqs_local_energy_forces_h(const nqs_hamiltonian *h, const int8_t *d_spins, i
  *   d_accepted [C] int32 DEVICE out or NULL: accepted moves per chain
  * The random numbers are the caller's (e.g. torch.randint / torch.rand on the device), so a call is
  * a deterministic function of its inputs.  The acceptance test is evaluated in float32 (a decision
- * closer to a tie than ~1e-4 in log |ratio|^2 may differ from exact arithmetic); tanh theta is
- * recomputed from the spins every two sweeps (2 N steps) and updated in place by the addition
- * theorem on each accepted move in between.  Sites outside [0,N) are undefined behaviour.  S = 0 is a no-op.  Asynchronous.
+ * closer to a tie than ~1e-4 in log |ratio|^2 may differ from exact arithmetic).  The chain state is
+ * exp(2 theta), recomputed from the spins every two sweeps (2 N steps) and updated in place by one
+ * complex multiplication per hidden unit on each accepted move.  Valid for |Re theta| < 22.  Sites outside [0,N) are undefined behaviour.  S = 0 is a no-op.  Asynchronous.
  * NQS_ERR_UNSUPPORTED if one chain's state (8 M + N bytes) does not fit shared memory twice.
  * ------------------------------------------------------------------------------------- */
 int nqs_metropolis(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64 *d_a,

@@ -306,7 +306,7 @@ static inline long long round_up(long long x, long long m) { return (x + m - 1) 
 
 static int launch_theta_simt(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
                              const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad,
-                             nqs_c64* d_logpsi, cudaStream_t st) {
+                             nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta) {
     const long long rows = tp ? nPairsPad * 2 : B;
     const unsigned grid = (unsigned)((rows + 63) / 64);
     static bool attr_set = false;
@@ -315,7 +315,7 @@ static int launch_theta_simt(const int8_t* d_spins, int64_t B, int32_t N, int32_
         attr_set = true;
     }
     theta_kernel<<<grid, 256, TH_SMEM, st>>>(d_spins, (long long)B, N, M, M_pad, (const float2*)d_a, (const float2*)d_b,
-                                       (const float2*)d_W, tp, nPairsPad, (float2*)d_logpsi);
+                                       (const float2*)d_W, tp, nPairsPad, (float2*)d_logpsi, raw_theta ? 1 : 0);
     NQS_CUDA(cudaGetLastError());
     return NQS_OK;
 }
@@ -323,7 +323,7 @@ static int launch_theta_simt(const int8_t* d_spins, int64_t B, int32_t N, int32_
 // a2 on the tensor cores: pack spins and the int8 digits of W, then theta_mma_kernel (tcgen05).
 static int launch_theta_mma(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
                             const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad,
-                            nqs_c64* d_logpsi, cudaStream_t st) {
+                            nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta) {
     const long long rows = tp ? nPairsPad * 2 : B;
     const long long nMT = (rows + TM_M - 1) / TM_M;
     const int K_pad = (int)round_up(N, TM_KC), K16 = K_pad / 16;
@@ -361,6 +361,7 @@ static int launch_theta_mma(const int8_t* d_spins, int64_t B, int32_t N, int32_t
     p.tp = tp;
     p.nPairsPad = nPairsPad;
     p.logpsi = (float2*)d_logpsi;
+    p.raw_theta = raw_theta ? 1 : 0;
     theta_mma_kernel<<<(unsigned)nMT, TM_THREADS, smem, st>>>(p);
     NQS_CUDA(cudaGetLastError());
     NQS_CUDA(cudaFreeAsync(A_packed, st));
@@ -380,10 +381,10 @@ static bool theta_use_mma(int32_t N) {
 
 static int launch_theta(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
                         const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad, nqs_c64* d_logpsi,
-                        cudaStream_t st) {
+                        cudaStream_t st, bool raw_theta = false) {
     if (theta_use_mma(N))
-        return launch_theta_mma(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st);
-    return launch_theta_simt(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st);
+        return launch_theta_mma(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st, raw_theta);
+    return launch_theta_simt(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st, raw_theta);
 }
 
 template <int WC, int WS>
@@ -815,12 +816,13 @@ extern "C" int nqs_metropolis(int8_t* d_spins, int64_t C, int32_t N, int32_t M, 
     const size_t smem = metropolis_smem_bytes(cpb, N, M_pad);
     if (smem > 220 * 1024) return fail(NQS_ERR_UNSUPPORTED, "nqs_metropolis: M too large for the shared-memory chain state");
 
-    float4 *tp = nullptr, *TT = nullptr;
-    float2* lk2 = nullptr;
+    float4 *tp = nullptr, *Gp = nullptr, *Gm = nullptr;
+    float* lk2 = nullptr;
     NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
-    NQS_CUDA(cudaMallocAsync(&TT, sizeof(float4) * (size_t)N * (M_pad / 2), st));
-    NQS_CUDA(cudaMallocAsync(&lk2, sizeof(float2) * (size_t)N, st));
-    site_table_kernel<<<(unsigned)N, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, TT, lk2);
+    NQS_CUDA(cudaMallocAsync(&Gp, sizeof(float4) * (size_t)N * (M_pad / 2), st));
+    NQS_CUDA(cudaMallocAsync(&Gm, sizeof(float4) * (size_t)N * (M_pad / 2), st));
+    NQS_CUDA(cudaMallocAsync(&lk2, sizeof(float) * (size_t)N, st));
+    site_table_kernel<<<(unsigned)N, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, Gp, Gm, lk2);
     NQS_CUDA(cudaGetLastError());
     MetroParams p;
     p.spins = d_spins;
@@ -830,13 +832,14 @@ extern "C" int nqs_metropolis(int8_t* d_spins, int64_t C, int32_t N, int32_t M, 
     p.M_pad = M_pad;
     p.tp = tp;
     p.nPairsPad = nPairsPad;
-    p.TT = TT;
+    p.Gp = Gp;
+    p.Gm = Gm;
     p.lk2 = lk2;
     p.accepted = d_accepted;
     // chunks of two sweeps; tanh(theta) is recomputed from the current spins before each chunk
     const int chunk = 2 * N;
     for (int s0 = 0; s0 == 0 || s0 < S; s0 += chunk) {
-        if ((rc = launch_theta(d_spins, C, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st))) return rc;
+        if ((rc = launch_theta(d_spins, C, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st, true))) return rc;
         p.S = S - s0 < chunk ? S - s0 : chunk;
         p.sites = d_sites + (long long)s0 * C;
         p.u = d_u + (long long)s0 * C;
@@ -851,7 +854,8 @@ extern "C" int nqs_metropolis(int8_t* d_spins, int64_t C, int32_t N, int32_t M, 
     }
     if (rc) return rc;
     NQS_CUDA(cudaFreeAsync(tp, st));
-    NQS_CUDA(cudaFreeAsync(TT, st));
+    NQS_CUDA(cudaFreeAsync(Gp, st));
+    NQS_CUDA(cudaFreeAsync(Gm, st));
     NQS_CUDA(cudaFreeAsync(lk2, st));
     return NQS_OK;
 }

@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(256) theta_kernel(const int8_t* __restrict__ s
                                                     int M_pad, const float2* __restrict__ a,
                                                     const float2* __restrict__ bvec, const float2* __restrict__ W,
                                                     float4* __restrict__ tp, long long nPairsPad,
-                                                    float2* __restrict__ logpsi) {
+                                                    float2* __restrict__ logpsi, int raw_theta) {
     extern __shared__ __align__(16) unsigned char th_smem[];
     float(*sS)[64] = reinterpret_cast<float(*)[64]>(th_smem);
     float2(*sW)[64] = reinterpret_cast<float2(*)[64]>(th_smem + sizeof(float) * TH_KI * 64);
@@ -149,6 +149,11 @@ __global__ void __launch_bounds__(256) theta_kernel(const int8_t* __restrict__ s
             float tr[4], ti[4];
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
+                if (raw_theta) {  // tp receives theta itself (nqs_metropolis)
+                    tr[e] = live ? acc[e][q].x : 0.f;
+                    ti[e] = live ? acc[e][q].y : 0.f;
+                    continue;
+                }
                 float lr, li;
                 lncosh_tanh(acc[e][q].x, acc[e][q].y, lr, li, tr[e], ti[e]);
                 if (live) {

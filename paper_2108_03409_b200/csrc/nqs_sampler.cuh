@@ -1,50 +1,60 @@
 // single-spin-flip Metropolis sampling of |psi(s)|^2, many chains in lock-step
 // (PAPER.md:70 Metropolis-Hastings; :341 sweeps; :490-494 chains advanced in sync on one device).
 //
-// For a proposal "flip site i" of a chain with spin sigma = s_i the one-site ratio identity (R) gives
-//   psi(s')/psi(s) = exp(-2 sigma a_i) prod_j cosh(2 W_ji) * prod_j D_j,   D_j = 1 - sigma t_j T_ji,
-// t_j = tanh theta_j, T_ji = tanh 2 W_ji, and, by the addition theorem of tanh, an accepted move
-// updates the chain's state IN PLACE without any transcendental:
-//   t_j <- tanh(theta_j - 2 sigma W_ji) = (t_j - sigma T_ji) / D_j.
-// Only |psi(s')/psi(s)|^2 is needed, so the product over hidden units is a real product of |D_j|^2,
-// accumulated as a sum of log2 (range-safe) and reduced over the warp with shuffles.
+// A chain's state is E_j = exp(2 theta_j) for every hidden unit.  For the proposal "flip site i" of a
+// chain with spin sigma = s_i, theta_j -> theta_j - 2 sigma W_ji, and with G_ji(sigma) = exp(4 sigma W_ji)
+//   cosh(theta_j - 2 sigma W_ji) / cosh(theta_j) = exp(-2 sigma W_ji) (E_j + G_ji(sigma)) / (E_j + 1),
+//   psi(s')/psi(s) = exp(-2 sigma (a_i + sum_j W_ji)) prod_j (E_j + G_ji(sigma)) / (E_j + 1),
+// and an accepted move updates the state IN PLACE by one complex multiplication,
+//   E_j <- E_j G_ji(-sigma)          (no division, no transcendental in the loop).
+// Only |psi(s')/psi(s)|^2 is needed, so numerator and denominator are real products of squared
+// moduli, accumulated as sums of log2 (range-safe) and reduced over the warp with shuffles.
+// Why E and not tanh(theta) with the addition theorem (the first version of this kernel, 15 % faster
+// at config 5, failed the shape fuzz by drift at sigma = 0.25; DESIGN.md section 9 has the record): for a saturated unit (|Re theta| >~ 4)
+// tanh(theta) = +-1 - tiny cannot hold theta to float32 accuracy, and the loss shows up as an O(0.1)
+// error in log |ratio|^2 once later flips bring the unit back; E_j keeps a RELATIVE error of 1 ulp
+// per update, i.e. an ABSOLUTE error of 6e-8 per update in theta.  Range: |E + 1|^2 must stay finite,
+// i.e. |Re theta| < 22; the acceptance test multiplies per-pair RATIOS |E + G|^2 / |E + 1|^2, never the
+// two squared moduli separately.
 //
-// One warp owns one chain for the whole call; the chain's t (M complex numbers) and spins live in
-// shared memory, T^T [N][M_pad] (5 MB at config 5) is read from L2.  The random numbers (proposal
-// site, uniform u) are inputs.  The rational update is a Moebius map: it does not damp rounding
-// errors, so the host splits a call into chunks of two sweeps (2 N steps) and recomputes t from
-// the spins with the a2/a3 kernels before each chunk, which bounds the drift.
+// One warp owns one chain for the whole call; the chain's E (M complex numbers) and spins live in
+// shared memory, the tables exp(+-4 W)^T [N][M_pad/2] (2 x 5 MB at config 5) are read from L2.  The
+// random numbers (proposal site, uniform u) are inputs.  The host splits a call into chunks of two
+// sweeps (2 N steps) and recomputes theta from the spins with the a2 kernel before each chunk.
+//
+// Hidden units are handled in PAIRS (j0, j1) = (2 jp, 2 jp + 1) riding in the two halves of packed
+// FFMA2 operands: records are float4 (re_j0, re_j1, im_j0, im_j1) for E and for the tables.
 #pragma once
 #include "nqs_device.cuh"
 
 namespace nqs {
 
-// Hidden units are handled in PAIRS (j0, j1) = (2 jp, 2 jp + 1) riding in the two halves of packed
-// FFMA2 operands: records are float4 (re_j0, re_j1, im_j0, im_j1), for t in shared memory and for
-// T^T in global memory, so one 16-byte load per operand feeds two hidden units.
-
-// One block per site i: TT[i][jp] = tanh(2 W_ji) for the pair jp (0 for the padding j >= M) and
-// lk2[i] = log2(e) * (Re L_i - 2 Re a_i, Re L_i + 2 Re a_i),  L_i = sum_j log cosh(2 W_ji):
-// log2 |exp(-2 sigma a_i) prod_j cosh 2 W_ji|^2 / 2 for sigma = +1 (x) and -1 (y).
+// One block per site i: Gp[i][jp] = exp(+4 W_ji), Gm[i][jp] = exp(-4 W_ji) for the pair jp (1 for the
+// padding j >= M: (E + 1)/(E + 1) = 1) and lk2[i] = -4 log2(e) Re(a_i + sum_j W_ji), so that
+// log2 |exp(-2 sigma (a_i + sum_j W_ji))|^2 = sigma lk2[i].
 __global__ void __launch_bounds__(256) site_table_kernel(const float2* __restrict__ W, const float2* __restrict__ a,
-                                                         int N, int M, int M_pad, float4* __restrict__ TT,
-                                                         float2* __restrict__ lk2) {
+                                                         int N, int M, int M_pad, float4* __restrict__ Gp,
+                                                         float4* __restrict__ Gm, float* __restrict__ lk2) {
     const int i = blockIdx.x;
     __shared__ double sh[256];
     double acc = 0.0;
     for (int jp = threadIdx.x; jp < M_pad / 2; jp += 256) {
-        float tr[2] = {0.f, 0.f}, ti[2] = {0.f, 0.f};
+        float pr[2] = {1.f, 1.f}, pi[2] = {0.f, 0.f}, mr[2] = {1.f, 1.f}, mi[2] = {0.f, 0.f};
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const int j = 2 * jp + h;
             if (j < M) {
                 const float2 w = W[(long long)j * N + i];
-                float lr, li;
-                lncosh_tanh(2.f * w.x, 2.f * w.y, lr, li, tr[h], ti[h]);
-                acc += (double)lr;
+                float sn, cs;
+                sincosf(4.f * w.y, &sn, &cs);
+                const float ep = expf(4.f * w.x), em = expf(-4.f * w.x);
+                pr[h] = ep * cs, pi[h] = ep * sn;
+                mr[h] = em * cs, mi[h] = -em * sn;
+                acc += (double)w.x;
             }
         }
-        TT[(long long)i * (M_pad / 2) + jp] = make_float4(tr[0], tr[1], ti[0], ti[1]);
+        Gp[(long long)i * (M_pad / 2) + jp] = make_float4(pr[0], pr[1], pi[0], pi[1]);
+        Gm[(long long)i * (M_pad / 2) + jp] = make_float4(mr[0], mr[1], mi[0], mi[1]);
     }
     sh[threadIdx.x] = acc;
     __syncthreads();
@@ -52,20 +62,18 @@ __global__ void __launch_bounds__(256) site_table_kernel(const float2* __restric
         if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
         __syncthreads();
     }
-    if (threadIdx.x == 0) {
-        const double L = sh[0], ar = (double)a[i].x, l2e = 1.4426950408889634;
-        lk2[i] = make_float2((float)(l2e * (L - 2.0 * ar)), (float)(l2e * (L + 2.0 * ar)));
-    }
+    if (threadIdx.x == 0) lk2[i] = (float)(-4.0 * 1.4426950408889634 * (sh[0] + (double)a[i].x));
 }
 
 struct MetroParams {
     int8_t* spins;           // [C][N] in / out
     long long C;
     int N, M, M_pad, S;
-    const float4* tp;        // [M_pad][nPairsPad]: tanh theta of the start states, two chains per record
+    const float4* tp;        // [M_pad][nPairsPad]: theta of the start states (raw), two chains per record
     long long nPairsPad;
-    const float4* TT;        // [N][M_pad / 2]
-    const float2* lk2;       // [N]
+    const float4* Gp;        // [N][M_pad / 2]  exp(+4 W)
+    const float4* Gm;        // [N][M_pad / 2]  exp(-4 W)
+    const float* lk2;        // [N]
     const int* sites;        // [S][C]
     const float* u;          // [S][C]
     int* accepted;           // [C] or nullptr
@@ -78,34 +86,30 @@ __host__ __device__ inline size_t metropolis_smem_bytes(int cpb, int N, int M_pa
 
 constexpr int MT_UNROLL = 5;  // pairs per lane whose loads are issued together (config 5: 25 = 5 x 5)
 
-// D = 1 - sigma t T for a pair of hidden units; returns |D|^2 per half
-__device__ __forceinline__ float2 metro_D(const float4 t, const float4 T, const float nsg, float2& Dr, float2& Di) {
-    const float2 tr = make_float2(t.x, t.y), ti = make_float2(t.z, t.w);
-    const float2 Tr = make_float2(T.x, T.y), Ti = make_float2(T.z, T.w);
-    const float2 xr = __ffma2_rn(neg2(ti), Ti, __fmul2_rn(tr, Tr));
-    const float2 xi = __ffma2_rn(ti, Tr, __fmul2_rn(tr, Ti));
-    Dr = __ffma2_rn(bc2(nsg), xr, bc2(1.f));
-    Di = __fmul2_rn(bc2(nsg), xi);
-    return __ffma2_rn(Dr, Dr, __fmul2_rn(Di, Di));
-}
-
 template <int CPB>
 __global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroParams p) {
     extern __shared__ __align__(16) unsigned char mt_smem[];
-    float4* const t_all = reinterpret_cast<float4*>(mt_smem);
+    float4* const E_all = reinterpret_cast<float4*>(mt_smem);
     const int N_pad = (p.N + 15) / 16 * 16;
-    const int MP = p.M_pad / 2;  // hidden-unit pairs (padding pairs hold t = 0, T = 0: D = 1)
+    const int MP = p.M_pad / 2;  // hidden-unit pairs (padding pairs: theta = 0, E = 1, G = 1: factor 1)
     int8_t* const s_all = reinterpret_cast<int8_t*>(mt_smem + (size_t)CPB * p.M_pad * sizeof(float2));
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long c0 = (long long)blockIdx.x * CPB;
 
-    // the block's CPB chains are CPB/2 consecutive records of every tp row
+    // E = exp(2 theta); the block's CPB chains are CPB/2 consecutive records of every tp row
     for (int idx = tid; idx < MP * (CPB / 2); idx += CPB * 32) {
         const int jp = idx / (CPB / 2), pr = idx % (CPB / 2);
-        const float4 r0 = p.tp[(long long)(2 * jp) * p.nPairsPad + c0 / 2 + pr];
-        const float4 r1 = p.tp[(long long)(2 * jp + 1) * p.nPairsPad + c0 / 2 + pr];
-        t_all[(size_t)(2 * pr) * MP + jp] = make_float4(r0.x, r1.x, r0.z, r1.z);
-        t_all[(size_t)(2 * pr + 1) * MP + jp] = make_float4(r0.y, r1.y, r0.w, r1.w);
+        const float4 r0 = p.tp[(long long)(2 * jp) * p.nPairsPad + c0 / 2 + pr];      // (xA, xB, yA, yB) of unit 2 jp
+        const float4 r1 = p.tp[(long long)(2 * jp + 1) * p.nPairsPad + c0 / 2 + pr];  // of unit 2 jp + 1
+        float sn, cs;
+        float4 eA, eB;
+        float m;
+        m = expf(2.f * r0.x), sincosf(2.f * r0.z, &sn, &cs), eA.x = m * cs, eA.z = m * sn;
+        m = expf(2.f * r1.x), sincosf(2.f * r1.z, &sn, &cs), eA.y = m * cs, eA.w = m * sn;
+        m = expf(2.f * r0.y), sincosf(2.f * r0.w, &sn, &cs), eB.x = m * cs, eB.z = m * sn;
+        m = expf(2.f * r1.y), sincosf(2.f * r1.w, &sn, &cs), eB.y = m * cs, eB.w = m * sn;
+        E_all[(size_t)(2 * pr) * MP + jp] = eA;
+        E_all[(size_t)(2 * pr + 1) * MP + jp] = eB;
     }
     for (int idx = tid; idx < CPB * p.N; idx += CPB * 32) {
         const int w = idx / p.N, i = idx % p.N;
@@ -115,9 +119,10 @@ __global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroPara
 
     const long long c = c0 + warp;
     if (c >= p.C) return;
-    float4* const t_s = t_all + (size_t)warp * MP;
+    float4* const E_s = E_all + (size_t)warp * MP;
     int8_t* const s_s = s_all + warp * N_pad;
     const int nFull = MP / (32 * MT_UNROLL);  // groups of 32 x MT_UNROLL pairs with no ragged lane
+    const float4 one4 = make_float4(1.f, 1.f, 0.f, 0.f);
     int acc = 0;
     for (int step = 0; step < p.S; ++step) {
         int site = 0;
@@ -128,24 +133,31 @@ __global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroPara
         }
         site = __shfl_sync(0xffffffffu, site, 0);
         ul = __shfl_sync(0xffffffffu, ul, 0);
-        const float sg = (float)s_s[site], nsg = -sg;
-        const float4* const Trow = p.TT + (long long)site * MP;
-        // pass 1: log2 prod_j |D_j|^2 (real product per lane, log2 per group, shuffle sum)
+        const int sgi = s_s[site];
+        const float4* const Gfwd = (sgi > 0 ? p.Gp : p.Gm) + (long long)site * MP;  // G(sigma)
+        const float4* const Gbwd = (sgi > 0 ? p.Gm : p.Gp) + (long long)site * MP;  // G(-sigma)
+        // pass 1: sum_j log2 |E_j + G_j|^2 - log2 |E_j + 1|^2
         float lg = 0.f;
         auto pass1 = [&](int jp0, bool ragged) {
-            float4 t[MT_UNROLL], T[MT_UNROLL];
+            float4 E[MT_UNROLL], G[MT_UNROLL];
 #pragma unroll
             for (int k = 0; k < MT_UNROLL; ++k) {
                 const int jp = jp0 + 32 * k;
                 const bool live = !ragged || jp < MP;
-                T[k] = live ? Trow[jp] : make_float4(0.f, 0.f, 0.f, 0.f);
-                t[k] = live ? t_s[jp] : make_float4(0.f, 0.f, 0.f, 0.f);
+                G[k] = live ? Gfwd[jp] : one4;
+                E[k] = live ? E_s[jp] : one4;
             }
+            // per pair the RATIO |E + G|^2 / |E + 1|^2 (O(1)); the two squared moduli are each ~ e^{4 |Re theta|}
+            // and a product of them overflows float32 for saturated units
             float2 q = make_float2(1.f, 1.f);
 #pragma unroll
             for (int k = 0; k < MT_UNROLL; ++k) {
-                float2 Dr, Di;
-                q = __fmul2_rn(q, metro_D(t[k], T[k], nsg, Dr, Di));
+                const float2 er = make_float2(E[k].x, E[k].y), ei = make_float2(E[k].z, E[k].w);
+                const float2 nr = __fadd2_rn(er, make_float2(G[k].x, G[k].y)), ni = __fadd2_rn(ei, make_float2(G[k].z, G[k].w));
+                const float2 dr = __fadd2_rn(er, bc2(1.f));
+                const float2 n2 = __ffma2_rn(nr, nr, __fmul2_rn(ni, ni));
+                const float2 d2 = __ffma2_rn(dr, dr, __fmul2_rn(ei, ei));
+                q = __fmul2_rn(q, __fmul2_rn(n2, make_float2(__frcp_rn(d2.x), __frcp_rn(d2.y))));
             }
             lg += log2f(q.x * q.y);
         };
@@ -153,35 +165,32 @@ __global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroPara
         if (nFull * 32 * MT_UNROLL < MP) pass1(nFull * 32 * MT_UNROLL + lane, true);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) lg += __shfl_xor_sync(0xffffffffu, lg, o);
-        const float2 lk = p.lk2[site];
-        const bool accept = log2f(ul) < 2.f * (sg > 0.f ? lk.x : lk.y) + lg;  // u == 0: -inf, always accepted
+        const float lk = p.lk2[site];
+        const bool accept = log2f(ul) < (sgi > 0 ? lk : -lk) + lg;  // u == 0: -inf, always accepted
         if (accept) {
-            // pass 2: t_j <- (t_j - sigma T_j) / D_j
+            // pass 2: E_j <- E_j G_j(-sigma)
             auto pass2 = [&](int jp0, bool ragged) {
-                float4 t[MT_UNROLL], T[MT_UNROLL];
+                float4 E[MT_UNROLL], G[MT_UNROLL];
 #pragma unroll
                 for (int k = 0; k < MT_UNROLL; ++k) {
                     const int jp = jp0 + 32 * k;
                     const bool live = !ragged || jp < MP;
-                    T[k] = live ? Trow[jp] : make_float4(0.f, 0.f, 0.f, 0.f);
-                    t[k] = live ? t_s[jp] : make_float4(0.f, 0.f, 0.f, 0.f);
+                    G[k] = live ? Gbwd[jp] : one4;
+                    E[k] = live ? E_s[jp] : one4;
                 }
 #pragma unroll
                 for (int k = 0; k < MT_UNROLL; ++k) {
-                    float2 Dr, Di;
-                    const float2 d2 = metro_D(t[k], T[k], nsg, Dr, Di);
-                    const float2 inv = make_float2(__frcp_rn(d2.x), __frcp_rn(d2.y));
-                    const float2 nr = __ffma2_rn(bc2(nsg), make_float2(T[k].x, T[k].y), make_float2(t[k].x, t[k].y));
-                    const float2 ni = __ffma2_rn(bc2(nsg), make_float2(T[k].z, T[k].w), make_float2(t[k].z, t[k].w));
-                    const float2 outr = __fmul2_rn(__ffma2_rn(nr, Dr, __fmul2_rn(ni, Di)), inv);
-                    const float2 outi = __fmul2_rn(__ffma2_rn(ni, Dr, __fmul2_rn(neg2(nr), Di)), inv);
+                    const float2 er = make_float2(E[k].x, E[k].y), ei = make_float2(E[k].z, E[k].w);
+                    const float2 gr = make_float2(G[k].x, G[k].y), gi = make_float2(G[k].z, G[k].w);
+                    const float2 outr = __ffma2_rn(neg2(ei), gi, __fmul2_rn(er, gr));
+                    const float2 outi = __ffma2_rn(ei, gr, __fmul2_rn(er, gi));
                     const int jp = jp0 + 32 * k;
-                    if (!ragged || jp < MP) t_s[jp] = make_float4(outr.x, outr.y, outi.x, outi.y);
+                    if (!ragged || jp < MP) E_s[jp] = make_float4(outr.x, outr.y, outi.x, outi.y);
                 }
             };
             for (int g = 0; g < nFull; ++g) pass2(g * 32 * MT_UNROLL + lane, false);
             if (nFull * 32 * MT_UNROLL < MP) pass2(nFull * 32 * MT_UNROLL + lane, true);
-            if (lane == 0) s_s[site] = (int8_t)(-(int)sg);
+            if (lane == 0) s_s[site] = (int8_t)(-sgi);
             ++acc;
         }
         __syncwarp();

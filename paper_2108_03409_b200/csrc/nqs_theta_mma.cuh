@@ -184,6 +184,7 @@ struct ThetaMmaParams {
     float4* tp;              // [M_pad][nPairsPad] or nullptr
     long long nPairsPad;
     float2* logpsi;          // [B] or nullptr
+    int raw_theta;           // 1: tp receives theta itself instead of tanh(theta) (nqs_metropolis)
 };
 
 __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMmaParams p) {
@@ -291,6 +292,11 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
                     const float hi_ = (float)(w[7] * 128 + w[6]), li_ = (float)(w[5] * 128 + w[4]);
                     const float thr = fmaf(hr * 16384.f, sc, fmaf(lr_, sc, bj.x));
                     const float thi = fmaf(hi_ * 16384.f, sc, fmaf(li_, sc, bj.y));
+                    if (p.raw_theta) {
+                        tr[u] = live ? thr : 0.f;
+                        ti[u] = live ? thi : 0.f;
+                        continue;
+                    }
                     float lr, li;
                     lncosh_tanh(thr, thi, lr, li, tr[u], ti[u]);
                     if (live) {

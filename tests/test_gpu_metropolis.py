@@ -4,8 +4,10 @@ Floating point decides an integer here (accept / reject), and the kernel takes t
 float32 from a product form the oracle does not use.  So: the oracle reports for
 every chain how close its closest decision was to a tie (min_margin, in log |ratio|^2); chains whose
 margin exceeds MARGIN must come out BIT-IDENTICAL (final spins and accepted count); the others must
-still be valid configurations.  MARGIN = 2e-4 is ~10x the float32 error of log |ratio|^2 (<= ~2e-5 at
-these sizes) and keeps > 85 % of the chains in the exact comparison.
+still be valid configurations.  MARGIN and the robust-fraction floor were set empirically, after a
+first choice (1e-3, >= 90 %) failed on the robust fraction: 2e-4 is about 10x the float32 error of
+log |ratio|^2 seen at these sizes.  See DESIGN.md section 9 for the two kernel formulations this rule
+was run against and which cases each failed.
 """
 import numpy as np
 import pytest
@@ -58,7 +60,8 @@ def compare(final, acc, ref_final, ref_acc, margin, what, min_robust=0.85):
     (40, 80, 1000, 200, 0.05, 2),   # config-2 shapes, 5 sweeps
     (37, 45, 333, 150, 0.2, 3),     # ragged sizes, chains not a multiple of the block
     (100, 400, 2048, 100, 0.03, 4), # config-3 shapes, one sweep
-    (20, 30, 64, 2000, 0.25, 5),    # long chains: drift of the in-place tanh update over 100 sweeps
+    (20, 30, 64, 2000, 0.25, 5),    # long chains: drift of the in-place update over 100 sweeps
+    (142, 95, 463, 227, 0.25, 6),   # saturated hidden units (|Re theta| up to ~13): range of the ratio product
 ])
 def test_metropolis_vs_oracle(nqs, oracle, N, M, C, S, sigma, seed):
     w = wl.make_random(N, M, C, 4, sigma, 200 + seed)
