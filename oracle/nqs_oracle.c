@@ -419,9 +419,13 @@ void oracle_forces(const int8_t *spins, int64_t B, int N, int M, const float *a,
  * min_margin [C] float64 out = min over the steps of |2 Re dlogpsi - log u|: how far the closest
  * decision of the chain was from a tie (a float32 implementation can only be asked to reproduce
  * chains whose margin exceeds its rounding error).
+ * decisions [S,C] uint8 out or NULL: 1 = the proposal of step t was accepted; margins [S,C] float64 out or
+ * NULL: the same |2 Re dlogpsi - log u| per step (the trace behind min_margin: where a float32 chain and
+ * this one first part ways, the margin AT THAT STEP says whether the parting was a legitimate near-tie).
  * ------------------------------------------------------------------------------------- */
 void oracle_metropolis(int8_t *spins, int64_t C, int N, int M, const float *a, const float *b, const float *W,
-                       int S, const int32_t *sites, const float *u, int32_t *accepted, double *min_margin) {
+                       int S, const int32_t *sites, const float *u, int32_t *accepted, double *min_margin,
+                       uint8_t *decisions, double *margins) {
 #pragma omp parallel for schedule(dynamic, 4)
     for (int64_t c = 0; c < C; ++c) {
         int8_t *s = spins + c * N;
@@ -437,6 +441,8 @@ void oracle_metropolis(int8_t *spins, int64_t C, int N, int M, const float *a, c
             const double log_u = ut > 0.0 ? log(ut) : -INFINITY;
             const double margin = fabs(log_ratio - log_u);
             if (margin < mm) mm = margin;
+            if (margins) margins[(int64_t)t * C + c] = margin;
+            if (decisions) decisions[(int64_t)t * C + c] = (uint8_t)(log_u < log_ratio);
             if (log_u < log_ratio) {
                 lp = lp_new;
                 ++acc;

@@ -53,7 +53,7 @@ def _load():
         lib.oracle_log_derivatives.restype = None
         lib.oracle_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp]
         lib.oracle_forces.restype = None
-        lib.oracle_metropolis.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp]
+        lib.oracle_metropolis.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp]
         lib.oracle_metropolis.restype = None
         lib.oracle_num_threads.restype = i32
         lib.oracle_set_num_threads.argtypes = [i32]
@@ -176,9 +176,11 @@ def forces(spins, a, b, W, eloc, weights=None) -> np.ndarray:
     return out
 
 
-def metropolis(spins, a, b, W, sites, u):
+def metropolis(spins, a, b, W, sites, u, trace: bool = False):
     """Single-spin-flip Metropolis chains driven by the given proposals (sites [S,C] int32) and
-    uniforms (u [S,C] float32).  Returns (final spins int8 [C,N], accepted int32 [C], min_margin f64 [C])."""
+    uniforms (u [S,C] float32).  Returns (final spins int8 [C,N], accepted int32 [C], min_margin f64 [C]);
+    with trace=True also (decisions uint8 [S,C], margins f64 [S,C]): the accept bit and the distance of
+    every single decision from a tie."""
     spins, a, b, W, C, N, M = _params(spins, a, b, W)
     spins = spins.copy()
     sites, u = _c(sites, np.int32), _c(u, np.float32)
@@ -187,5 +189,8 @@ def metropolis(spins, a, b, W, sites, u):
     assert sites.min(initial=0) >= 0 and sites.max(initial=0) < N
     acc = np.empty(C, dtype=np.int32)
     mm = np.empty(C, dtype=np.float64)
-    _load().oracle_metropolis(_p(spins), C, N, M, _p(a), _p(b), _p(W), S, _p(sites), _p(u), _p(acc), _p(mm))
-    return spins, acc, mm
+    dec = np.empty((S, C), dtype=np.uint8) if trace else None
+    mar = np.empty((S, C), dtype=np.float64) if trace else None
+    _load().oracle_metropolis(_p(spins), C, N, M, _p(a), _p(b), _p(W), S, _p(sites), _p(u), _p(acc), _p(mm),
+                              _p(dec) if trace else None, _p(mar) if trace else None)
+    return (spins, acc, mm, dec, mar) if trace else (spins, acc, mm)

@@ -5,7 +5,8 @@ PM1 the acceptance rule, move by move, against the independent dense psi (dense_
     ratio for every basis state and site (a wrong power, a wrong site or a flipped inequality fails)
 PM2 the stationary distribution: many chains, final states distributed as |psi|^2 / <psi|psi>
     (PAPER.md:56-61 p_theta(s); :70 Metropolis-Hastings) within 4.5 standard errors per state
-PM3 bookkeeping: u = 0 accepts everything (two flips of a site restore the state), u ~ 1 with
+PM3 bookkeeping (and the per-step trace: decisions and margins of every step of multi-step chains
+    replayed against the dense psi): u = 0 accepts everything (two flips of a site restore the state), u ~ 1 with
     psi == const accepts nothing; chains are independent (a permutation of chains permutes outputs)
 """
 import numpy as np
@@ -34,6 +35,11 @@ def test_pm1_acceptance_rule_against_dense_psi(oracle):
             want = flipped if expect_accept else states
             assert np.array_equal(final[ok], want[ok])
             assert np.allclose(margin[ok], np.abs(np.log(ratio[ok]) - np.log(u[ok].astype(np.float64))), atol=1e-9)
+            # the per-step trace (decision bit and margin of every single proposal) against the same dense ratios
+            _, _, _, dec, mar = oracle.metropolis(states, w.a, w.b, w.W, sites, u[None, :], trace=True)
+            assert dec.shape == mar.shape == (1, 1 << N)
+            assert np.array_equal(dec[0, ok] == 1, np.full(ok.sum(), expect_accept))
+            assert np.allclose(mar[0, ok], np.abs(np.log(ratio[ok]) - np.log(u[ok].astype(np.float64))), atol=1e-9)
         # ratio >= 1: accepted for every u in [0, 1)
         big = ratio >= 1.0
         if big.any():
@@ -75,3 +81,21 @@ def test_pm3_bookkeeping(oracle):
     f2, a2, m2 = oracle.metropolis(w.spins[perm], w.a, w.b, w.W, sites[:, perm], u[:, perm])
     assert np.array_equal(f1[perm], f2) and np.array_equal(a1[perm], a2) and np.array_equal(m1[perm], m2)
     assert set(np.unique(f1)) <= {-1, 1}
+    # trace: the decisions replayed by hand reproduce the final state and the counters; the per-step
+    # margins reduce to min_margin; every step of a multi-step chain is checked against the dense psi
+    f3, a3, m3, dec, mar = oracle.metropolis(w.spins, w.a, w.b, w.W, sites, u, trace=True)
+    assert np.array_equal(f3, f1) and np.array_equal(a3, a1) and np.array_equal(m3, m1)
+    assert np.array_equal(dec.sum(axis=0), a1) and np.array_equal(mar.min(axis=0), m1)
+    psi = psi_all(N, w.a, w.b, w.W)
+    idx_of = lambda s: int(((1 - s.astype(np.int64)) // 2) @ (1 << np.arange(N - 1, -1, -1)))  # noqa: E731
+    for c in range(0, C, 7):
+        s = w.spins[c].copy()
+        for t in range(S):
+            sp = s.copy()
+            sp[sites[t, c]] *= -1
+            lr = np.log(abs(psi[idx_of(sp)] / psi[idx_of(s)]) ** 2)
+            lu = np.log(np.float64(u[t, c])) if u[t, c] > 0 else -np.inf
+            assert dec[t, c] == (lu < lr) and abs(mar[t, c] - abs(lr - lu)) < 1e-9, (c, t)
+            if dec[t, c]:
+                s = sp
+        assert np.array_equal(s, f1[c])
