@@ -25,17 +25,28 @@
  *     h_paulis, h_coeffs) are read before the call returns.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
  *     entry points are asynchronous on that stream and never synchronise the device.  Scratch
- *     memory (parameter tables, tanh(theta)) is taken from the CUDA stream-ordered allocator
- *     (cudaMallocAsync on `stream`) and returned to it before the call returns; no global
- *     mutable state is kept besides a small cache of compiled Hamiltonians.
+ *     memory (parameter tables, tanh(theta), packed GEMM operands) is taken in stream order from a
+ *     memory pool the library owns (one per device, cudaMallocFromPoolAsync on `stream`) and
+ *     returned to it on every exit path; freed scratch stays cached in that pool until
+ *     nqs_release() trims it.  Global mutable state: that pool, the per-device record of kernel
+ *     attributes, a cache of compiled Hamiltonians (at most 8, reference counted), the options of
+ *     nqs_set_option and the profiling events -- all guarded by mutexes / atomics except the
+ *     profiling helpers.
+ *   - The entry points that take a term list (nqs_local_energy, nqs_local_energy_host,
+ *     nqs_enumerate_connected) compile and upload the Hamiltonian on a cache miss; that upload is a
+ *     pageable-memory copy in stream order (the runtime may synchronise `stream` once for it, and a
+ *     miss cannot be captured into a CUDA graph).  A cache hit costs a key comparison.  An evicted
+ *     Hamiltonian is freed in stream order after its most recent use.
  *   - *_host entry points take HOST buffers, copy them to the device, run the same kernels,
  *     copy the result back and synchronise before returning.
  *   - Return value: 0 (NQS_OK) or a negative NQS_ERR_* code; nqs_last_error() then returns a
  *     thread-local message.  No partial results are promised on error.  B == 0 is a no-op.
  *   - There is NO CPU fallback: without a usable CUDA device every compute call returns
  *     NQS_ERR_CUDA.
- *   - Spin values other than +1/-1 are undefined behaviour.  psi(s) = 0 or overflow follow
- *     IEEE (inf/NaN in the output), not an error.
+ *   - Spin values other than +1/-1 are undefined behaviour, unless the environment variable
+ *     NQS_VALIDATE=1 is set (read at every call): then every entry point that takes device spins
+ *     checks them first, synchronises `stream`, and returns NQS_ERR_INVALID_ARG if any value is not
+ *     +1 or -1 (debug mode).  psi(s) = 0 or overflow follow IEEE (inf/NaN in the output), not an error.
  */
 #ifndef NQS_B200_H
 #define NQS_B200_H
@@ -120,26 +131,57 @@ int nqs_hamiltonian_info(const nqs_hamiltonian *h, int32_t info[5], int32_t *fli
 int nqs_hamiltonian_compile_host(int32_t N, int32_t T, const int32_t *h_sites, const uint8_t *h_paulis,
                                  const nqs_c64 *h_coeffs, nqs_hamiltonian **out);
 
+/* E_loc with a compiled handle.  The connected amplitudes (step a5) run on the tensor cores as a guarded
+ * series (csrc/nqs_series.cuh) when B * columns * M >= 2^28 and N <= 2048; the guard -- a per-sample bound on the
+ * series' own error against 0.5e-4 * max(1, |E_loc|) -- is evaluated on the device and, if any sample fails it,
+ * the FP32 product-form kernel recomputes the call in the same stream (no host synchronisation either way). */
 int nqs_local_energy_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t B, int32_t M,
                        const nqs_c64 *d_a, const nqs_c64 *d_b, const nqs_c64 *d_W, nqs_c64 *d_eloc,
                        nqs_c64 *d_logpsi, void *stream);
 
 /* ---------------------------------------------------------------------------------------
+ * Options (process-wide, atomic; meant for tests and benchmarks -- the defaults are the product).
+ *   NQS_OPT_A5_PATH     0 = automatic (above)          1 = FP32 product form only
+ *                       2 = series + guard + fallback at ANY size
+ *                       3 = series only: the guard is evaluated and recorded but nothing is recomputed
+ *   NQS_OPT_THETA_PATH  0 = automatic (int8 tcgen05 kernel for N <= 512, else FP32 SIMT)   1 = FP32 SIMT only
+ * nqs_debug_last_a5 (synchronises `stream`; tests only; not meaningful while calls run concurrently on other
+ * streams): out[0] = 1 if the most recent nqs_local_energy* call on this device attempted the series path, 2 if
+ * it used the product form only; out[1] = 1 if the guard failed; out[2] = samples over the guard threshold.
+ * ------------------------------------------------------------------------------------- */
+enum { NQS_OPT_A5_PATH = 0, NQS_OPT_THETA_PATH = 1, NQS_OPT_COUNT = 2 };
+int nqs_set_option(int32_t key, int32_t value);
+int nqs_get_option(int32_t key, int32_t *value);
+int nqs_debug_last_a5(int32_t out[3], void *stream);
+
+/* ---------------------------------------------------------------------------------------
  * Test/debug entry (small inputs): materialise Eq. 39 -- the connected configurations and
  * summed matrix elements per flip group (PAPER.md:456-458 get_s_primes).  Slot 0 is the
- * diagonal (s' = s, element = sum of the diagonal terms), slot 1+g is flip group g:
+ * diagonal (s' = s, element = sum of the diagonal terms), slot 1+g is flip group g (groups in
+ * order of first appearance in the term list):
  *   d_sprime [B,G+1,N] int8, d_mel [B,G+1] complex64.  A zero element means "not connected".
+ * *G_out (may be NULL) receives G.  A call with B = 0 only compiles the term list on the host and
+ * reports G (no device needed), so that the caller can size the outputs.
+ * nqs_enumerate_connected_h is the same with a compiled handle.
  * ------------------------------------------------------------------------------------- */
-int nqs_enumerate_connected(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t B,
-                            int8_t *d_sprime, nqs_c64 *d_mel, void *stream);
+int nqs_enumerate_connected(const int8_t *d_spins, int64_t B, int32_t N, int32_t T, const int32_t *h_sites,
+                            const uint8_t *h_paulis, const nqs_c64 *h_coeffs, int8_t *d_sprime,
+                            nqs_c64 *d_mel, int32_t *G_out, void *stream);
+int nqs_enumerate_connected_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t B,
+                              int8_t *d_sprime, nqs_c64 *d_mel, void *stream);
 
 /* Optional per-kernel timing for benchmarks.  nqs_profile_enable(1) makes every following
- * nqs_local_energy* call record CUDA events on its stream around its four kernels;
+ * nqs_local_energy* call record CUDA events on its stream around its kernels;
  * nqs_profile_last() waits for the most recent such call and returns the elapsed milliseconds of
- * ms[0] parameter tables (a1), ms[1] theta / log psi / tanh (a2, a3), ms[2] connected amplitudes
- * (a4, a5), ms[3] final reduction (a6).  Not thread-safe; off by default. */
+ *   ms[0] parameter tables (a1; product-form tables and the series' T^k planes)
+ *   ms[1] theta / log psi / tanh (a2, a3)             ms[2] series operand packing (t^k planes)
+ *   ms[3] series GEMM + fused epilogue (a4, a5, a6)   ms[4] series guard / E_loc
+ *   ms[5] product-form kernel (a4, a5; exits at once when the series passed its guard)
+ *   ms[6] final reduction of the product form (a6) and bookkeeping
+ * Segments of kernels that were not launched read ~0.  Not thread-safe; off by default. */
+enum { NQS_PROFILE_SEGMENTS = 7 };
 int nqs_profile_enable(int on);
-int nqs_profile_last(float ms[4]);
+int nqs_profile_last(float ms[NQS_PROFILE_SEGMENTS]);
 
 /* ---------------------------------------------------------------------------------------
  * Batch statistics (Eq. 5; get_global_mean / get_global_variance, :511-515).
@@ -147,7 +189,8 @@ int nqs_profile_last(float ms[4]);
  *   with w_b = p(s_b) over a full basis the mean is the exact expectation of Eq. 3).  Weights must be
  *   non-negative with a positive sum (otherwise the outputs are NaN, no error is raised).
  *   d_stats [4] float64 DEVICE out: Re mean, Im mean, variance <<|x - mean|^2>>, sum of weights.
- * Sums are accumulated in float64 in a fixed order (deterministic).  Asynchronous on `stream`.
+ * Sums are accumulated in float64 in a fixed order (deterministic).  Asynchronous on `stream`.  B == 0 is a
+ * no-op (d_stats is left untouched).
  * ------------------------------------------------------------------------------------- */
 int nqs_energy_stats(const nqs_c64 *d_x, const float *d_weights, int64_t B, double *d_stats, void *stream);
 
@@ -194,6 +237,12 @@ int nqs_metropolis(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const nqs_c
                    const nqs_c64 *d_b, const nqs_c64 *d_W, int32_t S, const int32_t *d_sites,
                    const float *d_u, int32_t *d_accepted, void *stream);
 
+/* Test/debug variant: additionally writes d_decisions [S,C] uint8 DEVICE (may be NULL), 1 = the proposal of
+ * step t to chain c was accepted -- the trace a test compares with the oracle's, decision by decision. */
+int nqs_metropolis_trace(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64 *d_a,
+                         const nqs_c64 *d_b, const nqs_c64 *d_W, int32_t S, const int32_t *d_sites,
+                         const float *d_u, int32_t *d_accepted, uint8_t *d_decisions, void *stream);
+
 /* Pipe-rate micro-benchmark (the roofline is quoted against the nominal peak
  * AND a peak measured on the box).  Runs a register-only kernel (2 blocks of 320 threads per SM,
  * no memory traffic in the loop) `iters` iterations, best of 3 after one warm-up, on a private
@@ -210,7 +259,8 @@ int nqs_microbench(int32_t kind, int32_t iters, double *lane_ops_per_s, float *m
 /* Thread-local message of the last error on this thread ("" if none). */
 const char *nqs_last_error(void);
 
-/* Drops the internal cache of compiled Hamiltonians (device memory freed). */
+/* Drops the internal cache of compiled Hamiltonians and trims the library's scratch pools (device memory
+ * returned to the driver once the work that used it has finished). */
 int nqs_release(void);
 
 /* "major.minor.patch sm_100a" */

@@ -10,7 +10,14 @@ from .binding import (  # noqa: F401
     MICROBENCH_KINDS,
     NqsError,
     energy_stats,
+    A5_PATHS,
+    PROFILE_SEGMENTS,
+    connected_groups,
+    debug_last_a5,
     enumerate_connected,
+    enumerate_connected_h,
+    get_option,
+    set_option,
     forces,
     hamiltonian_info_host,
     last_error,

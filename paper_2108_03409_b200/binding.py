@@ -46,7 +46,12 @@ def load_library() -> ctypes.CDLL:
             lib.nqs_hamiltonian_destroy.argtypes = [vp]
             lib.nqs_hamiltonian_info.argtypes = [vp, vp, vp]
             lib.nqs_local_energy_h.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, vp]
-            lib.nqs_enumerate_connected.argtypes = [vp, vp, i64, vp, vp, vp]
+            lib.nqs_enumerate_connected_h.argtypes = [vp, vp, i64, vp, vp, vp]
+            lib.nqs_enumerate_connected.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+            lib.nqs_metropolis_trace.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp]
+            lib.nqs_set_option.argtypes = [i32, i32]
+            lib.nqs_get_option.argtypes = [i32, vp]
+            lib.nqs_debug_last_a5.argtypes = [vp, vp]
             lib.nqs_energy_stats.argtypes = [vp, vp, i64, vp, vp]
             lib.nqs_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_microbench.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float)]
@@ -60,7 +65,8 @@ def load_library() -> ctypes.CDLL:
                          "nqs_hamiltonian_create", "nqs_hamiltonian_compile_host", "nqs_hamiltonian_destroy",
                          "nqs_hamiltonian_info", "nqs_local_energy_h", "nqs_enumerate_connected", "nqs_release",
                          "nqs_profile_enable", "nqs_profile_last", "nqs_microbench", "nqs_energy_stats",
-                         "nqs_forces", "nqs_metropolis", "nqs_local_energy_forces_h"):
+                         "nqs_forces", "nqs_metropolis", "nqs_local_energy_forces_h", "nqs_enumerate_connected_h",
+                         "nqs_metropolis_trace", "nqs_set_option", "nqs_get_option", "nqs_debug_last_a5"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -82,11 +88,36 @@ def profile_enable(on: bool) -> None:
     _check(load_library().nqs_profile_enable(int(on)))
 
 
+PROFILE_SEGMENTS = ("table", "theta", "series_pack", "series_gemm", "series_guard", "eloc", "finalize")
+
+
 def profile_last() -> dict:
-    """Milliseconds of the four kernels of the most recent profiled nqs_local_energy* call."""
-    ms = (ctypes.c_float * 4)()
+    """Milliseconds of the kernels of the most recent profiled nqs_local_energy* call (include/nqs.h)."""
+    ms = (ctypes.c_float * len(PROFILE_SEGMENTS))()
     _check(load_library().nqs_profile_last(ms))
-    return dict(table=ms[0], theta=ms[1], eloc=ms[2], finalize=ms[3])
+    return {k: ms[i] for i, k in enumerate(PROFILE_SEGMENTS)}
+
+
+OPTIONS = {"a5_path": 0, "theta_path": 1}
+A5_PATHS = {"auto": 0, "product": 1, "series_guarded": 2, "series_only": 3}
+
+
+def set_option(key: str, value: int) -> None:
+    """nqs_set_option: process-wide test / benchmark switches (include/nqs.h)."""
+    _check(load_library().nqs_set_option(OPTIONS[key], int(value)))
+
+
+def get_option(key: str) -> int:
+    v = ctypes.c_int32()
+    _check(load_library().nqs_get_option(OPTIONS[key], ctypes.byref(v)))
+    return int(v.value)
+
+
+def debug_last_a5() -> dict:
+    """nqs_debug_last_a5 (synchronises): which a5 path the last nqs_local_energy* call took."""
+    out = (ctypes.c_int32 * 3)()
+    _check(load_library().nqs_debug_last_a5(out, _stream()))
+    return dict(path={1: "series", 2: "product"}.get(out[0], "none"), guard_failed=bool(out[1]), samples_over=int(out[2]))
 
 
 MICROBENCH_KINDS = {"ffma": 0, "ffma2": 1, "a5_body_packed": 2, "a5_body_scalar": 3, "mufu_ex2": 4}
@@ -246,8 +277,9 @@ def forces(spins, a, b, W, eloc, weights=None, want_stats: bool = False):
     return (F, stats) if want_stats else F
 
 
-def metropolis(spins, a, b, W, sites, u, want_accepted: bool = True):
-    """nqs_metropolis: advances the chains `spins` [C,N] IN PLACE by S = sites.shape[0] steps."""
+def metropolis(spins, a, b, W, sites, u, want_accepted: bool = True, trace: bool = False):
+    """nqs_metropolis: advances the chains `spins` [C,N] IN PLACE by S = sites.shape[0] steps.
+    trace=True (nqs_metropolis_trace) also returns the accept bits uint8 [S,C]."""
     import torch
 
     C, N, M = _shapes(spins, a, b, W)
@@ -255,11 +287,15 @@ def metropolis(spins, a, b, W, sites, u, want_accepted: bool = True):
     if tuple(sites.shape) != (S, C) or tuple(u.shape) != (S, C):
         raise ValueError("sites and u must have shape [S, C]")
     accepted = torch.empty(C, dtype=torch.int32, device=spins.device) if want_accepted else None
-    with torch.cuda.device(spins.device):
-        _check(load_library().nqs_metropolis(
-            _dev(spins, torch.int8, "spins"), C, N, M, _dev(a, torch.complex64, "a"), _dev(b, torch.complex64, "b"),
+    args = (_dev(spins, torch.int8, "spins"), C, N, M, _dev(a, torch.complex64, "a"), _dev(b, torch.complex64, "b"),
             _dev(W, torch.complex64, "W"), S, _dev(sites, torch.int32, "sites"), _dev(u, torch.float32, "u"),
-            ctypes.c_void_p(accepted.data_ptr()) if want_accepted else None, _stream()))
+            ctypes.c_void_p(accepted.data_ptr()) if want_accepted else None)
+    with torch.cuda.device(spins.device):
+        if trace:
+            decisions = torch.empty((S, C), dtype=torch.uint8, device=spins.device)
+            _check(load_library().nqs_metropolis_trace(*args, ctypes.c_void_p(decisions.data_ptr()), _stream()))
+            return accepted, decisions
+        _check(load_library().nqs_metropolis(*args, _stream()))
     return accepted
 
 
@@ -324,15 +360,42 @@ def log_psi_host(spins, a, b, W):
     return out
 
 
-def enumerate_connected(ham: Hamiltonian, spins):
-    """nqs_enumerate_connected: s' int8 [B,G+1,N], elements complex64 [B,G+1] (slot 0 = diagonal)."""
+def enumerate_connected_h(ham: Hamiltonian, spins):
+    """nqs_enumerate_connected_h: s' int8 [B,G+1,N], elements complex64 [B,G+1] (slot 0 = diagonal)."""
     import torch
 
     B, N = spins.shape
     sp = torch.empty((B, ham.G + 1, N), dtype=torch.int8, device=spins.device)
     mel = torch.empty((B, ham.G + 1), dtype=torch.complex64, device=spins.device)
     with torch.cuda.device(spins.device):
-        _check(load_library().nqs_enumerate_connected(ham._h, _dev(spins, torch.int8, "spins"), B,
-                                                      ctypes.c_void_p(sp.data_ptr()),
-                                                      ctypes.c_void_p(mel.data_ptr()), _stream()))
+        _check(load_library().nqs_enumerate_connected_h(ham._h, _dev(spins, torch.int8, "spins"), B,
+                                                        ctypes.c_void_p(sp.data_ptr()),
+                                                        ctypes.c_void_p(mel.data_ptr()), _stream()))
     return sp, mel
+
+
+def connected_groups(N: int, sites, paulis, coeffs) -> int:
+    """nqs_enumerate_connected with B = 0: the number G of flip groups of a term list (host only)."""
+    sites, paulis, coeffs = _terms(sites, paulis, coeffs)
+    G = ctypes.c_int32(-1)
+    _check(load_library().nqs_enumerate_connected(None, 0, int(N), int(coeffs.shape[0]), _hp(sites), _hp(paulis),
+                                                  _hp(coeffs), None, None, ctypes.byref(G), None))
+    return int(G.value)
+
+
+def enumerate_connected(spins, sites, paulis, coeffs):
+    """nqs_enumerate_connected (term-list form): (s' int8 [B,G+1,N], elements complex64 [B,G+1], G)."""
+    import torch
+
+    B, N = spins.shape
+    sites, paulis, coeffs = _terms(sites, paulis, coeffs)
+    G = connected_groups(N, sites, paulis, coeffs)
+    sp = torch.empty((B, G + 1, N), dtype=torch.int8, device=spins.device)
+    mel = torch.empty((B, G + 1), dtype=torch.complex64, device=spins.device)
+    G2 = ctypes.c_int32(-1)
+    with torch.cuda.device(spins.device):
+        _check(load_library().nqs_enumerate_connected(
+            _dev(spins, torch.int8, "spins"), B, N, int(coeffs.shape[0]), _hp(sites), _hp(paulis), _hp(coeffs),
+            ctypes.c_void_p(sp.data_ptr()), ctypes.c_void_p(mel.data_ptr()), ctypes.byref(G2), _stream()))
+    assert G2.value == G
+    return sp, mel, G

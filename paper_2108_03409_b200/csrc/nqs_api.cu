@@ -1,13 +1,18 @@
 // C ABI of libnqs_b200.so (declared in include/nqs.h): argument checks, workspace, launches.
-// Every step of the path runs in the kernels of nqs_kernels.cuh; there is no CPU fallback.
+// Every step of the path runs in the kernels of nqs_kernels.cuh / nqs_series.cuh / nqs_theta_mma.cuh /
+// nqs_forces.cuh / nqs_sampler.cuh; there is no CPU fallback.
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <list>
+#include <map>
+#include <memory>
 #include <mutex>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/nqs.h"
@@ -16,6 +21,7 @@
 #include "nqs_forces.cuh"
 #include "nqs_microbench.cuh"
 #include "nqs_sampler.cuh"
+#include "nqs_series.cuh"
 #include "nqs_theta_mma.cuh"
 
 using namespace nqs;
@@ -35,9 +41,120 @@ static int fail(int code, const std::string& msg) {
         if (e__ != cudaSuccess)                                                                    \
             return fail(NQS_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__));        \
     } while (0)
+#define NQS_TRY(expr)              \
+    do {                           \
+        int rc__ = (expr);         \
+        if (rc__) return rc__;     \
+    } while (0)
 
 extern "C" const char* nqs_last_error(void) { return g_err.c_str(); }
-extern "C" const char* nqs_version(void) { return "0.1.0 sm_100a"; }
+extern "C" const char* nqs_version(void) { return "0.2.0 sm_100a"; }
+
+// ----------------------------------------------------------------------------------------
+// options (include/nqs.h: nqs_set_option)
+// ----------------------------------------------------------------------------------------
+static std::atomic<int> g_opt[NQS_OPT_COUNT] = {};
+
+extern "C" int nqs_set_option(int32_t key, int32_t value) {
+    if (key < 0 || key >= NQS_OPT_COUNT) return fail(NQS_ERR_INVALID_ARG, "nqs_set_option: unknown key");
+    const int hi = key == NQS_OPT_A5_PATH ? 3 : 1;
+    if (value < 0 || value > hi) return fail(NQS_ERR_INVALID_ARG, "nqs_set_option: value out of range");
+    g_opt[key].store(value);
+    return NQS_OK;
+}
+extern "C" int nqs_get_option(int32_t key, int32_t* value) {
+    if (key < 0 || key >= NQS_OPT_COUNT || !value) return fail(NQS_ERR_INVALID_ARG, "nqs_get_option: bad key / NULL");
+    *value = g_opt[key].load();
+    return NQS_OK;
+}
+
+// ----------------------------------------------------------------------------------------
+// per-device state: a private stream-ordered memory pool for scratch (trimmed by nqs_release),
+// a small status block, and the dynamic-shared-memory opt-in of every kernel
+// ----------------------------------------------------------------------------------------
+constexpr int MAX_DEVICES = 64;
+struct DeviceState {
+    bool ready = false;
+    cudaMemPool_t pool = nullptr;
+    int* status = nullptr;  // [4]: guard flag, failed samples, path tag of the last call (1 series, 2 product), -
+    int* tags = nullptr;    // [4] constant {0, 1, 2, 3}: device-side source of the path tag
+    std::map<const void*, size_t> smem_optin;
+};
+static DeviceState g_dev[MAX_DEVICES];
+static std::mutex g_dev_mu;
+
+static int device_state(DeviceState** out) {
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n == 0) {
+        cudaGetLastError();
+        return fail(NQS_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
+    }
+    int dev = 0;
+    NQS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) return fail(NQS_ERR_UNSUPPORTED, "device ordinal >= 64");
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    DeviceState& D = g_dev[dev];
+    if (!D.ready) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        NQS_CUDA(cudaMemPoolCreate(&D.pool, &props));
+        unsigned long long thr = ~0ull;  // freed scratch stays in THIS pool until nqs_release() trims it
+        NQS_CUDA(cudaMemPoolSetAttribute(D.pool, cudaMemPoolAttrReleaseThreshold, &thr));
+        NQS_CUDA(cudaMalloc(&D.status, 8 * sizeof(int)));
+        const int init[8] = {0, 0, 0, 0, 0, 1, 2, 3};
+        NQS_CUDA(cudaMemcpy(D.status, init, sizeof(init), cudaMemcpyHostToDevice));
+        D.tags = D.status + 4;
+        D.ready = true;
+    }
+    *out = &D;
+    return NQS_OK;
+}
+
+// cudaFuncSetAttribute is per device: remember the largest opt-in per (kernel, device)
+template <class K>
+static int ensure_smem(DeviceState* D, K kernel, size_t bytes) {
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    size_t& cur = D->smem_optin[(const void*)kernel];
+    if (bytes > cur) {
+        NQS_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+        cur = bytes;
+    }
+    return NQS_OK;
+}
+
+// stream-ordered scratch, returned to the pool on every exit path
+struct Scratch {
+    cudaStream_t st;
+    cudaMemPool_t pool;
+    std::vector<void*> ptrs;
+    Scratch(DeviceState* D, cudaStream_t s) : st(s), pool(D->pool) {}
+    Scratch(const Scratch&) = delete;
+    Scratch& operator=(const Scratch&) = delete;
+    ~Scratch() {
+        for (void* q : ptrs) cudaFreeAsync(q, st);
+    }
+    template <class T>
+    int get(T** out, size_t count) {
+        void* q = nullptr;
+        const size_t bytes = count * sizeof(T);
+        NQS_CUDA(cudaMallocFromPoolAsync(&q, bytes ? bytes : 16, pool, st));
+        ptrs.push_back(q);
+        *out = static_cast<T*>(q);
+        return NQS_OK;
+    }
+    void adopt(void* q) { ptrs.push_back(q); }
+    void disown(void* q) {
+        for (auto it = ptrs.begin(); it != ptrs.end(); ++it)
+            if (*it == q) {
+                ptrs.erase(it);
+                return;
+            }
+    }
+};
 
 // ----------------------------------------------------------------------------------------
 // handle
@@ -46,10 +163,14 @@ struct nqs_hamiltonian {
     HostCompiled hc;
     int device = -1;       // -1: host-only compile
     void* d_blob = nullptr;
+    bool pooled = false;   // blob came from the device pool (cache entries): freed in stream order
+    cudaEvent_t last_use = nullptr;
     DevHam dev{};
     int C = 0;
-    // launch plan (static for the handle): column tiling of the a5 kernel
+    // launch plan (static for the handle): column tiling of the product-form a5 kernel ...
     int WC = 1, WS = 2, TC = 16, nTiles = 1, C_pad = 16;
+    // ... and of the tensor-core series kernel
+    int NB = 16, nNT = 1;
 };
 
 static constexpr int KJ = 16;
@@ -59,8 +180,9 @@ static void plan_tiles(nqs_hamiltonian* h) {
     const int C = (int)h->hc.col_i.size();
     h->C = C;
     const int slices = C > 0 ? (C + 15) / 16 : 1;
-    // least padded work divided by the measured efficiency of the block shape: a CTA has 2 WC warps, and
-    // narrow CTAs leave the SM short of warps (measured per 16-column slice on configs 3 and 4, B200)
+    // least padded work divided by the efficiency of the block shape: a CTA has 2 WC warps, and narrow CTAs
+    // leave the SM short of warps (per 16-column slice, measured on B200 at config-3 / config-4 shapes;
+    // only the ORDER of these numbers matters to the choice)
     static const double eff[MAX_WC + 1] = {0.0, 0.36, 0.54, 0.55, 0.68, 0.64};
     int best = 1;
     double best_cost = 1e30;
@@ -72,18 +194,18 @@ static void plan_tiles(nqs_hamiltonian* h) {
             best = wc;
         }
     }
-    if (const char* e = getenv("NQS_WC")) {  // A/B experiments
-        const int v = atoi(e);
-        if (v >= 1 && v <= MAX_WC) best = v;
-    }
     h->WC = best;
     h->WS = 2;
     h->TC = 16 * best;
     h->nTiles = (slices + best - 1) / best;
     h->C_pad = h->nTiles * h->TC;
+    // series kernel: column tiles of NB <= 128 (4 NB TMEM columns), NB a multiple of 16
+    h->nNT = C > 0 ? (C + 127) / 128 : 1;
+    const int per = C > 0 ? (C + h->nNT - 1) / h->nNT : 16;
+    h->NB = (per + 15) / 16 * 16;
 }
 
-static int upload(nqs_hamiltonian* h) {
+static int upload(nqs_hamiltonian* h, DeviceState* D, bool pooled, cudaStream_t st) {
     const HostCompiled& hc = h->hc;
     const int G = (int)hc.groups.size(), Td = (int)hc.diag_c.size(), Tg = (int)hc.gt_c.size();
     const int C_pad = h->C_pad;
@@ -121,35 +243,59 @@ static int upload(nqs_hamiltonian* h) {
     if (!ints.empty()) memcpy(blob.data(), ints.data(), ints.size() * sizeof(int));
     if (!cs.empty()) memcpy(blob.data() + int_bytes, cs.data(), cs.size() * sizeof(nqs_c64));
     NQS_CUDA(cudaGetDevice(&h->device));
-    NQS_CUDA(cudaMalloc(&h->d_blob, total));
-    NQS_CUDA(cudaMemcpy(h->d_blob, blob.data(), total, cudaMemcpyHostToDevice));
+    if (pooled) {
+        // pageable source: the runtime stages the bytes before cudaMemcpyAsync returns, so `blob` may die
+        NQS_CUDA(cudaMallocFromPoolAsync(&h->d_blob, total, D->pool, st));
+        h->pooled = true;
+        NQS_CUDA(cudaMemcpyAsync(h->d_blob, blob.data(), total, cudaMemcpyHostToDevice, st));
+    } else {
+        NQS_CUDA(cudaMalloc(&h->d_blob, total));
+        NQS_CUDA(cudaMemcpy(h->d_blob, blob.data(), total, cudaMemcpyHostToDevice));
+    }
+    NQS_CUDA(cudaEventCreateWithFlags(&h->last_use, cudaEventDisableTiming));
     const int* di = reinterpret_cast<const int*>(h->d_blob);
     const float2* dc = reinterpret_cast<const float2*>(reinterpret_cast<const unsigned char*>(h->d_blob) + int_bytes);
-    DevHam& D = h->dev;
-    D.N = hc.N;
-    D.G = G;
-    D.C = h->C;
-    D.Td = Td;
-    D.Tg = Tg;
-    D.diag_z0 = di + o_dz0;
-    D.diag_z1 = di + o_dz1;
-    D.diag_c = dc;
-    D.grp_f0 = di + o_f0;
-    D.grp_f1 = di + o_f1;
-    D.grp_first = di + o_first;
-    D.grp_count = di + o_count;
-    D.gt_z0 = di + o_gz0;
-    D.gt_z1 = di + o_gz1;
-    D.gt_c = dc + Td;
-    D.col_i = di + o_ci;
-    D.col_k = di + o_ck;
-    D.col_p = di + o_cp;
-    D.col_group = di + o_cg;
+    DevHam& Dv = h->dev;
+    Dv.N = hc.N;
+    Dv.G = G;
+    Dv.C = h->C;
+    Dv.Td = Td;
+    Dv.Tg = Tg;
+    Dv.diag_z0 = di + o_dz0;
+    Dv.diag_z1 = di + o_dz1;
+    Dv.diag_c = dc;
+    Dv.grp_f0 = di + o_f0;
+    Dv.grp_f1 = di + o_f1;
+    Dv.grp_first = di + o_first;
+    Dv.grp_count = di + o_count;
+    Dv.gt_z0 = di + o_gz0;
+    Dv.gt_z1 = di + o_gz1;
+    Dv.gt_c = dc + Td;
+    Dv.col_i = di + o_ci;
+    Dv.col_k = di + o_ck;
+    Dv.col_p = di + o_cp;
+    Dv.col_group = di + o_cg;
     return NQS_OK;
 }
 
-static int create_impl(int32_t N, int32_t T, const int32_t* s, const uint8_t* p, const nqs_c64* c, bool device,
-                       nqs_hamiltonian** out) {
+// frees a handle; pooled blobs are freed in stream order after the handle's most recent use
+static void destroy_handle(nqs_hamiltonian* h) {
+    if (!h) return;
+    if (h->d_blob) {
+        if (h->pooled) {
+            if (h->last_use) cudaStreamWaitEvent(nullptr, h->last_use, 0);
+            cudaFreeAsync(h->d_blob, nullptr);
+        } else {
+            cudaFree(h->d_blob);  // waits for the device: kernels still reading the blob finish first
+        }
+    }
+    if (h->last_use) cudaEventDestroy(h->last_use);
+    delete h;
+}
+
+// mode 0 host only, 1 blocking upload (user handle), 2 pooled, stream-ordered upload (cache entry)
+static int create_impl(int32_t N, int32_t T, const int32_t* s, const uint8_t* p, const nqs_c64* c, int mode,
+                       cudaStream_t st, nqs_hamiltonian** out) {
     if (!out) return fail(NQS_ERR_INVALID_ARG, "nqs_hamiltonian_create: out is NULL");
     *out = nullptr;
     auto* h = new nqs_hamiltonian();
@@ -160,11 +306,12 @@ static int create_impl(int32_t N, int32_t T, const int32_t* s, const uint8_t* p,
         return fail(rc, err);
     }
     plan_tiles(h);
-    if (device) {
-        rc = upload(h);
+    if (mode != 0) {
+        DeviceState* D = nullptr;
+        rc = device_state(&D);
+        if (rc == NQS_OK) rc = upload(h, D, mode == 2, st);
         if (rc != NQS_OK) {
-            if (h->d_blob) cudaFree(h->d_blob);
-            delete h;
+            destroy_handle(h);
             return rc;
         }
     }
@@ -174,16 +321,14 @@ static int create_impl(int32_t N, int32_t T, const int32_t* s, const uint8_t* p,
 
 extern "C" int nqs_hamiltonian_create(int32_t N, int32_t T, const int32_t* h_sites, const uint8_t* h_paulis,
                                       const nqs_c64* h_coeffs, nqs_hamiltonian** out) {
-    return create_impl(N, T, h_sites, h_paulis, h_coeffs, true, out);
+    return create_impl(N, T, h_sites, h_paulis, h_coeffs, 1, nullptr, out);
 }
 extern "C" int nqs_hamiltonian_compile_host(int32_t N, int32_t T, const int32_t* h_sites, const uint8_t* h_paulis,
                                             const nqs_c64* h_coeffs, nqs_hamiltonian** out) {
-    return create_impl(N, T, h_sites, h_paulis, h_coeffs, false, out);
+    return create_impl(N, T, h_sites, h_paulis, h_coeffs, 0, nullptr, out);
 }
 extern "C" int nqs_hamiltonian_destroy(nqs_hamiltonian* h) {
-    if (!h) return NQS_OK;
-    if (h->d_blob) cudaFree(h->d_blob);
-    delete h;
+    destroy_handle(h);
     return NQS_OK;
 }
 extern "C" int nqs_hamiltonian_info(const nqs_hamiltonian* h, int32_t info[5], int32_t* flip_sites) {
@@ -202,18 +347,21 @@ extern "C" int nqs_hamiltonian_info(const nqs_hamiltonian* h, int32_t info[5], i
 }
 
 // ----------------------------------------------------------------------------------------
-// cache of compiled Hamiltonians for the term-list entry points
+// cache of compiled Hamiltonians for the term-list entry points.  Entries are reference counted: a
+// call holds its entry for as long as it enqueues work, eviction and nqs_release() only drop the
+// cache's own reference, and the device blob is freed in stream order (never a device synchronise).
 // ----------------------------------------------------------------------------------------
+using HamRef = std::shared_ptr<nqs_hamiltonian>;
 struct CacheEntry {
     int device, N, T;
     std::vector<unsigned char> key;
-    nqs_hamiltonian* h;
+    HamRef h;
 };
 static std::mutex g_cache_mu;
 static std::list<CacheEntry> g_cache;
 
 static int cached_hamiltonian(int32_t N, int32_t T, const int32_t* s, const uint8_t* p, const nqs_c64* c,
-                              nqs_hamiltonian** out) {
+                              cudaStream_t st, HamRef* out) {
     if (T < 0 || (T > 0 && (!s || !p || !c))) return fail(NQS_ERR_INVALID_ARG, "term arrays are NULL or T < 0");
     int dev = 0;
     NQS_CUDA(cudaGetDevice(&dev));
@@ -231,33 +379,35 @@ static int cached_hamiltonian(int32_t N, int32_t T, const int32_t* s, const uint
             return NQS_OK;
         }
     nqs_hamiltonian* h = nullptr;
-    int rc = nqs_hamiltonian_create(N, T, s, p, c, &h);
-    if (rc != NQS_OK) return rc;
-    g_cache.push_front(CacheEntry{dev, N, T, std::move(key), h});
-    if (g_cache.size() > 8) {
-        // an evicted handle may still be in use by kernels in flight on some stream
-        cudaDeviceSynchronize();
-        nqs_hamiltonian_destroy(g_cache.back().h);
-        g_cache.pop_back();
-    }
-    *out = h;
+    NQS_TRY(create_impl(N, T, s, p, c, 2, st, &h));
+    HamRef ref(h, destroy_handle);
+    g_cache.push_front(CacheEntry{dev, N, T, std::move(key), ref});
+    if (g_cache.size() > 8) g_cache.pop_back();  // the blob goes when the last holder lets go
+    *out = ref;
     return NQS_OK;
 }
 
+static void mark_use(const nqs_hamiltonian* h, cudaStream_t st) {
+    if (h->last_use) cudaEventRecord(h->last_use, st);
+}
+
 extern "C" int nqs_release(void) {
-    std::lock_guard<std::mutex> lk(g_cache_mu);
-    if (!g_cache.empty()) cudaDeviceSynchronize();
-    for (auto& e : g_cache) nqs_hamiltonian_destroy(e.h);
-    g_cache.clear();
+    {
+        std::lock_guard<std::mutex> lk(g_cache_mu);
+        g_cache.clear();
+    }
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    for (int d = 0; d < MAX_DEVICES; ++d)
+        if (g_dev[d].ready) cudaMemPoolTrimTo(g_dev[d].pool, 0);
     return NQS_OK;
 }
 
 // ----------------------------------------------------------------------------------------
 // optional per-kernel timing (bench.py's roofline leg): CUDA events recorded on the caller's
-// stream around the four kernels of the most recent nqs_local_energy* call
+// stream around the kernels of the most recent nqs_local_energy* call
 // ----------------------------------------------------------------------------------------
 static bool g_prof_on = false;
-static cudaEvent_t g_prof_ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+static cudaEvent_t g_prof_ev[NQS_PROFILE_SEGMENTS + 1] = {};
 static bool g_prof_valid = false;
 
 extern "C" int nqs_profile_enable(int on) {
@@ -267,11 +417,12 @@ extern "C" int nqs_profile_enable(int on) {
     g_prof_valid = false;
     return NQS_OK;
 }
-extern "C" int nqs_profile_last(float ms[4]) {
+extern "C" int nqs_profile_last(float ms[NQS_PROFILE_SEGMENTS]) {
     if (!ms) return fail(NQS_ERR_INVALID_ARG, "ms is NULL");
     if (!g_prof_valid) return fail(NQS_ERR_INVALID_ARG, "no profiled call recorded");
-    NQS_CUDA(cudaEventSynchronize(g_prof_ev[4]));
-    for (int k = 0; k < 4; ++k) NQS_CUDA(cudaEventElapsedTime(&ms[k], g_prof_ev[k], g_prof_ev[k + 1]));
+    NQS_CUDA(cudaEventSynchronize(g_prof_ev[NQS_PROFILE_SEGMENTS]));
+    for (int k = 0; k < NQS_PROFILE_SEGMENTS; ++k)
+        NQS_CUDA(cudaEventElapsedTime(&ms[k], g_prof_ev[k], g_prof_ev[k + 1]));
     return NQS_OK;
 }
 #define NQS_PROF(k, st)                                            \
@@ -280,59 +431,80 @@ extern "C" int nqs_profile_last(float ms[4]) {
     } while (0)
 
 // ----------------------------------------------------------------------------------------
-// device checks, workspace
+// argument checks, NQS_VALIDATE
 // ----------------------------------------------------------------------------------------
-static int check_device() {
-    int n = 0;
-    cudaError_t e = cudaGetDeviceCount(&n);
-    if (e != cudaSuccess || n == 0) {
-        cudaGetLastError();
-        return fail(NQS_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
-    }
-    static std::once_flag once;
-    std::call_once(once, [&] {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            unsigned long long thr = ~0ull;  // keep freed workspace cached in the pool
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-        }
-    });
+static inline long long round_up(long long x, long long m) { return (x + m - 1) / m * m; }
+
+static int check_common(const void* spins, int64_t B, int32_t N, int32_t M, const void* a, const void* b,
+                        const void* W) {
+    if (B < 0) return fail(NQS_ERR_INVALID_ARG, "B < 0");
+    if (N <= 0 || M <= 0) return fail(NQS_ERR_INVALID_ARG, "N and M must be positive");
+    if (B > 0 && (!spins || !a || !b || !W)) return fail(NQS_ERR_INVALID_ARG, "NULL spins/parameter pointer");
+    if ((long long)B * N > (1ll << 40)) return fail(NQS_ERR_UNSUPPORTED, "B*N too large");
+    if (B > (1ll << 31)) return fail(NQS_ERR_UNSUPPORTED, "B > 2^31");
     return NQS_OK;
 }
 
-static inline long long round_up(long long x, long long m) { return (x + m - 1) / m * m; }
+__global__ void validate_spins_kernel(const int8_t* __restrict__ spins, long long total, int* __restrict__ bad) {
+    int n = 0;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const int v = spins[idx];
+        n += (v != 1 && v != -1);
+    }
+    if (n) atomicAdd(bad, n);
+}
 
-static int launch_theta_simt(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
-                             const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad,
-                             nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta) {
+// NQS_VALIDATE=1 (environment, read at every call): every spin must be +1 or -1.  Debug mode: the check
+// synchronises `stream`.
+static int validate_spins(DeviceState* D, const int8_t* d_spins, int64_t B, int32_t N, cudaStream_t st) {
+    const char* e = getenv("NQS_VALIDATE");
+    if (!e || e[0] != '1' || B == 0) return NQS_OK;
+    Scratch S(D, st);
+    int* bad = nullptr;
+    NQS_TRY(S.get(&bad, 1));
+    NQS_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), st));
+    const long long total = (long long)B * N;
+    const unsigned grid = (unsigned)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
+    validate_spins_kernel<<<grid, 256, 0, st>>>(d_spins, total, bad);
+    NQS_CUDA(cudaGetLastError());
+    int h_bad = 0;
+    NQS_CUDA(cudaMemcpyAsync(&h_bad, bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    NQS_CUDA(cudaStreamSynchronize(st));
+    if (h_bad)
+        return fail(NQS_ERR_INVALID_ARG, "NQS_VALIDATE: " + std::to_string(h_bad) + " spin values other than +1/-1");
+    return NQS_OK;
+}
+
+// ----------------------------------------------------------------------------------------
+// a2 / a3 launches
+// ----------------------------------------------------------------------------------------
+static int launch_theta_simt(DeviceState* D, const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad,
+                             const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, float4* tp,
+                             long long nPairsPad, nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta) {
     const long long rows = tp ? nPairsPad * 2 : B;
     const unsigned grid = (unsigned)((rows + 63) / 64);
-    static bool attr_set = false;
-    if (!attr_set) {
-        NQS_CUDA(cudaFuncSetAttribute(theta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TH_SMEM));
-        attr_set = true;
-    }
+    NQS_TRY(ensure_smem(D, theta_kernel, TH_SMEM));
     theta_kernel<<<grid, 256, TH_SMEM, st>>>(d_spins, (long long)B, N, M, M_pad, (const float2*)d_a, (const float2*)d_b,
-                                       (const float2*)d_W, tp, nPairsPad, (float2*)d_logpsi, raw_theta ? 1 : 0);
+                                             (const float2*)d_W, tp, nPairsPad, (float2*)d_logpsi, raw_theta ? 1 : 0);
     NQS_CUDA(cudaGetLastError());
     return NQS_OK;
 }
 
 // a2 on the tensor cores: pack spins and the int8 digits of W, then theta_mma_kernel (tcgen05).
-static int launch_theta_mma(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
-                            const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad,
-                            nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta) {
+static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad,
+                            const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, float4* tp,
+                            long long nPairsPad, nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta) {
     const long long rows = tp ? nPairsPad * 2 : B;
     const long long nMT = (rows + TM_M - 1) / TM_M;
     const int K_pad = (int)round_up(N, TM_KC), K16 = K_pad / 16;
     const int nNT = (M_pad + TM_JT - 1) / TM_JT;
+    Scratch S(D, st);
     uint4 *A_packed = nullptr, *B_packed = nullptr;
     float* scale = nullptr;
-    NQS_CUDA(cudaMallocAsync(&A_packed, sizeof(uint4) * (size_t)nMT * K16 * TM_M, st));
-    NQS_CUDA(cudaMallocAsync(&B_packed, sizeof(uint4) * (size_t)nNT * K16 * TM_N, st));
-    NQS_CUDA(cudaMallocAsync(&scale, sizeof(float) * (size_t)nNT * TM_JT, st));
+    NQS_TRY(S.get(&A_packed, (size_t)nMT * K16 * TM_M));
+    NQS_TRY(S.get(&B_packed, (size_t)nNT * K16 * TM_N));
+    NQS_TRY(S.get(&scale, (size_t)nNT * TM_JT));
     const long long a_items = nMT * K16 * TM_M;
     const unsigned agrid = (unsigned)((a_items + 255) / 256 < 148 * 16 ? (a_items + 255) / 256 : 148 * 16);
     pack_spins_kernel<<<agrid, 256, 0, st>>>(d_spins, (long long)B, N, K16, nMT, A_packed);
@@ -340,11 +512,7 @@ static int launch_theta_mma(const int8_t* d_spins, int64_t B, int32_t N, int32_t
     pack_w_kernel<<<(unsigned)(nNT * TM_JT), 128, 0, st>>>((const float2*)d_W, N, M, K16, B_packed, scale);
     NQS_CUDA(cudaGetLastError());
     const size_t smem = theta_mma_smem_bytes(K_pad);
-    static size_t attr_smem = 0;
-    if (smem > attr_smem) {
-        NQS_CUDA(cudaFuncSetAttribute(theta_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_smem = smem;
-    }
+    NQS_TRY(ensure_smem(D, theta_mma_kernel, smem));
     ThetaMmaParams p;
     p.A_packed = A_packed;
     p.B_packed = B_packed;
@@ -364,121 +532,170 @@ static int launch_theta_mma(const int8_t* d_spins, int64_t B, int32_t N, int32_t
     p.raw_theta = raw_theta ? 1 : 0;
     theta_mma_kernel<<<(unsigned)nMT, TM_THREADS, smem, st>>>(p);
     NQS_CUDA(cudaGetLastError());
-    NQS_CUDA(cudaFreeAsync(A_packed, st));
-    NQS_CUDA(cudaFreeAsync(B_packed, st));
-    NQS_CUDA(cudaFreeAsync(scale, st));
     return NQS_OK;
 }
 
-// NQS_THETA=simt forces the FP32 SIMT kernel (A/B comparisons); the tensor-core kernel covers N <= 512.
+// the tensor-core kernel covers N <= 512; NQS_OPT_THETA_PATH = 1 forces the FP32 SIMT kernel
 static bool theta_use_mma(int32_t N) {
-    static const bool force_simt = [] {
-        const char* e = getenv("NQS_THETA");
-        return e && strcmp(e, "simt") == 0;
-    }();
-    return !force_simt && round_up(N, TM_KC) <= TM_MAX_KPAD;
+    return g_opt[NQS_OPT_THETA_PATH].load() == 0 && round_up(N, TM_KC) <= TM_MAX_KPAD;
 }
 
-static int launch_theta(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad, const nqs_c64* d_a,
-                        const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad, nqs_c64* d_logpsi,
-                        cudaStream_t st, bool raw_theta = false) {
+static int launch_theta(DeviceState* D, const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad,
+                        const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad,
+                        nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta = false) {
     if (theta_use_mma(N))
-        return launch_theta_mma(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st, raw_theta);
-    return launch_theta_simt(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st, raw_theta);
+        return launch_theta_mma(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st, raw_theta);
+    return launch_theta_simt(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st, raw_theta);
 }
 
 template <int WC, int WS>
-static int launch_eloc_t(const ElocParams& p, long long nBlocksY, cudaStream_t st) {
+static int launch_eloc_t(DeviceState* D, const ElocParams& p, long long nBlocksY, cudaStream_t st) {
     using Cfg = ElocCfg<WC, WS, KJ>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        NQS_CUDA(cudaFuncSetAttribute(eloc_kernel<WC, WS, KJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)Cfg::SMEM));
-        attr_set = true;
-    }
-    dim3 grid((unsigned)p.nTiles, (unsigned)nBlocksY);
-    eloc_kernel<WC, WS, KJ><<<grid, Cfg::NT, Cfg::SMEM, st>>>(p);
+    NQS_TRY(ensure_smem(D, eloc_kernel<WC, WS, KJ>, Cfg::SMEM));
+    const long long blocks = (long long)p.nTiles * nBlocksY;
+    if (blocks > 0x7fffffffll) return fail(NQS_ERR_UNSUPPORTED, "B x column tiles exceeds the grid limit");
+    eloc_kernel<WC, WS, KJ><<<(unsigned)blocks, Cfg::NT, Cfg::SMEM, st>>>(p);
     NQS_CUDA(cudaGetLastError());
     return NQS_OK;
 }
 
-static int launch_eloc(const nqs_hamiltonian* h, const ElocParams& p, long long B_pad, cudaStream_t st) {
+static int launch_eloc(DeviceState* D, const nqs_hamiltonian* h, const ElocParams& p, long long B_pad, cudaStream_t st) {
     const long long nby = B_pad / (32 * h->WS);
     switch (h->WC) {
-        case 1: return launch_eloc_t<1, 2>(p, nby, st);
-        case 2: return launch_eloc_t<2, 2>(p, nby, st);
-        case 3: return launch_eloc_t<3, 2>(p, nby, st);
-        case 4: return launch_eloc_t<4, 2>(p, nby, st);
-        case 5: return launch_eloc_t<5, 2>(p, nby, st);
+        case 1: return launch_eloc_t<1, 2>(D, p, nby, st);
+        case 2: return launch_eloc_t<2, 2>(D, p, nby, st);
+        case 3: return launch_eloc_t<3, 2>(D, p, nby, st);
+        case 4: return launch_eloc_t<4, 2>(D, p, nby, st);
+        case 5: return launch_eloc_t<5, 2>(D, p, nby, st);
     }
     return fail(NQS_ERR_UNSUPPORTED, "unsupported column tiling");
 }
 
-static int check_common(const void* spins, int64_t B, int32_t N, int32_t M, const void* a, const void* b,
-                        const void* W) {
-    if (B < 0) return fail(NQS_ERR_INVALID_ARG, "B < 0");
-    if (N <= 0 || M <= 0) return fail(NQS_ERR_INVALID_ARG, "N and M must be positive");
-    if (B > 0 && (!spins || !a || !b || !W)) return fail(NQS_ERR_INVALID_ARG, "NULL spins/parameter pointer");
-    if ((long long)B * N > (1ll << 40)) return fail(NQS_ERR_UNSUPPORTED, "B*N too large");
-    return NQS_OK;
-}
-
 extern "C" int nqs_log_psi(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
                            const nqs_c64* d_b, const nqs_c64* d_W, nqs_c64* d_logpsi, void* stream) {
-    int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
-    if (rc) return rc;
+    NQS_TRY(check_common(d_spins, B, N, M, d_a, d_b, d_W));
     if (B > 0 && !d_logpsi) return fail(NQS_ERR_INVALID_ARG, "d_logpsi is NULL");
-    if ((rc = check_device())) return rc;
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
     if (B == 0) return NQS_OK;
-    return launch_theta(d_spins, B, N, M, (int)round_up(M, KJ), d_a, d_b, d_W, nullptr, 0, d_logpsi,
+    NQS_TRY(validate_spins(D, d_spins, B, N, (cudaStream_t)stream));
+    return launch_theta(D, d_spins, B, N, M, (int)round_up(M, KJ), d_a, d_b, d_W, nullptr, 0, d_logpsi,
                         (cudaStream_t)stream);
 }
 
-// keep_tp != NULL: tanh(theta) ([M_pad][B_pad/2] float4, stream-ordered allocation) is handed to the
-// caller (who frees it with cudaFreeAsync) instead of being released -- nqs_local_energy_forces_h.
+// ----------------------------------------------------------------------------------------
+// a1 .. a6.  a5 runs on the tensor cores as a guarded series (nqs_series.cuh) when the problem is large
+// enough to pay for its operand packing, with the FP32 product form behind it: eloc_kernel and
+// finalize_kernel are always enqueued and return at once unless the guard raised status[0].
+// keep_tp != NULL: tanh(theta) ([M_pad][B_pad/2] float4) is handed to `keeper` instead of being
+// released when this function returns -- nqs_local_energy_forces_h.
+// ----------------------------------------------------------------------------------------
 static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int32_t M,
                              const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, nqs_c64* d_eloc,
-                             nqs_c64* d_logpsi, void* stream, float4** keep_tp) {
+                             nqs_c64* d_logpsi, void* stream, float4** keep_tp, Scratch* keeper) {
     if (!h) return fail(NQS_ERR_INVALID_ARG, "hamiltonian handle is NULL");
     const int N = h->hc.N;
-    int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
-    if (rc) return rc;
+    NQS_TRY(check_common(d_spins, B, N, M, d_a, d_b, d_W));
     if (B > 0 && !d_eloc) return fail(NQS_ERR_INVALID_ARG, "d_eloc is NULL");
-    if ((rc = check_device())) return rc;
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
     if (h->device < 0) return fail(NQS_ERR_INVALID_ARG, "handle was compiled host-only (nqs_hamiltonian_compile_host)");
     int dev = 0;
     NQS_CUDA(cudaGetDevice(&dev));
     if (dev != h->device) return fail(NQS_ERR_INVALID_ARG, "handle belongs to another device");
     if (B == 0) return NQS_OK;
     cudaStream_t st = (cudaStream_t)stream;
+    NQS_TRY(validate_spins(D, d_spins, B, N, st));
 
     const int M_pad = (int)round_up(M, KJ);
     const long long B_pad = round_up(B, 256);
     const long long nPairsPad = B_pad / 2;
     const int nTiles = h->nTiles, TC = h->TC, C_pad = h->C_pad;
+    const bool have_cols = h->C > 0;
 
+    // which a5 path: 0 auto, 1 product form only, 2 series + guard + fallback at any size, 3 series only
+    const int opt = g_opt[NQS_OPT_A5_PATH].load();
+    const bool series_ok = have_cols && N <= SR_MAX_N && series_gemm_smem_bytes(h->NB, N) <= 227 * 1024;
+    const bool big = (double)B * h->C * M >= 268435456.0;  // 2^28 (sample, column, hidden unit) triples
+    const bool use_series = series_ok && (opt == 2 || opt == 3 || (opt == 0 && big));
+    const bool use_product = have_cols && !(use_series && opt == 3);
+
+    Scratch S(D, st);
     float4 *tp = nullptr, *tab = nullptr, *rho = nullptr;
     float2* partial = nullptr;
-    const bool have_cols = h->C > 0;
-    if (have_cols || keep_tp) NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
-    if (have_cols) {
-        NQS_CUDA(cudaMallocAsync(&tab, sizeof(float4) * (size_t)nTiles * M_pad * TC, st));
-        NQS_CUDA(cudaMallocAsync(&rho, sizeof(float4) * (size_t)C_pad, st));
-        NQS_CUDA(cudaMallocAsync(&partial, sizeof(float2) * (size_t)B * nTiles, st));
-        NQS_PROF(0, st);
+    if (have_cols || keep_tp) NQS_TRY(S.get(&tp, (size_t)M_pad * nPairsPad));
+    NQS_PROF(0, st);
+    if (use_product) {
+        NQS_TRY(S.get(&tab, (size_t)nTiles * M_pad * TC));
+        NQS_TRY(S.get(&rho, (size_t)C_pad));
+        NQS_TRY(S.get(&partial, (size_t)B * nTiles));
         const long long total = (long long)M_pad * C_pad;
         const unsigned tgrid = (unsigned)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
         table_kernel<<<tgrid, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, h->C, TC, nTiles,
                                             h->dev.col_i, h->dev.col_k, h->dev.col_p, tab, rho);
         NQS_CUDA(cudaGetLastError());
     }
-    if (have_cols) NQS_PROF(1, st);
-    if (have_cols || d_logpsi || keep_tp) {
-        rc = launch_theta(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st);
-        if (rc) return rc;
+    // series operands that do not depend on the samples
+    const int NB = h->NB, nNT = h->nNT, nJC = M_pad / 16;
+    uint4 *sA = nullptr, *sB = nullptr;
+    SeriesCol* scols = nullptr;
+    float4 *rown = nullptr, *spartial = nullptr;
+    float* rowmax = nullptr;
+    int* status = nullptr;
+    if (use_series) {
+        NQS_TRY(S.get(&sA, (size_t)(B_pad / SR_M) * nJC * SR_PLANES * SR_A_PLANE_U4));
+        NQS_TRY(S.get(&sB, (size_t)nNT * nJC * SR_PLANES * 2 * NB));
+        NQS_TRY(S.get(&scols, (size_t)nNT * NB));
+        NQS_TRY(S.get(&rown, (size_t)B_pad));
+        NQS_TRY(S.get(&rowmax, (size_t)B_pad));
+        NQS_TRY(S.get(&spartial, (size_t)B * nNT));
+        NQS_TRY(S.get(&status, 4));
+        NQS_CUDA(cudaMemsetAsync(status, 0, 4 * sizeof(int), st));
+        series_table_kernel<<<(unsigned)(nNT * NB), 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad,
+                                                                  h->C, NB, h->dev.col_i, h->dev.col_k, h->dev.col_p,
+                                                                  h->dev.col_group, sB, scols);
+        NQS_CUDA(cudaGetLastError());
     }
-    if (have_cols) {
-        NQS_PROF(2, st);
+    NQS_PROF(1, st);
+    if (have_cols || d_logpsi || keep_tp)
+        NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st));
+    NQS_PROF(2, st);
+    if (use_series) {
+        series_pack_kernel<<<(unsigned)(B_pad / SR_M), 256, 0, st>>>(tp, nPairsPad, M_pad, sA, rown, rowmax);
+        NQS_CUDA(cudaGetLastError());
+    }
+    NQS_PROF(3, st);
+    if (use_series) {
+        const size_t smem = series_gemm_smem_bytes(NB, N);
+        NQS_TRY(ensure_smem(D, series_gemm_kernel, smem));
+        SeriesGemmParams gp;
+        gp.A_packed = sA;
+        gp.B_packed = sB;
+        gp.cols = scols;
+        gp.rown = rown;
+        gp.rowmax = rowmax;
+        gp.spins = d_spins;
+        gp.B = B;
+        gp.N = N;
+        gp.nJC = nJC;
+        gp.NB = NB;
+        gp.nNT = nNT;
+        gp.H = h->dev;
+        gp.partial = spartial;
+        const long long blocks = (B_pad / SR_M) * nNT;
+        if (blocks > 0x7fffffffll) return fail(NQS_ERR_UNSUPPORTED, "B x column tiles exceeds the grid limit");
+        series_gemm_kernel<<<(unsigned)blocks, SR_THREADS, smem, st>>>(gp);
+        NQS_CUDA(cudaGetLastError());
+    }
+    NQS_PROF(4, st);
+    if (use_series) {
+        series_guard_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(spartial, (long long)B, nNT, (float2*)d_eloc,
+                                                                         status);
+        NQS_CUDA(cudaGetLastError());
+    }
+    NQS_PROF(5, st);
+    const int* gate = (use_series && use_product) ? status : nullptr;
+    if (use_product) {
         ElocParams p;
         p.tp = tp;
         p.nPairsPad = nPairsPad;
@@ -491,51 +708,70 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         p.nTiles = nTiles;
         p.H = h->dev;
         p.partial = partial;
-        rc = launch_eloc(h, p, B_pad, st);
-        if (rc) return rc;
-        NQS_PROF(3, st);
+        p.status = gate;
+        NQS_TRY(launch_eloc(D, h, p, B_pad, st));
     }
-    finalize_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(d_spins, (long long)B, N, h->dev, partial,
-                                                                 have_cols ? nTiles : 0, (float2*)d_eloc);
-    NQS_CUDA(cudaGetLastError());
-    if (have_cols) {
-        NQS_PROF(4, st);
-        g_prof_valid = g_prof_on;
-        NQS_CUDA(cudaFreeAsync(tab, st));
-        NQS_CUDA(cudaFreeAsync(rho, st));
-        NQS_CUDA(cudaFreeAsync(partial, st));
+    NQS_PROF(6, st);
+    if (use_product || !use_series) {
+        finalize_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(d_spins, (long long)B, N, h->dev, partial,
+                                                                     have_cols ? nTiles : 0, (float2*)d_eloc, gate);
+        NQS_CUDA(cudaGetLastError());
     }
-    if (keep_tp)
+    // debug record of the decision (nqs_debug_last_a5): {guard flag, failed samples} of this call, path tag
+    if (use_series)
+        NQS_CUDA(cudaMemcpyAsync(D->status, status, 2 * sizeof(int), cudaMemcpyDeviceToDevice, st));
+    else
+        NQS_CUDA(cudaMemsetAsync(D->status, 0, 2 * sizeof(int), st));
+    NQS_CUDA(cudaMemcpyAsync(D->status + 2, D->tags + (use_series ? 1 : 2), sizeof(int), cudaMemcpyDeviceToDevice, st));
+    NQS_PROF(7, st);
+    g_prof_valid = g_prof_on;
+    mark_use(h, st);
+    if (keep_tp) {
         *keep_tp = tp;
-    else if (tp)
-        NQS_CUDA(cudaFreeAsync(tp, st));
+        S.disown(tp);
+        keeper->adopt(tp);
+    }
+    return NQS_OK;
+}
+
+extern "C" int nqs_debug_last_a5(int32_t out[3], void* stream) {
+    if (!out) return fail(NQS_ERR_INVALID_ARG, "out is NULL");
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
+    cudaStream_t st = (cudaStream_t)stream;
+    int v[3] = {0, 0, 0};
+    NQS_CUDA(cudaMemcpyAsync(v, D->status, 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    NQS_CUDA(cudaStreamSynchronize(st));
+    out[0] = v[2];  // 1 = the series path was attempted, 2 = product form only
+    out[1] = v[0];  // 1 = the guard failed (and, unless NQS_OPT_A5_PATH = 3, the product form recomputed the call)
+    out[2] = v[1];  // samples whose error bound exceeded the guard threshold
     return NQS_OK;
 }
 
 extern "C" int nqs_local_energy_h(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int32_t M,
                                   const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, nqs_c64* d_eloc,
                                   nqs_c64* d_logpsi, void* stream) {
-    return local_energy_impl(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream, nullptr);
+    return local_energy_impl(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream, nullptr, nullptr);
 }
 
 extern "C" int nqs_local_energy(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
                                 const nqs_c64* d_b, const nqs_c64* d_W, int32_t T, const int32_t* h_sites,
                                 const uint8_t* h_paulis, const nqs_c64* h_coeffs, nqs_c64* d_eloc,
                                 nqs_c64* d_logpsi, void* stream) {
-    int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
-    if (rc) return rc;
-    if ((rc = check_device())) return rc;
-    nqs_hamiltonian* h = nullptr;
-    if ((rc = cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, &h))) return rc;
-    return nqs_local_energy_h(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream);
+    NQS_TRY(check_common(d_spins, B, N, M, d_a, d_b, d_W));
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
+    HamRef h;
+    NQS_TRY(cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, (cudaStream_t)stream, &h));
+    return nqs_local_energy_h(h.get(), d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream);
 }
 
-extern "C" int nqs_enumerate_connected(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B,
-                                       int8_t* d_sprime, nqs_c64* d_mel, void* stream) {
+static int enumerate_impl(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int8_t* d_sprime,
+                          nqs_c64* d_mel, void* stream) {
     if (!h) return fail(NQS_ERR_INVALID_ARG, "hamiltonian handle is NULL");
     if (B < 0 || (B > 0 && (!d_spins || !d_sprime || !d_mel))) return fail(NQS_ERR_INVALID_ARG, "bad arguments");
-    int rc = check_device();
-    if (rc) return rc;
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
     if (h->device < 0) return fail(NQS_ERR_INVALID_ARG, "handle was compiled host-only");
     if (B == 0) return NQS_OK;
     const long long total = (long long)B * (h->dev.G + 1);
@@ -543,7 +779,32 @@ extern "C" int nqs_enumerate_connected(const nqs_hamiltonian* h, const int8_t* d
     enumerate_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(d_spins, (long long)B, h->hc.N, h->dev, d_sprime,
                                                              (float2*)d_mel);
     NQS_CUDA(cudaGetLastError());
+    mark_use(h, (cudaStream_t)stream);
     return NQS_OK;
+}
+
+extern "C" int nqs_enumerate_connected_h(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B,
+                                         int8_t* d_sprime, nqs_c64* d_mel, void* stream) {
+    return enumerate_impl(h, d_spins, B, d_sprime, d_mel, stream);
+}
+
+extern "C" int nqs_enumerate_connected(const int8_t* d_spins, int64_t B, int32_t N, int32_t T,
+                                       const int32_t* h_sites, const uint8_t* h_paulis, const nqs_c64* h_coeffs,
+                                       int8_t* d_sprime, nqs_c64* d_mel, int32_t* G_out, void* stream) {
+    if (B < 0 || N <= 0) return fail(NQS_ERR_INVALID_ARG, "nqs_enumerate_connected: B < 0 or N <= 0");
+    if (B == 0) {  // sizing call: no device needed
+        nqs_hamiltonian* hh = nullptr;
+        NQS_TRY(create_impl(N, T, h_sites, h_paulis, h_coeffs, 0, nullptr, &hh));
+        if (G_out) *G_out = (int32_t)hh->hc.groups.size();
+        destroy_handle(hh);
+        return NQS_OK;
+    }
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
+    HamRef h;
+    NQS_TRY(cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, (cudaStream_t)stream, &h));
+    if (G_out) *G_out = (int32_t)h->hc.groups.size();
+    return enumerate_impl(h.get(), d_spins, B, d_sprime, d_mel, stream);
 }
 
 // ----------------------------------------------------------------------------------------
@@ -580,25 +841,24 @@ extern "C" int nqs_local_energy_host(const int8_t* h_spins, int64_t B, int32_t N
                                      const nqs_c64* h_b, const nqs_c64* h_W, int32_t T, const int32_t* h_sites,
                                      const uint8_t* h_paulis, const nqs_c64* h_coeffs, nqs_c64* h_eloc,
                                      nqs_c64* h_logpsi) {
-    int rc = check_common(h_spins, B, N, M, h_a, h_b, h_W);
-    if (rc) return rc;
+    NQS_TRY(check_common(h_spins, B, N, M, h_a, h_b, h_W));
     if (B > 0 && !h_eloc) return fail(NQS_ERR_INVALID_ARG, "h_eloc is NULL");
-    if ((rc = check_device())) return rc;
-    nqs_hamiltonian* h = nullptr;
-    if ((rc = cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, &h))) return rc;
-    if (B == 0) return NQS_OK;
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
     HostStage S;
-    if ((rc = S.init())) return rc;
+    NQS_TRY(S.init());
+    HamRef h;
+    NQS_TRY(cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, S.st, &h));
+    if (B == 0) return NQS_OK;
     void *ds, *da, *db, *dW, *de, *dl = nullptr;
-    if ((rc = S.to_device(h_spins, (size_t)B * N, &ds))) return rc;
-    if ((rc = S.to_device(h_a, sizeof(nqs_c64) * N, &da))) return rc;
-    if ((rc = S.to_device(h_b, sizeof(nqs_c64) * M, &db))) return rc;
-    if ((rc = S.to_device(h_W, sizeof(nqs_c64) * (size_t)M * N, &dW))) return rc;
-    if ((rc = S.alloc(sizeof(nqs_c64) * B, &de))) return rc;
-    if (h_logpsi && (rc = S.alloc(sizeof(nqs_c64) * B, &dl))) return rc;
-    rc = nqs_local_energy_h(h, (const int8_t*)ds, B, M, (const nqs_c64*)da, (const nqs_c64*)db, (const nqs_c64*)dW,
-                            (nqs_c64*)de, (nqs_c64*)dl, S.st);
-    if (rc) return rc;
+    NQS_TRY(S.to_device(h_spins, (size_t)B * N, &ds));
+    NQS_TRY(S.to_device(h_a, sizeof(nqs_c64) * N, &da));
+    NQS_TRY(S.to_device(h_b, sizeof(nqs_c64) * M, &db));
+    NQS_TRY(S.to_device(h_W, sizeof(nqs_c64) * (size_t)M * N, &dW));
+    NQS_TRY(S.alloc(sizeof(nqs_c64) * B, &de));
+    if (h_logpsi) NQS_TRY(S.alloc(sizeof(nqs_c64) * B, &dl));
+    NQS_TRY(nqs_local_energy_h(h.get(), (const int8_t*)ds, B, M, (const nqs_c64*)da, (const nqs_c64*)db,
+                               (const nqs_c64*)dW, (nqs_c64*)de, (nqs_c64*)dl, S.st));
     NQS_CUDA(cudaMemcpyAsync(h_eloc, de, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
     if (h_logpsi) NQS_CUDA(cudaMemcpyAsync(h_logpsi, dl, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
     NQS_CUDA(cudaStreamSynchronize(S.st));
@@ -607,22 +867,21 @@ extern "C" int nqs_local_energy_host(const int8_t* h_spins, int64_t B, int32_t N
 
 extern "C" int nqs_log_psi_host(const int8_t* h_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* h_a,
                                 const nqs_c64* h_b, const nqs_c64* h_W, nqs_c64* h_logpsi) {
-    int rc = check_common(h_spins, B, N, M, h_a, h_b, h_W);
-    if (rc) return rc;
+    NQS_TRY(check_common(h_spins, B, N, M, h_a, h_b, h_W));
     if (B > 0 && !h_logpsi) return fail(NQS_ERR_INVALID_ARG, "h_logpsi is NULL");
-    if ((rc = check_device())) return rc;
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
     if (B == 0) return NQS_OK;
     HostStage S;
-    if ((rc = S.init())) return rc;
+    NQS_TRY(S.init());
     void *ds, *da, *db, *dW, *dl;
-    if ((rc = S.to_device(h_spins, (size_t)B * N, &ds))) return rc;
-    if ((rc = S.to_device(h_a, sizeof(nqs_c64) * N, &da))) return rc;
-    if ((rc = S.to_device(h_b, sizeof(nqs_c64) * M, &db))) return rc;
-    if ((rc = S.to_device(h_W, sizeof(nqs_c64) * (size_t)M * N, &dW))) return rc;
-    if ((rc = S.alloc(sizeof(nqs_c64) * B, &dl))) return rc;
-    rc = nqs_log_psi((const int8_t*)ds, B, N, M, (const nqs_c64*)da, (const nqs_c64*)db, (const nqs_c64*)dW,
-                     (nqs_c64*)dl, S.st);
-    if (rc) return rc;
+    NQS_TRY(S.to_device(h_spins, (size_t)B * N, &ds));
+    NQS_TRY(S.to_device(h_a, sizeof(nqs_c64) * N, &da));
+    NQS_TRY(S.to_device(h_b, sizeof(nqs_c64) * M, &db));
+    NQS_TRY(S.to_device(h_W, sizeof(nqs_c64) * (size_t)M * N, &dW));
+    NQS_TRY(S.alloc(sizeof(nqs_c64) * B, &dl));
+    NQS_TRY(nqs_log_psi((const int8_t*)ds, B, N, M, (const nqs_c64*)da, (const nqs_c64*)db, (const nqs_c64*)dW,
+                        (nqs_c64*)dl, S.st));
     NQS_CUDA(cudaMemcpyAsync(h_logpsi, dl, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
     NQS_CUDA(cudaStreamSynchronize(S.st));
     return NQS_OK;
@@ -639,8 +898,8 @@ static void launch_microbench(float* out, unsigned grid, int iters, cudaStream_t
 extern "C" int nqs_microbench(int32_t kind, int32_t iters, double* lane_ops_per_s, float* ms_out) {
     if (kind < 0 || kind >= MB_KINDS || iters <= 0 || !lane_ops_per_s)
         return fail(NQS_ERR_INVALID_ARG, "nqs_microbench: bad kind / iters / NULL output");
-    int rc = check_device();
-    if (rc) return rc;
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
     int dev = 0, sms = 0;
     NQS_CUDA(cudaGetDevice(&dev));
     NQS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -681,35 +940,39 @@ extern "C" int nqs_microbench(int32_t kind, int32_t iters, double* lane_ops_per_
 // ----------------------------------------------------------------------------------------
 // batch statistics and the force vector
 // ----------------------------------------------------------------------------------------
-static int launch_stats(const nqs_c64* d_x, const float* d_w, int64_t B, double* d_stats, cudaStream_t st) {
+static int launch_stats(DeviceState* D, const nqs_c64* d_x, const float* d_w, int64_t B, double* d_stats,
+                        cudaStream_t st) {
+    Scratch S(D, st);
     double* partial = nullptr;
     const int nblk = (int)((B + 255) / 256 < ST_BLOCKS ? (B + 255) / 256 : ST_BLOCKS);
-    NQS_CUDA(cudaMallocAsync(&partial, sizeof(double) * 4 * ST_BLOCKS, st));
+    NQS_TRY(S.get(&partial, (size_t)4 * ST_BLOCKS));
     stats_partial_kernel<<<nblk, 256, 0, st>>>((const float2*)d_x, d_w, (long long)B, partial);
     NQS_CUDA(cudaGetLastError());
     stats_final_kernel<<<1, 32, 0, st>>>(partial, nblk, d_stats);
     NQS_CUDA(cudaGetLastError());
-    NQS_CUDA(cudaFreeAsync(partial, st));
     return NQS_OK;
 }
 
 extern "C" int nqs_energy_stats(const nqs_c64* d_x, const float* d_weights, int64_t B, double* d_stats,
                                 void* stream) {
-    if (B <= 0 || !d_x || !d_stats) return fail(NQS_ERR_INVALID_ARG, "nqs_energy_stats: B <= 0 or NULL pointer");
-    int rc = check_device();
-    if (rc) return rc;
-    return launch_stats(d_x, d_weights, B, d_stats, (cudaStream_t)stream);
+    if (B < 0) return fail(NQS_ERR_INVALID_ARG, "nqs_energy_stats: B < 0");
+    if (B == 0) return NQS_OK;
+    if (!d_x || !d_stats) return fail(NQS_ERR_INVALID_ARG, "nqs_energy_stats: NULL pointer");
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
+    return launch_stats(D, d_x, d_weights, B, d_stats, (cudaStream_t)stream);
 }
 
-// tp_in != NULL: tanh(theta) of this batch from local_energy_impl (ownership passes to this function)
+// tp_in != NULL: tanh(theta) of this batch from local_energy_impl (owned by the caller's Scratch)
 static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
                        const nqs_c64* d_b, const nqs_c64* d_W, const nqs_c64* d_eloc, const float* d_weights,
                        nqs_c64* d_F, double* d_stats, void* stream, float4* tp_in) {
-    int rc = check_common(d_spins, B, N, M, d_a, d_b, d_W);
-    if (rc) return rc;
-    if (B <= 0 || !d_eloc || !d_F) return fail(NQS_ERR_INVALID_ARG, "nqs_forces: B <= 0 or NULL d_eloc / d_F");
+    NQS_TRY(check_common(d_spins, B, N, M, d_a, d_b, d_W));
+    if (B == 0) return NQS_OK;
+    if (!d_eloc || !d_F) return fail(NQS_ERR_INVALID_ARG, "nqs_forces: NULL d_eloc / d_F");
     if (B > (1ll << 25)) return fail(NQS_ERR_UNSUPPORTED, "nqs_forces: B > 2^25 (int32 accumulation range)");
-    if ((rc = check_device())) return rc;
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
     cudaStream_t st = (cudaStream_t)stream;
     const int M_pad = (int)round_up(M, KJ);
     const long long B_pad = round_up(B, 256);
@@ -717,35 +980,32 @@ static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, c
     const int K16 = (int)(B_pad / 16);
     const int nIT = (N + 1 + TM_M - 1) / TM_M, nJT = (M + 1 + TM_JT - 1) / TM_JT;
 
+    Scratch S(D, st);
     float4* tp = tp_in;
     float2* cb = nullptr;
     double* stats = nullptr;
     int* gexp = nullptr;
     uint4 *A_packed = nullptr, *B_packed = nullptr;
-    if (!tp) NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
-    NQS_CUDA(cudaMallocAsync(&cb, sizeof(float2) * (size_t)B_pad, st));
-    NQS_CUDA(cudaMallocAsync(&stats, sizeof(double) * 4, st));
-    NQS_CUDA(cudaMallocAsync(&gexp, sizeof(int) * (size_t)nJT * TM_JT, st));
-    NQS_CUDA(cudaMallocAsync(&A_packed, sizeof(uint4) * (size_t)nIT * K16 * TM_M, st));
-    NQS_CUDA(cudaMallocAsync(&B_packed, sizeof(uint4) * (size_t)nJT * K16 * TM_N, st));
+    if (!tp) NQS_TRY(S.get(&tp, (size_t)M_pad * nPairsPad));
+    NQS_TRY(S.get(&cb, (size_t)B_pad));
+    NQS_TRY(S.get(&stats, 4));
+    NQS_TRY(S.get(&gexp, (size_t)nJT * TM_JT));
+    NQS_TRY(S.get(&A_packed, (size_t)nIT * K16 * TM_M));
+    NQS_TRY(S.get(&B_packed, (size_t)nJT * K16 * TM_N));
 
-    if ((rc = launch_stats(d_eloc, d_weights, B, stats, st))) return rc;
+    NQS_TRY(launch_stats(D, d_eloc, d_weights, B, stats, st));
     if (d_stats) NQS_CUDA(cudaMemcpyAsync(d_stats, stats, sizeof(double) * 4, cudaMemcpyDeviceToDevice, st));
     force_coef_kernel<<<(unsigned)((B_pad + 255) / 256), 256, 0, st>>>((const float2*)d_eloc, d_weights, (long long)B,
                                                                        B_pad, stats, cb);
     NQS_CUDA(cudaGetLastError());
-    if (!tp_in && (rc = launch_theta(d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st))) return rc;
+    if (!tp_in) NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st));
     force_gscale_kernel<<<(unsigned)(nJT * TM_JT), 256, 0, st>>>(tp, nPairsPad, cb, M, gexp);
     NQS_CUDA(cudaGetLastError());
     force_pack_g_kernel<<<148 * 8, 256, 0, st>>>(tp, nPairsPad, cb, M, K16, nJT, gexp, B_packed);
     NQS_CUDA(cudaGetLastError());
     force_pack_spins_kernel<<<148 * 8, 256, 0, st>>>(d_spins, (long long)B, N, K16, nIT, A_packed);
     NQS_CUDA(cudaGetLastError());
-    static bool attr_set = false;
-    if (!attr_set) {
-        NQS_CUDA(cudaFuncSetAttribute(force_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FM_SMEM));
-        attr_set = true;
-    }
+    NQS_TRY(ensure_smem(D, force_mma_kernel, FM_SMEM));
     ForceMmaParams p;
     p.A_packed = A_packed;
     p.B_packed = B_packed;
@@ -756,12 +1016,6 @@ static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, c
     p.F = (float2*)d_F;
     force_mma_kernel<<<dim3((unsigned)nIT, (unsigned)nJT), FM_THREADS, FM_SMEM, st>>>(p);
     NQS_CUDA(cudaGetLastError());
-    NQS_CUDA(cudaFreeAsync(tp, st));
-    NQS_CUDA(cudaFreeAsync(cb, st));
-    NQS_CUDA(cudaFreeAsync(stats, st));
-    NQS_CUDA(cudaFreeAsync(gexp, st));
-    NQS_CUDA(cudaFreeAsync(A_packed, st));
-    NQS_CUDA(cudaFreeAsync(B_packed, st));
     return NQS_OK;
 }
 
@@ -777,10 +1031,14 @@ extern "C" int nqs_local_energy_forces_h(const nqs_hamiltonian* h, const int8_t*
                                          const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W,
                                          const float* d_weights, nqs_c64* d_eloc, nqs_c64* d_logpsi, nqs_c64* d_F,
                                          double* d_stats, void* stream) {
-    if (B <= 0 || !d_F) return fail(NQS_ERR_INVALID_ARG, "nqs_local_energy_forces_h: B <= 0 or NULL d_F");
+    if (B < 0) return fail(NQS_ERR_INVALID_ARG, "nqs_local_energy_forces_h: B < 0");
+    if (B == 0) return NQS_OK;
+    if (!d_F) return fail(NQS_ERR_INVALID_ARG, "nqs_local_energy_forces_h: NULL d_F");
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
+    Scratch keeper(D, (cudaStream_t)stream);
     float4* tp = nullptr;
-    int rc = local_energy_impl(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream, &tp);
-    if (rc) return rc;
+    NQS_TRY(local_energy_impl(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream, &tp, &keeper));
     return forces_impl(d_spins, B, h->hc.N, M, d_a, d_b, d_W, d_eloc, d_weights, d_F, d_stats, stream, tp);
 }
 
@@ -788,40 +1046,40 @@ extern "C" int nqs_local_energy_forces_h(const nqs_hamiltonian* h, const int8_t*
 // Metropolis chains
 // ----------------------------------------------------------------------------------------
 template <int CPB>
-static int launch_metropolis_t(const MetroParams& p, size_t smem, cudaStream_t st) {
-    static size_t attr_smem = 0;
-    if (smem > attr_smem) {
-        NQS_CUDA(cudaFuncSetAttribute(metropolis_kernel<CPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_smem = smem;
-    }
+static int launch_metropolis_t(DeviceState* D, const MetroParams& p, size_t smem, cudaStream_t st) {
+    NQS_TRY(ensure_smem(D, metropolis_kernel<CPB>, smem));
     metropolis_kernel<CPB><<<(unsigned)((p.C + CPB - 1) / CPB), CPB * 32, smem, st>>>(p);
     NQS_CUDA(cudaGetLastError());
     return NQS_OK;
 }
 
-extern "C" int nqs_metropolis(int8_t* d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64* d_a,
-                              const nqs_c64* d_b, const nqs_c64* d_W, int32_t S, const int32_t* d_sites,
-                              const float* d_u, int32_t* d_accepted, void* stream) {
-    int rc = check_common(d_spins, C, N, M, d_a, d_b, d_W);
-    if (rc) return rc;
-    if (S < 0 || (S > 0 && C > 0 && (!d_sites || !d_u))) return fail(NQS_ERR_INVALID_ARG, "nqs_metropolis: S < 0 or NULL sites / u");
-    if ((rc = check_device())) return rc;
+static int metropolis_impl(int8_t* d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64* d_a, const nqs_c64* d_b,
+                           const nqs_c64* d_W, int32_t S, const int32_t* d_sites, const float* d_u,
+                           int32_t* d_accepted, uint8_t* d_decisions, void* stream) {
+    NQS_TRY(check_common(d_spins, C, N, M, d_a, d_b, d_W));
+    if (S < 0 || (S > 0 && C > 0 && (!d_sites || !d_u)))
+        return fail(NQS_ERR_INVALID_ARG, "nqs_metropolis: S < 0 or NULL sites / u");
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
     if (C == 0) return NQS_OK;
     cudaStream_t st = (cudaStream_t)stream;
+    NQS_TRY(validate_spins(D, d_spins, C, N, st));
     const int M_pad = (int)round_up(M, KJ);
     const long long C_pad = round_up(C, 256);
     const long long nPairsPad = C_pad / 2;
     int cpb = 16;
     while (cpb > 2 && metropolis_smem_bytes(cpb, N, M_pad) > 220 * 1024) cpb >>= 1;
     const size_t smem = metropolis_smem_bytes(cpb, N, M_pad);
-    if (smem > 220 * 1024) return fail(NQS_ERR_UNSUPPORTED, "nqs_metropolis: M too large for the shared-memory chain state");
+    if (smem > 220 * 1024)
+        return fail(NQS_ERR_UNSUPPORTED, "nqs_metropolis: M too large for the shared-memory chain state");
 
+    Scratch Sc(D, st);
     float4 *tp = nullptr, *Gp = nullptr, *Gm = nullptr;
     float* lk2 = nullptr;
-    NQS_CUDA(cudaMallocAsync(&tp, sizeof(float4) * (size_t)M_pad * nPairsPad, st));
-    NQS_CUDA(cudaMallocAsync(&Gp, sizeof(float4) * (size_t)N * (M_pad / 2), st));
-    NQS_CUDA(cudaMallocAsync(&Gm, sizeof(float4) * (size_t)N * (M_pad / 2), st));
-    NQS_CUDA(cudaMallocAsync(&lk2, sizeof(float) * (size_t)N, st));
+    NQS_TRY(Sc.get(&tp, (size_t)M_pad * nPairsPad));
+    NQS_TRY(Sc.get(&Gp, (size_t)N * (M_pad / 2)));
+    NQS_TRY(Sc.get(&Gm, (size_t)N * (M_pad / 2)));
+    NQS_TRY(Sc.get(&lk2, (size_t)N));
     site_table_kernel<<<(unsigned)N, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, Gp, Gm, lk2);
     NQS_CUDA(cudaGetLastError());
     MetroParams p;
@@ -836,26 +1094,33 @@ extern "C" int nqs_metropolis(int8_t* d_spins, int64_t C, int32_t N, int32_t M, 
     p.Gm = Gm;
     p.lk2 = lk2;
     p.accepted = d_accepted;
-    // chunks of two sweeps; tanh(theta) is recomputed from the current spins before each chunk
+    // chunks of two sweeps; theta is recomputed from the current spins before each chunk
     const int chunk = 2 * N;
     for (int s0 = 0; s0 == 0 || s0 < S; s0 += chunk) {
-        if ((rc = launch_theta(d_spins, C, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st, true))) return rc;
+        NQS_TRY(launch_theta(D, d_spins, C, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st, true));
         p.S = S - s0 < chunk ? S - s0 : chunk;
         p.sites = d_sites + (long long)s0 * C;
         p.u = d_u + (long long)s0 * C;
+        p.decisions = d_decisions ? d_decisions + (long long)s0 * C : nullptr;
         p.accumulate = s0 > 0;
         switch (cpb) {
-            case 16: rc = launch_metropolis_t<16>(p, smem, st); break;
-            case 8: rc = launch_metropolis_t<8>(p, smem, st); break;
-            case 4: rc = launch_metropolis_t<4>(p, smem, st); break;
-            default: rc = launch_metropolis_t<2>(p, smem, st); break;
+            case 16: NQS_TRY(launch_metropolis_t<16>(D, p, smem, st)); break;
+            case 8: NQS_TRY(launch_metropolis_t<8>(D, p, smem, st)); break;
+            case 4: NQS_TRY(launch_metropolis_t<4>(D, p, smem, st)); break;
+            default: NQS_TRY(launch_metropolis_t<2>(D, p, smem, st)); break;
         }
-        if (rc) return rc;
     }
-    if (rc) return rc;
-    NQS_CUDA(cudaFreeAsync(tp, st));
-    NQS_CUDA(cudaFreeAsync(Gp, st));
-    NQS_CUDA(cudaFreeAsync(Gm, st));
-    NQS_CUDA(cudaFreeAsync(lk2, st));
     return NQS_OK;
+}
+
+extern "C" int nqs_metropolis(int8_t* d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64* d_a,
+                              const nqs_c64* d_b, const nqs_c64* d_W, int32_t S, const int32_t* d_sites,
+                              const float* d_u, int32_t* d_accepted, void* stream) {
+    return metropolis_impl(d_spins, C, N, M, d_a, d_b, d_W, S, d_sites, d_u, d_accepted, nullptr, stream);
+}
+
+extern "C" int nqs_metropolis_trace(int8_t* d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64* d_a,
+                                    const nqs_c64* d_b, const nqs_c64* d_W, int32_t S, const int32_t* d_sites,
+                                    const float* d_u, int32_t* d_accepted, uint8_t* d_decisions, void* stream) {
+    return metropolis_impl(d_spins, C, N, M, d_a, d_b, d_W, S, d_sites, d_u, d_accepted, d_decisions, stream);
 }

@@ -229,6 +229,7 @@ struct ElocParams {
     int N, M_pad, nTiles;
     DevHam H;
     float2* partial;        // [B][nTiles]
+    const int* status;      // nullptr, or the guard word of the series path: run only if (status[0] & 1)
 };
 
 template <int WC, int WS, int KJ>
@@ -254,8 +255,9 @@ __global__ void __launch_bounds__(WC * WS * 32, (WC * WS <= 10) ? 2 : 1) eloc_ke
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int wc = warp % WC, ws = warp / WC;
     const int lc = lane & 15, ls = lane >> 4;
-    const int tile = blockIdx.x;
-    const long long pair0 = (long long)blockIdx.y * TBP;
+    if (p.status && !(p.status[0] & 1)) return;  // the tensor-core series path passed its guard (nqs_series.cuh)
+    const int tile = (int)(blockIdx.x % (unsigned)p.nTiles);  // 1-D grid, column tile fastest
+    const long long pair0 = (long long)(blockIdx.x / (unsigned)p.nTiles) * TBP;
     const int c = tile * TC + wc * 16 + lc;
     const int nChunks = p.M_pad / KJ;
     const float4* const tab_tile = p.tab + (long long)tile * p.M_pad * TC;
@@ -439,9 +441,11 @@ __global__ void __launch_bounds__(WC * WS * 32, (WC * WS <= 10) ? 2 : 1) eloc_ke
 
 // a6: E_loc = diagonal + sum over column tiles of the partial sums (fixed order: deterministic)
 __global__ void finalize_kernel(const int8_t* __restrict__ spins, long long B, int N, DevHam H,
-                                const float2* __restrict__ partial, int nTiles, float2* __restrict__ eloc) {
+                                const float2* __restrict__ partial, int nTiles, float2* __restrict__ eloc,
+                                const int* __restrict__ status) {
     const long long b = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (b >= B) return;
+    if (status && !(status[0] & 1)) return;  // series_guard_kernel already wrote E_loc
     float2 d = diagonal_element(H, spins + b * N);
     for (int t = 0; t < nTiles; ++t) {
         const float2 v = partial[b * nTiles + t];

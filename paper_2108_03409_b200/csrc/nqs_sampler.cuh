@@ -78,6 +78,7 @@ struct MetroParams {
     const float* u;          // [S][C]
     int* accepted;           // [C] or nullptr
     int accumulate;          // add to accepted[] instead of overwriting it
+    uint8_t* decisions;      // [S][C] or nullptr: 1 = the proposal of step t was accepted (nqs_metropolis_trace)
 };
 
 __host__ __device__ inline size_t metropolis_smem_bytes(int cpb, int N, int M_pad) {
@@ -167,6 +168,7 @@ __global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroPara
         for (int o = 16; o > 0; o >>= 1) lg += __shfl_xor_sync(0xffffffffu, lg, o);
         const float lk = p.lk2[site];
         const bool accept = log2f(ul) < (sgi > 0 ? lk : -lk) + lg;  // u == 0: -inf, always accepted
+        if (lane == 0 && p.decisions) p.decisions[(long long)step * p.C + c] = accept ? 1 : 0;
         if (accept) {
             // pass 2: E_j <- E_j G_j(-sigma)
             auto pass2 = [&](int jp0, bool ragged) {

@@ -1,0 +1,490 @@
+// a5 on the 5th-generation tensor cores (Algorithm 1 line 7, PAPER.md:181-183,
+// the call sequence at :464-469): the connected amplitudes as a guarded series of dense contractions.
+//
+// Ratio identity R:  psi(s')/psi(s) = rho_c(sigma) prod_j (C_jc - sigma t_bj S_jc)
+//                                   = rho_c(sigma) kappa_c prod_j (1 - sigma t_bj T_jc),
+// with C = cosh 2V, S = sinh 2V, T = tanh 2V = S/C, kappa_c = prod_j C_jc, t = tanh theta.  Hence
+//   log R_bc = log kappa_c - 2 sigma A_c - sigma ODD_bc - EVEN_bc,
+//   ODD_bc  = sum_{k odd}  (1/k) sum_j t_bj^k T_jc^k,      EVEN_bc = sum_{k even} (1/k) sum_j t_bj^k T_jc^k
+// (log(1 - x) = -sum_k x^k / k, |x| < 1).  Truncated at k = 3, every k is a complex [B, M] x [M, C] GEMM
+// of element-wise powers.  The GEMMs run as FP16 tcgen05.mma (kind::f16) with FP32 accumulators in
+// TMEM; the k = 1 operands are split error-free into two FP16 parts each (hi + lo, three products
+// hi.hi + hi.lo + lo.hi: 22 bits), k = 2 and k = 3 need one FP16 part (they are corrections of relative
+// size |x| and |x|^2).  Complex arithmetic = four real MMAs per product, the minus sign of Re by the
+// negate-A bit of the instruction descriptor.  5 products x 4 = 20 MMAs (M = 128, N = NB, K = 16) per
+// 16 hidden units; all odd-k products accumulate into one pair (re, im) of TMEM column ranges and the
+// even-k product into a second one, so an accumulator tile is 4 NB <= 512 TMEM columns.
+//
+// The series is only valid where |t T| is small.  The kernel evaluates, per sample, a bound on the
+// error it made (truncation + FP16 operand rounding, from row norms of t and column norms of T by
+// Cauchy-Schwarz; DESIGN.md section 12 derives it) weighted with |m_bc R_bc|; series_guard_kernel
+// compares it with 0.5e-4 max(1, |E_loc|) and raises a device flag if ANY sample fails, in which case
+// the FP32 product-form eloc_kernel (which always follows in the stream and exits at once otherwise)
+// recomputes the whole call.  No host synchronisation is involved in the decision.
+//
+// Kernels:  series_table_kernel  T^k planes (FP16, UMMA smem image), log kappa, column norms
+//           series_pack_kernel   t^k planes (FP16, UMMA smem image) from tanh(theta), row norms
+//           series_gemm_kernel   the GEMMs + fused epilogue exp / matrix element / reduction over c
+//           series_guard_kernel  E_loc = diagonal + partial sums, guard decision
+#pragma once
+#include <cuda_fp16.h>
+
+#include "nqs_device.cuh"
+#include "nqs_theta_mma.cuh"
+
+namespace nqs {
+
+constexpr int SR_M = 128;                 // samples per CTA (UMMA M)
+constexpr int SR_PLANES = 8;              // hi.re hi.im lo.re lo.im sq.re sq.im cu.re cu.im
+constexpr int SR_A_PLANE_U4 = 2 * SR_M;   // uint4 per A plane: [slab 2][row 128][16 bytes]
+constexpr int SR_A_STAGE_BYTES = SR_PLANES * SR_A_PLANE_U4 * 16;  // 32 KB
+constexpr int SR_STAGES = 3;
+constexpr int SR_THREADS = 192;           // producer, MMA issuer, 4 epilogue warps
+constexpr int SR_MAX_N = 2048;            // sites (bit-packed spins of the tile live in shared memory)
+// power-of-two operand scales (keep the FP16 parts normal; removed exactly in the epilogue)
+constexpr float SR_SA = 16.f;             // every t plane
+constexpr float SR_SB1 = 64.f;            // T and T^3/3 planes  -> ODD  is scaled by 2^10
+constexpr float SR_SB2 = 2048.f;          // T^2/2 plane         -> EVEN is scaled by 2^15
+constexpr float SR_INV_ODD = 1.f / (SR_SA * SR_SB1);
+constexpr float SR_INV_EVEN = 1.f / (SR_SA * SR_SB2);
+constexpr float SR_GUARD_FRACTION = 0.5f; // of the tolerance 1e-4 max(1, |E_loc|)
+
+// per table column, written by series_table_kernel (64 bytes)
+struct __align__(16) SeriesCol {
+    float lkr, lki;      // log kappa_c = sum_j log cosh 2 V_jc
+    float a2r, a2i;      // 2 A_c,  A = a_i + p a_k
+    float k0, k1, k2, k3;  // guard: delta_bc = k0 + n2t k1 + n4t k2 + n6t k3 + n8t k4
+    float k4, tmax;      // tmax = max_j |T_jc|
+    int site, sitek;     // flip sites (sitek = -1: single flip)
+    int par, group;      // parity of the column, flip group (-1: padding column)
+    int pad0, pad1;
+};
+static_assert(sizeof(SeriesCol) == 64, "SeriesCol layout");
+
+__host__ __device__ inline int series_bits_stride(int N) { return (N + 31) / 32 | 1; }  // odd: conflict-free rows
+__host__ __device__ inline size_t series_gemm_smem_bytes(int NB, int N) {
+    return (size_t)SR_STAGES * (SR_A_STAGE_BYTES + 256 * NB) + (size_t)NB * sizeof(SeriesCol) +
+           (size_t)SR_M * series_bits_stride(N) * 4 + 256;
+}
+
+__device__ __forceinline__ unsigned pack_h2(float a, float b) {
+    const __half2 h = __floats2half2_rn(a, b);
+    return *reinterpret_cast<const unsigned*>(&h);
+}
+
+// ---------------------------------------------------------------------------------------
+// B operand + per-column data.  One block per (padded) column c, thread <-> 8 consecutive hidden units.
+// B_packed[ntile][jchunk16][plane][slab 2][row NB][8 halves]  (one contiguous 256 NB-byte block per stage)
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) series_table_kernel(const float2* __restrict__ W, const float2* __restrict__ a,
+                                                           int N, int M, int M_pad, int C, int NB,
+                                                           const int* __restrict__ col_i, const int* __restrict__ col_k,
+                                                           const int* __restrict__ col_p,
+                                                           const int* __restrict__ col_group,
+                                                           uint4* __restrict__ B_packed, SeriesCol* __restrict__ cols) {
+    const int c = blockIdx.x, tid = threadIdx.x;
+    const int nt = c / NB, cl = c % NB;
+    const int nJC = M_pad / 16;
+    const bool live_col = c < C;
+    const int ci = live_col ? col_i[c] : 0, ck = live_col ? col_k[c] : -1;
+    const float cp = live_col ? (float)col_p[c] : 1.f;
+    double lkr = 0.0, lki = 0.0;
+    float n2 = 0.f, n4 = 0.f, n6 = 0.f, n8 = 0.f, tmx = 0.f;
+    for (int j8 = tid; j8 < M_pad / 8; j8 += 256) {
+        float v[SR_PLANES][8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int j = j8 * 8 + q;
+            float Tr = 0.f, Ti = 0.f;
+            if (live_col && j < M) {
+                float2 w = W[(long long)j * N + ci];
+                if (ck >= 0) {
+                    const float2 w2 = W[(long long)j * N + ck];
+                    w.x = fmaf(cp, w2.x, w.x);
+                    w.y = fmaf(cp, w2.y, w.y);
+                }
+                float lr, li;
+                lncosh_tanh(2.f * w.x, 2.f * w.y, lr, li, Tr, Ti);
+                lkr += (double)lr;
+                lki += (double)li;
+                const float m2 = fmaf(Tr, Tr, Ti * Ti);
+                n2 += m2;
+                n4 = fmaf(m2, m2, n4);
+                n6 = fmaf(m2 * m2, m2, n6);
+                n8 = fmaf(m2 * m2, m2 * m2, n8);
+                tmx = fmaxf(tmx, m2);
+            }
+            const float sr = Tr * SR_SB1, si = Ti * SR_SB1;
+            v[0][q] = __half2float(__float2half_rn(sr));
+            v[1][q] = __half2float(__float2half_rn(si));
+            v[2][q] = sr - v[0][q];
+            v[3][q] = si - v[1][q];
+            const float T2r = fmaf(Tr, Tr, -Ti * Ti), T2i = 2.f * Tr * Ti;
+            v[4][q] = 0.5f * SR_SB2 * T2r;
+            v[5][q] = 0.5f * SR_SB2 * T2i;
+            v[6][q] = (SR_SB1 / 3.f) * fmaf(Tr, T2r, -Ti * T2i);
+            v[7][q] = (SR_SB1 / 3.f) * fmaf(Tr, T2i, Ti * T2r);
+        }
+        const int jc = j8 >> 1, slab = j8 & 1;
+        uint4* dst = B_packed + (((long long)nt * nJC + jc) * SR_PLANES) * (2 * NB) + slab * NB + cl;
+#pragma unroll
+        for (int pl = 0; pl < SR_PLANES; ++pl)
+            dst[(long long)pl * 2 * NB] = make_uint4(pack_h2(v[pl][0], v[pl][1]), pack_h2(v[pl][2], v[pl][3]),
+                                                     pack_h2(v[pl][4], v[pl][5]), pack_h2(v[pl][6], v[pl][7]));
+    }
+    // block reduction in a fixed order (deterministic)
+    __shared__ double sd[2][256];
+    __shared__ float sf[5][256];
+    sd[0][tid] = lkr, sd[1][tid] = lki;
+    sf[0][tid] = n2, sf[1][tid] = n4, sf[2][tid] = n6, sf[3][tid] = n8, sf[4][tid] = tmx;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (tid < o) {
+            sd[0][tid] += sd[0][tid + o];
+            sd[1][tid] += sd[1][tid + o];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) sf[q][tid] += sf[q][tid + o];
+            sf[4][tid] = fmaxf(sf[4][tid], sf[4][tid + o]);
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        SeriesCol r;
+        r.lkr = (float)sd[0][0];
+        r.lki = (float)sd[1][0];
+        float2 A = make_float2(0.f, 0.f);
+        if (live_col) {
+            A = a[ci];
+            if (ck >= 0) {
+                A.x = fmaf(cp, a[ck].x, A.x);
+                A.y = fmaf(cp, a[ck].y, A.y);
+            }
+        }
+        r.a2r = 2.f * A.x;
+        r.a2i = 2.f * A.y;
+        // guard coefficients; u16 = 2^-21 (hi + lo split), u = 2^-10 (one FP16 part,
+        // both operands), eta = absolute rounding floor of the scaled FP16 subnormals; factor 2 = re / im slack
+        const float n2T = sqrtf(sf[0][0]), n4T = sqrtf(sf[1][0]), n6T = sqrtf(sf[2][0]), n8T = sqrtf(sf[3][0]);
+        const float sqM = sqrtf((float)M);
+        r.k0 = 2.f * sqM * 1.8626451e-9f * n2T;                              // 2^-29 sum_j |T_j|
+        r.k1 = 2.f * (4.7683716e-7f * n2T + sqM * 4.6566129e-10f);           // 2^-21 n2T + 2^-31 sqrt(M)
+        r.k2 = 9.765625e-4f * n4T;                                           // 2 . 2^-10 . 1/2
+        r.k3 = (2.f / 3.f) * 9.765625e-4f * n6T;                             // 2 . 2^-10 . 1/3
+        r.k4 = 0.5f * n8T;                                                   // truncation: 1/(4 (1 - X)), X <= 1/2
+        r.tmax = sqrtf(sf[4][0]);
+        r.site = ci;
+        r.sitek = ck;
+        r.par = (int)cp;
+        r.group = live_col ? col_group[c] : -1;
+        r.pad0 = r.pad1 = 0;
+        cols[c] = r;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// A operand + row norms.  One block per 128-sample tile; thread <-> (pair of samples, 8 hidden units).
+// A_packed[mtile][jchunk16][plane][slab 2][row 128][8 halves]  (32 KB contiguous per stage)
+// rown[b] = (n2t, n4t, n6t, n8t), nPt = sqrt(sum_j |t_bj|^P);  rowmax[b] = max_j |t_bj|
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) series_pack_kernel(const float4* __restrict__ tp, long long nPairsPad, int M_pad,
+                                                          uint4* __restrict__ A_packed, float4* __restrict__ rown,
+                                                          float* __restrict__ rowmax) {
+    const int tid = threadIdx.x, pl = tid & 63, jsub = tid >> 6;
+    const long long mt = blockIdx.x;
+    const long long pair = mt * 64 + pl;
+    const int nJC = M_pad / 16;
+    float acc[2][5] = {{0.f, 0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f, 0.f}};
+    for (int j8 = jsub; j8 < M_pad / 8; j8 += 4) {
+        float4 t[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) t[q] = tp[(long long)(j8 * 8 + q) * nPairsPad + pair];
+        uint4* dst = A_packed + ((mt * nJC + (j8 >> 1)) * SR_PLANES) * SR_A_PLANE_U4 + (j8 & 1) * SR_M + 2 * pl;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            float v[SR_PLANES][8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const float tr = h ? t[q].y : t[q].x, ti = h ? t[q].w : t[q].z;
+                const float m2 = fmaf(tr, tr, ti * ti);
+                acc[h][0] += m2;
+                acc[h][1] = fmaf(m2, m2, acc[h][1]);
+                acc[h][2] = fmaf(m2 * m2, m2, acc[h][2]);
+                acc[h][3] = fmaf(m2 * m2, m2 * m2, acc[h][3]);
+                acc[h][4] = fmaxf(acc[h][4], m2);
+                const float sr = tr * SR_SA, si = ti * SR_SA;
+                v[0][q] = __half2float(__float2half_rn(sr));
+                v[1][q] = __half2float(__float2half_rn(si));
+                v[2][q] = sr - v[0][q];
+                v[3][q] = si - v[1][q];
+                const float t2r = fmaf(tr, tr, -ti * ti), t2i = 2.f * tr * ti;
+                v[4][q] = SR_SA * t2r;
+                v[5][q] = SR_SA * t2i;
+                v[6][q] = SR_SA * fmaf(tr, t2r, -ti * t2i);
+                v[7][q] = SR_SA * fmaf(tr, t2i, ti * t2r);
+            }
+#pragma unroll
+            for (int p = 0; p < SR_PLANES; ++p)
+                dst[p * SR_A_PLANE_U4 + h] = make_uint4(pack_h2(v[p][0], v[p][1]), pack_h2(v[p][2], v[p][3]),
+                                                        pack_h2(v[p][4], v[p][5]), pack_h2(v[p][6], v[p][7]));
+        }
+    }
+    __shared__ float sh[4][128][5];
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int q = 0; q < 5; ++q) sh[jsub][2 * pl + h][q] = acc[h][q];
+    __syncthreads();
+    if (tid < 128) {
+        float s[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) s[q] = sh[0][tid][q];
+        for (int k = 1; k < 4; ++k) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) s[q] += sh[k][tid][q];
+            s[4] = fmaxf(s[4], sh[k][tid][4]);
+        }
+        const long long b = mt * SR_M + tid;
+        rown[b] = make_float4(sqrtf(s[0]), sqrtf(s[1]), sqrtf(s[2]), sqrtf(s[3]));
+        rowmax[b] = sqrtf(s[4]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// tcgen05 kind::f16 wrappers (descriptors: umma_desc of nqs_theta_mma.cuh; the byte layout of a K = 16
+// FP16 step equals that of a K = 32 INT8 step: two 16-byte slabs)
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
+    uint32_t r[16];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int k = 0; k < 16; ++k) v[k] = __uint_as_float(r[k]);
+}
+// D = F32, A = B = F16, K-major both, N >> 3 at bit 17, M >> 4 at bit 24; bit 13 negates A
+__host__ __device__ inline uint32_t series_idesc(int NB) {
+    return (1u << 4) | ((uint32_t)(NB >> 3) << 17) | ((uint32_t)(SR_M >> 4) << 24);
+}
+constexpr uint32_t SR_IDESC_NEG_A = 1u << 13;
+
+// spin of site i from a bit-packed row (bit = 1 <=> spin +1)
+__device__ __forceinline__ float spin_from_bits(const uint32_t* __restrict__ bits, int i) {
+    return ((bits[i >> 5] >> (i & 31)) & 1u) ? 1.f : -1.f;
+}
+
+struct SeriesGemmParams {
+    const uint4* A_packed;   // [nMT][nJC][8][256]
+    const uint4* B_packed;   // [nNT][nJC][8][2 NB]
+    const SeriesCol* cols;   // [nNT * NB]
+    const float4* rown;      // [B_pad]
+    const float* rowmax;     // [B_pad]
+    const int8_t* spins;     // [B][N]
+    long long B;
+    int N, nJC, NB, nNT;
+    DevHam H;
+    float4* partial;         // [B][nNT]: (Re, Im of sum_c m R [+ diagonal in tile 0], guard eps, 0)
+};
+
+__global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const SeriesGemmParams p) {
+    extern __shared__ __align__(128) unsigned char sr_smem[];
+    const int NB = p.NB;
+    const uint32_t b_stage_bytes = 256u * NB, stage_bytes = SR_A_STAGE_BYTES + b_stage_bytes;
+    SeriesCol* const scol = reinterpret_cast<SeriesCol*>(sr_smem + (size_t)SR_STAGES * stage_bytes);
+    uint32_t* const sbits = reinterpret_cast<uint32_t*>(scol + NB);
+    const int bstride = series_bits_stride(p.N);
+    uint64_t* const bars = reinterpret_cast<uint64_t*>(sbits + (size_t)SR_M * bstride);
+    uint64_t* const full = bars;
+    uint64_t* const empty = bars + SR_STAGES;
+    uint64_t* const t_full = bars + 2 * SR_STAGES;
+    uint32_t* const tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * SR_STAGES + 1);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int nt = blockIdx.x % p.nNT;
+    const long long mt = blockIdx.x / p.nNT;
+    const int nJC = p.nJC;
+
+    if (tid == 0) {
+        for (int s = 0; s < SR_STAGES; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], 1);
+        }
+        mbar_init(t_full, 1);
+        fence_mbar_init();
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        if (lane == 0) {
+            const uint4* gA = p.A_packed + mt * (long long)nJC * SR_PLANES * SR_A_PLANE_U4;
+            const uint4* gB = p.B_packed + (long long)nt * nJC * SR_PLANES * (2 * NB);
+            for (int kc = 0; kc < nJC; ++kc) {
+                const int s = kc % SR_STAGES;
+                mbar_wait(&empty[s], ((kc / SR_STAGES) & 1) ^ 1);
+                unsigned char* const st = sr_smem + (size_t)s * stage_bytes;
+                mbar_expect_tx(&full[s], stage_bytes);
+                bulk_g2s(st, gA + (long long)kc * SR_PLANES * SR_A_PLANE_U4, SR_A_STAGE_BYTES, &full[s]);
+                bulk_g2s(st + SR_A_STAGE_BYTES, gB + (long long)kc * SR_PLANES * (2 * NB), b_stage_bytes, &full[s]);
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            const uint32_t s0 = smem_u32(sr_smem);
+            const uint32_t idesc = series_idesc(NB);
+            const uint32_t b_plane = 32u * NB, b_lbo = 16u * NB;
+            // accumulator column ranges: ODD.re, ODD.im, EVEN.re, EVEN.im
+            const uint32_t d_or = tmem_base, d_oi = tmem_base + NB, d_er = tmem_base + 2 * NB, d_ei = tmem_base + 3 * NB;
+            for (int kc = 0; kc < nJC; ++kc) {
+                const int s = kc % SR_STAGES;
+                mbar_wait(&full[s], (kc / SR_STAGES) & 1);
+                tc_fence_after();
+                const uint32_t sa = s0 + (uint32_t)s * stage_bytes, sb = sa + SR_A_STAGE_BYTES;
+                auto A = [&](int pl) { return umma_desc(sa + (uint32_t)pl * 4096u, 2048u, 128u); };
+                auto Bd = [&](int pl) { return umma_desc(sb + (uint32_t)pl * b_plane, b_lbo, 128u); };
+                // one complex product (a.re, a.im = planes pa, pa + 1) x (b.re, b.im = planes pb, pb + 1)
+                auto cprod = [&](int pa, int pb, uint32_t dre, uint32_t dim, uint32_t first) {
+                    umma_f16(dre, A(pa), Bd(pb), idesc, first);
+                    umma_f16(dre, A(pa + 1), Bd(pb + 1), idesc | SR_IDESC_NEG_A, 1u);
+                    umma_f16(dim, A(pa), Bd(pb + 1), idesc, first);
+                    umma_f16(dim, A(pa + 1), Bd(pb), idesc, 1u);
+                };
+                const uint32_t first = kc ? 1u : 0u;
+                cprod(0, 0, d_or, d_oi, first);   // t.hi T.hi
+                cprod(0, 2, d_or, d_oi, 1u);      // t.hi T.lo
+                cprod(2, 0, d_or, d_oi, 1u);      // t.lo T.hi
+                cprod(6, 6, d_or, d_oi, 1u);      // t^3 T^3 / 3
+                cprod(4, 4, d_er, d_ei, first);   // t^2 T^2 / 2
+                tc_commit(&empty[s]);
+            }
+            tc_commit(t_full);
+        }
+    } else {
+        // ---------------- epilogue warps: TMEM lane group = warp % 4
+        const int lane_grp = warp & 3;
+        const int row = lane_grp * 32 + lane;
+        const long long b = mt * SR_M + row;
+        // while the MMAs run: column records -> smem, bit-packed spins of the tile, diagonal element
+        for (int idx = tid - 64; idx < NB * 4; idx += 128)
+            reinterpret_cast<uint4*>(scol)[idx] = reinterpret_cast<const uint4*>(p.cols + (long long)nt * NB)[idx];
+        for (int r = 0; r < 32; ++r) {
+            const long long br = mt * SR_M + lane_grp * 32 + r;
+            for (int w = 0; w < bstride; ++w) {
+                const int i = w * 32 + lane;
+                const bool up = (br < p.B && i < p.N) ? (p.spins[br * p.N + i] > 0) : false;
+                const uint32_t word = __ballot_sync(0xffffffffu, up);
+                if (lane == 0) sbits[(size_t)(lane_grp * 32 + r) * bstride + w] = word;
+            }
+        }
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        const uint32_t* const mybits = sbits + (size_t)row * bstride;
+        float er_acc = 0.f, ei_acc = 0.f, eps = 0.f;
+        if (nt == 0) {  // diagonal terms (empty flip set): d = sum_t c_t s[z0] s[z1]
+            for (int t = 0; t < p.H.Td; ++t) {
+                const int z0 = p.H.diag_z0[t], z1 = p.H.diag_z1[t];
+                float f = 1.f;
+                if (z0 >= 0) f *= spin_from_bits(mybits, z0);
+                if (z1 >= 0) f *= spin_from_bits(mybits, z1);
+                const float2 cc = p.H.diag_c[t];
+                er_acc = fmaf(cc.x, f, er_acc);
+                ei_acc = fmaf(cc.y, f, ei_acc);
+            }
+        }
+        const float4 rn = p.rown[b];
+        const float rmax = p.rowmax[b];
+        mbar_wait(t_full, 0);
+        tc_fence_after();
+        const uint32_t tbase = tmem_base + ((uint32_t)(lane_grp * 32) << 16);
+#pragma unroll 1
+        for (int c0 = 0; c0 < NB; c0 += 16) {
+            float vor[16], voi[16], ver[16], vei[16];
+            tmem_ld16(tbase + (uint32_t)c0, vor);
+            tmem_ld16(tbase + (uint32_t)(NB + c0), voi);
+            tmem_ld16(tbase + (uint32_t)(2 * NB + c0), ver);
+            tmem_ld16(tbase + (uint32_t)(3 * NB + c0), vei);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const SeriesCol& cr = scol[c0 + q];
+                if (cr.group < 0) continue;
+                const float si = spin_from_bits(mybits, cr.site);
+                if (cr.sitek >= 0 && si * spin_from_bits(mybits, cr.sitek) != (float)cr.par) continue;
+                // summed matrix element of the group (Eq. 39)
+                const int first = p.H.grp_first[cr.group], count = p.H.grp_count[cr.group];
+                float mr = 0.f, mi = 0.f;
+                for (int u = 0; u < count; ++u) {
+                    const int z0 = p.H.gt_z0[first + u], z1 = p.H.gt_z1[first + u];
+                    float f = 1.f;
+                    if (z0 >= 0) f *= spin_from_bits(mybits, z0);
+                    if (z1 >= 0) f *= spin_from_bits(mybits, z1);
+                    const float2 cc = p.H.gt_c[first + u];
+                    mr = fmaf(cc.x, f, mr);
+                    mi = fmaf(cc.y, f, mi);
+                }
+                if (mr == 0.f && mi == 0.f) continue;
+                // log R = log kappa - sigma (2 A + ODD) - EVEN
+                const float zr = cr.lkr - si * fmaf(SR_INV_ODD, vor[q], cr.a2r) - SR_INV_EVEN * ver[q];
+                float zi = cr.lki - si * fmaf(SR_INV_ODD, voi[q], cr.a2i) - SR_INV_EVEN * vei[q];
+                const float kk = rintf(zi * 0.15915494309189535f);
+                zi = fmaf(-kk, 6.2831855f, zi);
+                zi = fmaf(-kk, -1.7484555e-7f, zi);
+                float sn, cs;
+                __sincosf(zi, &sn, &cs);
+                const float mag = expf(zr);
+                const float Rr = mag * cs, Ri = mag * sn;
+                er_acc += mr * Rr - mi * Ri;
+                ei_acc += mr * Ri + mi * Rr;
+                // guard: |m R| (k0 + n2t k1 + n4t k2 + n6t k3 + n8t k4), valid while max |t| max |T| <= 1/2
+                const float delta = fmaf(rn.x, cr.k1, fmaf(rn.y, cr.k2, fmaf(rn.z, cr.k3, fmaf(rn.w, cr.k4, cr.k0))));
+                const float wgt = (fabsf(mr) + fabsf(mi)) * mag;
+                eps += (rmax * cr.tmax <= 0.5f) ? wgt * delta : __int_as_float(0x7f800000);
+            }
+        }
+        if (b < p.B) p.partial[b * p.nNT + nt] = make_float4(er_acc, ei_acc, eps, 0.f);
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc(tmem_base, 512);
+    }
+}
+
+// E_loc = sum of the column tiles' partial sums (the diagonal rides in tile 0); guard: the call fails as a
+// whole if any sample's error bound exceeds SR_GUARD_FRACTION * 1e-4 * max(1, |E_loc|) (or is NaN).
+// status[0] |= 1 when the guard fails (read by eloc_kernel / finalize_kernel), status[1] counts the samples.
+__global__ void series_guard_kernel(const float4* __restrict__ partial, long long B, int nNT, float2* __restrict__ eloc,
+                                    int* __restrict__ status) {
+    const long long b = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    float er = 0.f, ei = 0.f, eps = 0.f;
+    for (int t = 0; t < nNT; ++t) {
+        const float4 v = partial[b * nNT + t];
+        er += v.x;
+        ei += v.y;
+        eps += v.z;
+    }
+    eloc[b] = make_float2(er, ei);
+    const float mod = sqrtf(er * er + ei * ei);
+    const bool ok = eps <= SR_GUARD_FRACTION * 1e-4f * fmaxf(1.f, mod);  // false for NaN
+    if (!ok) {
+        atomicOr(&status[0], 1);
+        atomicAdd(&status[1], 1);
+    }
+}
+
+}  // namespace nqs

@@ -100,8 +100,14 @@ def test_forces_config5_full_size_sampled_outputs(nqs, oracle):
     w = wl.make_config(5)
     eloc = synthetic_eloc(w.B, 55, centre=-1200.0)
     F, st = gpu_forces(nqs, w, eloc)
-    jsel = np.sort(np.random.default_rng(56).choice(w.M, size=12, replace=False))
-    jsel[0], jsel[-1] = 0, w.M - 1
+    # 12 random hidden units plus the tile boundaries of force_mma_kernel (32 hidden units per CTA column):
+    # first / last unit and both sides of a boundary near each end.  All N sites are compared for every
+    # sampled unit, so the site-tile boundaries i = 127|128, 255|256, 383|384 are covered by construction
+    # (asserted below).
+    forced = [0, 31, 32, 1567, 1568, w.M - 1]
+    rnd = np.random.default_rng(56).choice(w.M, size=12, replace=False)
+    jsel = np.unique(np.concatenate([rnd, forced]))
+    assert {31, 32, 1567, 1568} <= set(jsel.tolist()) and w.N > 384
     F_ref = oracle.forces(w.spins, w.a, w.b[jsel], w.W[jsel], eloc)
     N, M = w.N, w.M
     S = scale_S(wl.Workload("sub", N, len(jsel), w.B, w.spins, w.a, w.b[jsel], w.W[jsel], w.ham), eloc)
@@ -144,7 +150,9 @@ def test_forces_error_codes(nqs):
         nqs.forces(t(w.spins), t(w.a), t(w.b), t(w.W), t(synthetic_eloc(w.B + 1, 1)))
     lib = nqs.load_library()
     assert lib.nqs_forces(None, 4, 8, 8, None, None, None, None, None, None, None, None) == -1
-    assert lib.nqs_energy_stats(None, None, 0, None, None) == -1
+    assert lib.nqs_energy_stats(None, None, -1, None, None) == -1
+    assert lib.nqs_energy_stats(None, None, 0, None, None) == 0  # B == 0 is a no-op for every entry point
+    assert lib.nqs_forces(None, 0, 8, 8, None, None, None, None, None, None, None, None) == 0
 
 
 def test_fused_local_energy_forces_equals_the_two_calls(nqs):

@@ -1,13 +1,17 @@
 """Parity of nqs_metropolis against the float64 oracle.
 
 Floating point decides an integer here (accept / reject), and the kernel takes the decision in
-float32 from a product form the oracle does not use.  So: the oracle reports for
-every chain how close its closest decision was to a tie (min_margin, in log |ratio|^2); chains whose
-margin exceeds MARGIN must come out BIT-IDENTICAL (final spins and accepted count); the others must
-still be valid configurations.  MARGIN and the robust-fraction floor were set empirically, after a
-first choice (1e-3, >= 90 %) failed on the robust fraction: 2e-4 is about 10x the float32 error of
-log |ratio|^2 seen at these sizes.  See DESIGN.md section 9 for the two kernel formulations this rule
-was run against and which cases each failed.
+float32 from a product form the oracle does not use.  Several chains are therefore correct; what is
+unique is checked on EVERY chain (reading Q19): both sides emit their per-step
+accept bits (nqs_metropolis_trace / oracle.metropolis(trace=True)), and
+  * a chain whose decisions never differ from the oracle's must be bit-identical in final spins and
+    accepted count;
+  * where a chain differs, the FIRST step at which the two decide differently must be a near-tie for the
+    oracle at that very step: margin |2 Re dlog psi - log u| < MARGIN.  (After that step the two chains are
+    in different states and are no longer comparable; the chain must still be a valid configuration and
+    consistent with its own accept bits.)
+MARGIN = 2e-4 is about 10x the float32 error of log |ratio|^2 seen at these sizes; it was set empirically
+in round 1 and has not been changed.  There is no robust-fraction floor any more: it judged the inputs.
 """
 import numpy as np
 import pytest
@@ -36,23 +40,48 @@ def proposals(S, C, N, seed):
     return rng.integers(0, N, (S, C)).astype(np.int32), rng.random((S, C), dtype=np.float32)
 
 
-def gpu_metropolis(nqs, spins, a, b, W, sites, u):
+def gpu_metropolis(nqs, spins, a, b, W, sites, u, trace=False):
     import torch
 
     d = torch.device("cuda:0")
     t = lambda x: torch.from_numpy(np.ascontiguousarray(x)).to(d)  # noqa: E731
     sp = t(spins.copy())
-    acc = nqs.metropolis(sp, t(a), t(b), t(W), t(sites), t(u))
+    out = nqs.metropolis(sp, t(a), t(b), t(W), t(sites), t(u), trace=trace)
     torch.cuda.synchronize()
-    return sp.cpu().numpy(), acc.cpu().numpy()
+    if trace:
+        return sp.cpu().numpy(), out[0].cpu().numpy(), out[1].cpu().numpy()
+    return sp.cpu().numpy(), out.cpu().numpy()
 
 
-def compare(final, acc, ref_final, ref_acc, margin, what, min_robust=0.85):
+def replay(start, sites, dec):
+    """The chain states implied by a table of accept bits (bit-exact index work, no arithmetic)."""
+    s = start.copy()
+    cols = np.arange(s.shape[0])
+    for t in range(sites.shape[0]):
+        acc = dec[t].astype(bool)
+        s[cols[acc], sites[t, acc]] *= -1
+    return s
+
+
+def compare(start, sites, final, acc, dec, ref_final, ref_acc, ref_dec, ref_mar, what):
+    """Every chain is judged: identical decisions => identical result; otherwise the first differing
+    decision must have been a near-tie in float64.  Returns the number of chains that parted ways."""
     assert set(np.unique(final)) <= {-1, 1}, what
-    robust = margin > MARGIN
-    assert robust.mean() >= min_robust, f"{what}: only {robust.mean():.2%} of the chains are robust"
-    bad = np.flatnonzero(robust & (np.any(final != ref_final, axis=1) | (acc != ref_acc)))
-    assert bad.size == 0, f"{what}: {bad.size} robust chains differ, first {bad[:5]}, margins {margin[bad[:5]]}"
+    assert set(np.unique(dec)) <= {0, 1}, what
+    # the kernel's outputs are consistent with its own trace
+    assert np.array_equal(dec.sum(axis=0), acc), f"{what}: accepted count != number of accept bits"
+    assert np.array_equal(replay(start, sites, dec), final), f"{what}: final spins do not follow from the accept bits"
+    differ = dec != ref_dec
+    parted = differ.any(axis=0)
+    same = ~parted
+    assert np.array_equal(final[same], ref_final[same]) and np.array_equal(acc[same], ref_acc[same]), what
+    if parted.any():
+        first = differ.argmax(axis=0)[parted]
+        m = ref_mar[first, np.flatnonzero(parted)]
+        bad = np.flatnonzero(m >= MARGIN)
+        assert bad.size == 0, (f"{what}: {bad.size} chains part from the oracle at a decision that was no tie: "
+                               f"chains {np.flatnonzero(parted)[bad[:5]]}, steps {first[bad[:5]]}, margins {m[bad[:5]]}")
+    return int(parted.sum())
 
 
 @pytest.mark.parametrize("N,M,C,S,sigma,seed", [
@@ -66,27 +95,34 @@ def compare(final, acc, ref_final, ref_acc, margin, what, min_robust=0.85):
 def test_metropolis_vs_oracle(nqs, oracle, N, M, C, S, sigma, seed):
     w = wl.make_random(N, M, C, 4, sigma, 200 + seed)
     sites, u = proposals(S, w.B, N, seed)
-    final, acc = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, u)
-    ref_final, ref_acc, margin = oracle.metropolis(w.spins, w.a, w.b, w.W, sites, u)
-    compare(final, acc, ref_final, ref_acc, margin, f"N={N} M={M} C={w.B} S={S}", min_robust=0.5 if S > 1000 else 0.85)
+    final, acc, dec = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, u, trace=True)
+    ref_final, ref_acc, _, ref_dec, ref_mar = oracle.metropolis(w.spins, w.a, w.b, w.W, sites, u, trace=True)
+    parted = compare(w.spins, sites, final, acc, dec, ref_final, ref_acc, ref_dec, ref_mar,
+                     f"N={N} M={M} C={w.B} S={S}")
+    assert parted <= 0.5 * w.B  # sanity only: the judgement is per chain, above
     assert 0.05 < acc.mean() / S <= 1.0
+    # the untraced entry point gives the same chains
+    f2, a2 = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, u)
+    assert np.array_equal(f2, final) and np.array_equal(a2, acc)
 
 
 def test_metropolis_config5_full_size_sampled_chains(nqs, oracle):
     """Config 5 at full size (65536 chains, the launch configuration of the sampler bench): chains are
-    independent, so the oracle replays 48 sampled chains one by one."""
+    independent, so the oracle replays 48 sampled chains one by one; every chain is checked against its
+    own accept bits."""
     w = wl.make_config(5)
     S = 24
     sites, u = proposals(S, w.B, w.N, 55)
-    final, acc = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, u)
+    final, acc, dec = gpu_metropolis(nqs, w.spins, w.a, w.b, w.W, sites, u, trace=True)
     assert set(np.unique(final)) <= {-1, 1}
+    assert np.array_equal(dec.sum(axis=0), acc)
+    assert np.array_equal(replay(w.spins, sites, dec), final)
     sel = np.sort(np.random.default_rng(56).choice(w.B, size=48, replace=False))
     sel[0], sel[-1] = 0, w.B - 1
-    ref_final, ref_acc, margin = oracle.metropolis(w.spins[sel], w.a, w.b, w.W, sites[:, sel], u[:, sel])
-    compare(final[sel], acc[sel], ref_final, ref_acc, margin, "config 5 sampled chains")
-    # every chain: the flipped sites are exactly the accepted proposals' parity
-    flips = (final != w.spins).sum(axis=1)
-    assert np.all(flips <= acc) and np.all((acc - flips) % 2 == 0)
+    ref_final, ref_acc, _, ref_dec, ref_mar = oracle.metropolis(w.spins[sel], w.a, w.b, w.W, sites[:, sel], u[:, sel],
+                                                                trace=True)
+    compare(w.spins[sel], sites[:, sel], final[sel], acc[sel], dec[:, sel], ref_final, ref_acc, ref_dec, ref_mar,
+            "config 5 sampled chains")
 
 
 def test_metropolis_properties(nqs):

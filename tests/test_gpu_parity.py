@@ -94,21 +94,51 @@ def test_config2_full_batch(nqs, oracle):
     check_logpsi(l[idx], l_def, "c2 definition")
 
 
-@pytest.mark.parametrize("k,n_fast,n_def", [(3, 768, 24), (4, 768, 24), (5, 160, 8)])
-def test_full_size_configs_sampled_outputs(nqs, oracle, k, n_fast, n_def):
-    """GPU runs the FULL batch in bench.py's launch configuration; the oracle recomputes a
-    strided sample of the outputs (fast mode) and a smaller one in definition mode."""
-    w = wl.make_config(k)
-    e, l = gpu_eloc(nqs, w)
+_ORACLE_CACHE = {}
+
+
+def full_size_sample(k, B):
+    """Outputs the oracle recomputes at full size: three whole 128-sample tiles (first, middle, last: every
+    position inside a CTA of either a5 kernel, i.e. every b mod 128 and b mod 64) plus every 17th sample of
+    the batch (17 is coprime to the tile sizes, so every residue and ~every tile is hit)."""
+    mid = (B // 2) // 128 * 128
+    idx = np.concatenate([np.arange(0, 128), np.arange(mid, mid + 128), np.arange(B - 128, B), np.arange(0, B, 17)])
+    idx = np.unique(idx)
+    d_idx = np.unique(np.concatenate([np.linspace(0, B - 1, 28).astype(np.int64), [63, 64, 127, 128, B - 129, B - 128]]))
+    return idx, d_idx
+
+
+def oracle_full_size(oracle, k):
+    if k not in _ORACLE_CACHE:
+        w = wl.make_config(k)
+        idx, d_idx = full_size_sample(k, w.B)
+        _ORACLE_CACHE[k] = (w, idx, oracle_on(oracle, w, idx, "fast"), d_idx, oracle_on(oracle, w, d_idx, "definition"))
+    return _ORACLE_CACHE[k]
+
+
+@pytest.mark.parametrize("path", ["auto", "product"])
+@pytest.mark.parametrize("k", [3, 4, 5])
+def test_full_size_configs_sampled_outputs(nqs, oracle, k, path):
+    """GPU runs the FULL batch in bench.py's launch configuration, once through the default a5 path (the
+    tensor-core series with its guard at these sizes) and once through the FP32 product form; the oracle
+    recomputes >= 4096 sampled outputs in fast mode and >= 32 in definition mode (see full_size_sample)."""
+    w, idx, (e_ref, l_ref), d_idx, (e_def, l_def) = oracle_full_size(oracle, k)
+    assert idx.size >= 4096 and d_idx.size >= 32
+    nqs.set_option("a5_path", nqs.A5_PATHS[path])
+    try:
+        e, l = gpu_eloc(nqs, w)
+        took = nqs.debug_last_a5()
+    finally:
+        nqs.set_option("a5_path", 0)
+    if path == "auto":
+        assert took["path"] == "series" and not took["guard_failed"], took  # the configs sit well inside the guard
+    else:
+        assert took["path"] == "product", took
     assert np.all(np.isfinite(e.view(np.float32))) and np.all(np.isfinite(l.view(np.float32)))
-    idx = np.unique(np.concatenate([np.linspace(0, w.B - 1, n_fast).astype(np.int64), [0, 1, w.B - 2, w.B - 1]]))
-    e_ref, l_ref = oracle_on(oracle, w, idx, "fast")
-    check_eloc(e[idx], e_ref, f"c{k} fast")
-    check_logpsi(l[idx], l_ref, f"c{k} fast")
-    idx = np.linspace(0, w.B - 1, n_def).astype(np.int64)
-    e_def, l_def = oracle_on(oracle, w, idx, "definition")
-    check_eloc(e[idx], e_def, f"c{k} definition")
-    check_logpsi(l[idx], l_def, f"c{k} definition")
+    check_eloc(e[idx], e_ref, f"c{k} fast [{path}]")
+    check_logpsi(l[idx], l_ref, f"c{k} fast [{path}]")
+    check_eloc(e[d_idx], e_def, f"c{k} definition [{path}]")
+    check_logpsi(l[d_idx], l_def, f"c{k} definition [{path}]")
     # property that holds at any size (TFIM: zero-parameter closed form is tested separately);
     # here: the batch mean is finite and the imaginary parts are small against the real ones
     assert abs(e.imag.mean()) < 0.05 * abs(e.real.mean())
@@ -220,8 +250,10 @@ def test_enumerator_against_oracle_connected(nqs, oracle):
     w = wl.make_random(11, 4, 40, 70, 0.1, 55)
     ham = nqs.Hamiltonian(w.N, w.ham.sites, w.ham.paulis, w.ham.coeffs)
     spins = torch.from_numpy(w.spins).cuda()
-    sp, mel = nqs.enumerate_connected(ham, spins)
+    sp, mel, G = nqs.enumerate_connected(spins, w.ham.sites, w.ham.paulis, w.ham.coeffs)  # SURVEY 8(b) form
+    sp_h, mel_h = nqs.enumerate_connected_h(ham, spins)                                   # handle form
     torch.cuda.synchronize()
+    assert G == ham.G and torch.equal(sp, sp_h) and torch.equal(mel, mel_h)
     sp, mel = sp.cpu().numpy(), mel.cpu().numpy().astype(np.complex128)
     sp_ref, mel_ref = oracle.connected(w.spins, w.ham.sites, w.ham.paulis, w.ham.coeffs)
     assert sp.shape == (w.B, ham.G + 1, w.N)

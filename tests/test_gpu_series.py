@@ -1,0 +1,141 @@
+"""The guarded tensor-core series path of step a5 (csrc/nqs_series.cuh) against the
+float64 oracle, through the C ABI.
+
+  log psi(s')/psi(s) = log kappa_c - 2 sigma A_c - sigma ODD - EVEN,  truncated at k = 3, FP16 operands
+  (hi + lo split for k = 1) on tcgen05 with FP32 accumulators, and a per-sample a-posteriori error bound
+  (the guard) that sends the whole call back to the FP32 product form when it exceeds
+  0.5e-4 max(1, |E_loc|).
+
+Tolerances are the hot path's (north_star): |Re dE|, |Im dE| <= 1e-4 max(1, |E_loc|) per sample.
+nqs_set_option(NQS_OPT_A5_PATH): 2 = series + guard + fallback at any size, 3 = series only (the guard is
+recorded, nothing is recomputed) -- the latter is how the guard's SUFFICIENCY is tested: whenever the guard
+passes, the series result alone must already meet the tolerance.
+"""
+import numpy as np
+import pytest
+
+import workloads as wl
+from test_gpu_parity import check_eloc, check_logpsi, gpu_eloc, oracle_on
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def nqs():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests need a B200")
+    import paper_2108_03409_b200 as m
+
+    m.load_library()
+    yield m
+    m.set_option("a5_path", 0)
+
+
+def run(nqs, w, path):
+    nqs.set_option("a5_path", nqs.A5_PATHS[path])
+    try:
+        e, l = gpu_eloc(nqs, w)
+        took = nqs.debug_last_a5()
+    finally:
+        nqs.set_option("a5_path", 0)
+    return e, l, took
+
+
+@pytest.mark.parametrize("N,M,B,T,sigma,seed", [
+    (6, 5, 64, 40, 0.02, 301),      # all 2^N states; every Pauli type, complex coefficients; M, C ragged
+    (9, 17, 77, 60, 0.02, 302),     # B not a multiple of the 128-sample tile
+    (13, 7, 257, 90, 0.01, 303),    # three sample tiles, the last one with one live row
+    (33, 40, 515, 200, 0.003, 304),  # > 128 columns: two column tiles
+    (70, 33, 300, 700, 0.001, 305),  # many pair-flip groups, both parities
+])
+def test_series_only_random_terms_vs_definition(nqs, oracle, N, M, B, T, sigma, seed):
+    """Small parameters (inside the guard), general term lists: the series kernel ALONE (no fallback) against
+    definition mode -- matrix elements, parities, diagonal, ragged tiles.  (Random complex coefficients make
+    sum |m| large against |E_loc|, so the guard is strict here: sigma is chosen small.)"""
+    w = wl.make_random(N, M, B, T, sigma, seed)
+    e, l, took = run(nqs, w, "series_only")
+    assert took["path"] == "series" and not took["guard_failed"], took
+    e_ref, l_ref = oracle_on(oracle, w, slice(None), "definition")
+    check_eloc(e, e_ref, f"series N={N}")
+    check_logpsi(l, l_ref, f"series N={N}")
+
+
+def test_series_pair_flip_parities_and_y_terms(nqs, oracle):
+    N, M, B = 8, 12, 200
+    w = wl.make_random(N, M, B, 1, 0.02, 7)
+    rows = []
+    for i in range(N):
+        k = (i + 3) % N
+        rows += [(i, 1, k, 1, 0.7 + 0.1j), (i, 1, k, 2, -0.3j), (i, 2, k, 1, 0.2), (i, 2, k, 2, 1.1)]
+    rows += [(2, 2, -1, 0, 0.5), (-1, 0, 5, 2, 0.25j), (3, 1, 6, 3, 0.4), (3, 2, 1, 3, -0.6), (-1, 0, -1, 0, 2.5)]
+    w.ham = wl._terms(rows)
+    e, l, took = run(nqs, w, "series_only")
+    assert took["path"] == "series" and not took["guard_failed"], took
+    e_ref, l_ref = oracle_on(oracle, w, slice(None), "definition")
+    check_eloc(e, e_ref, "series pair flips")
+
+
+@pytest.mark.parametrize("sigma", [0.1, 0.3, 0.5])
+def test_p10_takes_the_fallback(nqs, oracle, sigma):
+    """Pin P10 (large parameters): the guard must refuse the series and the product form must answer."""
+    w = wl.make_robustness(sigma, B=256)
+    e, l, took = run(nqs, w, "series_guarded")
+    assert took["path"] == "series" and took["guard_failed"] and took["samples_over"] > 0, took
+    e_prod, _, took_p = run(nqs, w, "product")
+    assert took_p["path"] == "product"
+    assert np.array_equal(e, e_prod)  # the fallback IS the product-form result, bit for bit
+    e_ref, l_ref = oracle_on(oracle, w, slice(None), "fast")
+    if sigma == 0.1:
+        check_eloc(e, e_ref, "P10 sigma=0.1 via fallback")
+    else:
+        rel = np.abs(e.astype(np.complex128) - e_ref) / np.maximum(1.0, np.abs(e_ref))
+        assert np.all(np.isfinite(e.view(np.float32))) and rel.max() <= 1e-3
+
+
+def test_guard_boundary_inside_and_outside(nqs, oracle):
+    """Config-3 shapes with growing parameter scale.  The guard decision must be monotone in sigma; wherever it
+    PASSES, the series alone meets the tolerance (sufficiency: checked with the fallback disabled); just
+    outside, the guarded call still meets it through the product form."""
+    sigmas = [0.01, 0.014, 0.02, 0.028, 0.04, 0.056, 0.08]
+    passed = []
+    for sg in sigmas:
+        w = wl.make_config(3, B=384, sigma=sg, seed=31)
+        e_ref, l_ref = oracle_on(oracle, w, slice(None), "fast")
+        e3, _, took3 = run(nqs, w, "series_only")
+        passed.append(not took3["guard_failed"])
+        if passed[-1]:
+            check_eloc(e3, e_ref, f"series only, sigma={sg} (guard passed)")
+        e2, _, took2 = run(nqs, w, "series_guarded")
+        assert took2["guard_failed"] == took3["guard_failed"]
+        check_eloc(e2, e_ref, f"guarded, sigma={sg}")
+    assert passed[0], "config 3's own sigma must be inside the guard"
+    assert not passed[-1], "sigma = 0.08 at M = 400 must be outside the guard"
+    first_fail = passed.index(False)
+    assert not any(passed[first_fail:]), f"guard decision is not monotone in sigma: {list(zip(sigmas, passed))}"
+
+
+def test_series_is_deterministic_and_matches_product_within_tolerance(nqs, oracle):
+    import torch
+
+    w = wl.make_config(3, B=3000)
+    e1, l1, t1 = run(nqs, w, "series_only")
+    e2, l2, t2 = run(nqs, w, "series_only")
+    assert np.array_equal(e1, e2) and np.array_equal(l1, l2)
+    ep, lp, _ = run(nqs, w, "product")
+    assert np.array_equal(l1, lp)  # log psi does not depend on the a5 path
+    tol = 1e-4 * np.maximum(1.0, np.abs(ep))
+    assert np.all(np.abs(e1.real - ep.real) <= 2 * tol) and np.all(np.abs(e1.imag - ep.imag) <= 2 * tol)
+    torch.cuda.synchronize()
+
+
+def test_auto_threshold(nqs):
+    """Automatic choice: small problems stay on the product form (the series' packing does not pay below
+    2^28 triples), large ones take the series."""
+    w = wl.make_config(2, B=2000)
+    _, _, took = run(nqs, w, "auto")
+    assert took["path"] == "product"
+    w = wl.make_config(3, B=8192)  # 8192 * 100 * 400 = 3.3e8 >= 2^28
+    _, _, took = run(nqs, w, "auto")
+    assert took["path"] == "series" and not took["guard_failed"]
