@@ -31,9 +31,25 @@ import workloads as wl  # noqa: E402
 SM_COUNT = 148
 FP32_LANES_PER_SM = 128
 L2_FLUSH_BYTES = 256 << 20
-# dram__bytes_read.sum + dram__bytes_write.sum of one eloc_kernel launch at config 5, from the
-# ncu --set full capture summarised in profiles/ (None until a capture exists)
-ELOC_KERNEL_DRAM_TRAFFIC_BYTES = 897_815_552  # profiles/r1_v3_ncu_summary.md: dram read + write per launch
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from `ncu --set full` captures
+# summarised under profiles/ -- (workload, kernel) -> (bytes, file).  No capture for that pair => traffic is null.
+NCU_DRAM_TRAFFIC = {
+    ("c5_tfim_20x20", "eloc_kernel"): (897_815_552, "profiles/r1_v3_ncu_summary.md"),
+}
+# nominal ratio of the dense INT8 to the dense BF16/FP16 tensor peak (B200_PROFILING.md: 4.5 vs 2.25 P)
+INT8_OVER_BF16 = 2.0
+
+
+def measured_peaks() -> dict:
+    """MEASURED_PEAKS.json (driver-written) or the profiling guide's stated fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return dict(bf16_tflops=float(d["bf16_tflops"]), bf16_tflops_sustained=float(d.get("bf16_tflops_sustained", 0.0)),
+                    hbm_gbs=float(d["hbm_gbs"]), source="MEASURED_PEAKS.json (of measured)")
+    return dict(bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, hbm_gbs=6650.0,
+                source="B200_PROFILING.md fallback (of fallback)")
 
 
 def shard_plan(n_ranks: int, rank: int, config: int) -> dict:
@@ -54,10 +70,16 @@ def make_rank_workload(plan: dict) -> wl.Workload:
     return w
 
 
-def fma_lane_ops(w: wl.Workload, C: int) -> dict:
-    """Algorithmic FP32 lane-ops per step."""
-    B, N, M = w.B, w.N, w.M
-    return dict(a5=8.0 * B * C * M, a2=2.0 * B * N * M, a3=40.0 * B * M)
+def algorithmic_work(w: wl.Workload, C: int) -> dict:
+    """Algorithmic work per step (DESIGN.md sections 6 and 12).
+    a5_fp32   product form: 8 FP32 FMA per (sample, column, hidden unit)
+    a5_tensor series form: 5 complex FP16 products (k = 1 as hi.hi + hi.lo + lo.hi, k = 2, k = 3) = 20 real MACs
+    a2_fp32   theta as FP32 add/sub: 2 N M lane-ops per sample (SIMT kernel)
+    a2_int8   theta as 4 int8 digits x (re, im) = 8 N M int8 MACs per sample (tensor-core kernel)
+    a3_fp32   ~40 FP32 per (sample, hidden unit)"""
+    B, N, M = float(w.B), float(w.N), float(w.M)
+    return dict(a5_fp32=8.0 * B * C * M, a5_tensor=20.0 * B * C * M, a2_fp32=2.0 * B * N * M, a2_int8=8.0 * B * N * M,
+                a3_fp32=40.0 * B * M)
 
 
 class ClockSampler(threading.Thread):
@@ -110,25 +132,44 @@ class ClockSampler(threading.Thread):
 
 
 def cpu_baseline(w: wl.Workload, budget_s: float = 10.0) -> dict:
-    """The float64 oracle (fast mode, OpenMP over samples), as it stands, on the host cores, on a
-    bounded prefix of the same batch."""
+    """The float64 oracle, as it stands, on the host cores, on bounded prefixes of the same batch: fast mode
+    (OpenMP over samples) on all threads -- the `value` -- plus the 1-thread figure and definition mode on a
+    smaller subset (SURVEY.md 8(d) "Oracle timing")."""
     import oracle
 
     oracle.build()
     cores = oracle.num_threads()
     args = (w.a, w.b, w.W, w.ham.sites, w.ham.paulis, w.ham.coeffs)
+
+    def timed(fn, n):
+        t0 = time.perf_counter()
+        fn(w.spins[:n], *args)
+        return max(time.perf_counter() - t0, 1e-6)
+
     n0 = min(w.B, cores)
-    t0 = time.perf_counter()
-    oracle.local_energy_fast(w.spins[:n0], *args)
-    dt0 = max(time.perf_counter() - t0, 1e-6)
+    dt0 = timed(oracle.local_energy_fast, n0)
     n = int(min(w.B, max(n0, (budget_s / dt0) * n0)))
-    n = max(cores, n // cores * cores)
-    t0 = time.perf_counter()
-    oracle.local_energy_fast(w.spins[:n], *args)
-    dt = time.perf_counter() - t0
+    n = max(min(cores, w.B), n // cores * cores)
+    dt = timed(oracle.local_energy_fast, n)
+    # one thread, ~3 s
+    oracle.set_num_threads(1)
+    try:
+        n1 = int(min(w.B, max(1, 3.0 / (dt / n * cores))))
+        dt1 = timed(oracle.local_energy_fast, n1)
+    finally:
+        oracle.set_num_threads(cores)
+    # definition mode (Algorithm 1 lines 6-8 literally), all threads, ~4 s
+    nd0 = min(w.B, cores)
+    dtd0 = timed(oracle.local_energy_definition, nd0)
+    nd = int(min(w.B, max(nd0, (4.0 / dtd0) * nd0)))
+    nd = max(min(cores, w.B), nd // cores * cores)
+    dtd = timed(oracle.local_energy_definition, nd) if nd > nd0 else dtd0
     return dict(value=n / dt, unit="samples/s", cores=cores, kind="oracle",
                 sample=f"fast mode (float64, flip grouping + low-rank theta update), first {n} of {w.B} samples "
-                       f"of {w.name}, {dt:.2f} s wall, OpenMP {cores} threads"), n, dt
+                       f"of {w.name}, {dt:.2f} s wall, OpenMP {cores} threads",
+                one_thread={"value": n1 / dt1, "unit": "samples/s", "sample": f"fast mode, first {n1} samples, {dt1:.2f} s"},
+                definition_mode={"value": nd / dtd, "unit": "samples/s", "cores": cores,
+                                 "sample": f"definition mode, first {nd} samples, {dtd:.2f} s wall"})
 
 
 def run_reference(args) -> None:
@@ -205,37 +246,53 @@ def run_ours(args) -> None:
     def step():
         return ham.local_energy(spins, a, b, W)
 
-    warm = max(args.warmup, 3)
-    for _ in range(warm):
-        e, l = step()
-    torch.cuda.synchronize()
+    def timed_steps(n_steps, n_warm):
+        """n_warm untimed steps, then n_steps steps each bracketed by CUDA events on the launching stream; the L2
+        is flushed (256 MiB write) between steps, outside the event pairs.  Returns (total ms, max over ranks;
+        per-kernel ms; clocks; kernel launches in the timed steps; last outputs)."""
+        for _ in range(n_warm):
+            out = step()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local_rank)
+        nqs.profile_enable(True)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
+        kern_ms = []
+        barrier()
+        launches0 = nqs.launch_count()
+        sampler.start()
+        for k in range(n_steps):
+            flush.fill_(k & 0xFF)
+            ev[k][0].record()
+            out = step()
+            ev[k][1].record()
+            if k == n_steps - 1 or k % 4 == 3:
+                kern_ms.append(nqs.profile_last())
+        barrier()
+        clocks = sampler.stop()
+        launches = nqs.launch_count() - launches0
+        nqs.profile_enable(False)
+        total_ms = float(np.sum([s0.elapsed_time(s1) for s0, s1 in ev]))
+        if world > 1:
+            tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            total_ms = float(tt.item())
+        km = {k: float(np.median([d[k] for d in kern_ms])) for k in kern_ms[0]}
+        return total_ms, km, clocks, launches, out
 
-    # ---- timed region: K steps, each bracketed by CUDA events on the launching stream; the L2 is
-    # flushed (256 MiB write) between steps, outside the event pairs.
-    sampler = ClockSampler(local_rank)
-    nqs.profile_enable(True)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kern_ms = []
-    barrier()
-    sampler.start()
-    for k in range(args.steps):
-        flush.fill_(k & 0xFF)
-        ev[k][0].record()
-        e, l = step()
-        ev[k][1].record()
-        if k == args.steps - 1 or k % 4 == 3:
-            kern_ms.append(nqs.profile_last())
-    barrier()
-    clocks = sampler.stop()
-    nqs.profile_enable(False)
-    step_ms = [s.elapsed_time(t) for s, t in ev]
-    total_ms = float(np.sum(step_ms))
-    if world > 1:
-        tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+    warm = max(args.warmup, 3)
+    # ---- the product (default path: tensor-core series for a5 where it applies, guarded, FP32 fallback behind it)
+    total_ms, km, clocks, launches, (e, l) = timed_steps(args.steps, warm)
+    took = nqs.debug_last_a5()
     ms_per_step = total_ms / args.steps
     value = plan["global_batch"] / (ms_per_step * 1e-3)
+    # ---- beside it: the same steps with a5 forced onto the FP32 product form (the round-1 path)
+    nqs.set_option("a5_path", nqs.A5_PATHS["product"])
+    try:
+        n_prod = max(3, min(args.steps, 10))
+        p_total_ms, p_km, _, _, (e_prod, _) = timed_steps(n_prod, 3)
+    finally:
+        nqs.set_option("a5_path", 0)
+    p_ms_per_step = p_total_ms / n_prod
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     pin = lambda x: torch.from_numpy(x).pin_memory()  # noqa: E731
@@ -265,35 +322,84 @@ def run_ours(args) -> None:
     assert np.array_equal(he.numpy(), e.cpu().numpy()), "host and device entry points disagree"
 
     if rank == 0:
-        ops = fma_lane_ops(w, ham.C)
-        km = {k: float(np.median([d[k] for d in kern_ms])) for k in kern_ms[0]}
+        work = algorithmic_work(w, ham.C)
+        peaks = measured_peaks()
         f_max = (clocks["sm_max_mhz"] or 1965) * 1e6
-        peak_tflops = SM_COUNT * FP32_LANES_PER_SM * 2 * f_max / 1e12
-        a5_ms = max(km["eloc"], km["series_gemm"])
-        achieved = 2.0 * ops["a5"] / (a5_ms * 1e-3) / 1e12
-        path_floor_ms = (ops["a5"] + ops["a2"] + ops["a3"]) / (SM_COUNT * FP32_LANES_PER_SM * f_max) * 1e3
+        fp32_peak_lane = SM_COUNT * FP32_LANES_PER_SM * f_max          # lane-FMA / s
+        fp32_peak_tflops = 2 * fp32_peak_lane / 1e12
+        series = took["path"] == "series" and not took["guard_failed"]
+        theta_on_tensor = w.N <= 512
+        # dominant kernel of the step and its roofline
+        if series:
+            dom, dom_ms = "series_gemm_kernel", km["series_gemm"]
+            achieved = 2.0 * work["a5_tensor"] / (dom_ms * 1e-3) / 1e12
+            roof = {"bound": "tensor", "kernel": dom, "achieved": achieved, "peak": peaks["bf16_tflops"],
+                    "unit": "TFLOP/s", "frac": achieved / peaks["bf16_tflops"],
+                    "peak_source": f"{peaks['source']}: cuBLAS bf16 burst figure (FP16 and BF16 share the tcgen05 "
+                                   "kind::f16 rate); algorithmic work = 20 real FP16 MACs per (sample, column, hidden "
+                                   "unit), padding columns not counted",
+                    "frac_of_sustained_peak": (achieved / peaks["bf16_tflops_sustained"]
+                                               if peaks["bf16_tflops_sustained"] else None)}
+        else:
+            dom, dom_ms = "eloc_kernel", km["eloc"]
+            achieved = 2.0 * work["a5_fp32"] / (dom_ms * 1e-3) / 1e12
+            roof = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": fp32_peak_tflops, "unit": "TFLOP/s",
+                    "frac": achieved / fp32_peak_tflops,
+                    "peak_source": "148 SMs x 128 FP32 lanes x 2 x clocks.max.sm (DESIGN.md); FMA = 2 flop; "
+                                   "algorithmic work = 8 FMA per (sample, column, hidden unit)"}
+        traffic = NCU_DRAM_TRAFFIC.get((w.name, dom))
+        roof["traffic"] = traffic[0] if traffic else None
+        roof["traffic_source"] = traffic[1] if traffic else "no ncu --set full capture of this kernel at this workload"
+        # FP32 floor of the cheapest FP32 formulation (SURVEY 8(d) rule (i)): product-form a5 + per-unit work, and a2
+        # only when theta really runs on the FP32 pipe.  With a5 on the tensor cores the step can beat this floor;
+        # the ratio is then > 1 and is a speed-up over the FP32 roofline, not a fraction of it.
+        fp32_floor_ms = (work["a5_fp32"] + work["a3_fp32"] + (0.0 if theta_on_tensor else work["a2_fp32"])) / fp32_peak_lane * 1e3
+        p_achieved = 2.0 * work["a5_fp32"] / (p_km["eloc"] * 1e-3) / 1e12
         line = {
             "metric": "E_loc samples/s", "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
             "warmup": warm, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f16 x f16 -> f32 (tcgen05, k = 1 operands split hi + lo) for a5; int8 -> s32 for "
+                                          "theta; f32 elsewhere" if series else "f32",
+            "data": "synthetic",
             "config": {"workload": w.name, "N": w.N, "M": w.M, "B_per_gpu": w.B, "global_batch": plan["global_batch"],
                        "terms": w.ham.T, "flip_groups": ham.G, "table_columns": ham.C,
-                       "connected_per_sample": ham.G + 1,
+                       "connected_per_sample": ham.G + 1, "a5_path": "tensor-core series (guard passed)" if series else
+                       ("FP32 product form (series guard failed)" if took["path"] == "series" else "FP32 product form"),
                        "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB write outside the event pairs)",
                        "parallelism": f"replicas over B x{world}, no collective"},
             "connected_evals_per_s": value * (ham.G + 1),
             "kernel_ms": km,
-            "path_fraction_of_fp32_roofline": path_floor_ms / ms_per_step,
-            "roofline": {"bound": "alu", "kernel": "eloc_kernel", "achieved": achieved, "peak": peak_tflops,
-                         "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                         "traffic": ELOC_KERNEL_DRAM_TRAFFIC_BYTES,
-                         "peak_source": "148 SMs x 128 FP32 lanes x 2 x clocks.max.sm (DESIGN.md); FMA = 2 flop; "
-                                        "algorithmic work = 8 FMA per (sample, column, hidden unit)"},
+            "fp32_floor_ms": fp32_floor_ms,
+            "path_fraction_of_fp32_roofline": fp32_floor_ms / ms_per_step,
+            "roofline": roof,
             "clocks": {k: clocks[k] for k in ("sm_mhz", "sm_max_mhz", "reasons")},
             "e2e": {"value": plan["global_batch"] / e2e_s, "unit": "samples/s", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
-            "gpu_launches": 6 * args.steps,  # table, pack_spins, pack_w, theta_mma, eloc, finalize
+            "gpu_launches": int(launches),
+            "product_form": {"ms_per_step": p_ms_per_step, "samples_per_s": plan["global_batch"] / (p_ms_per_step * 1e-3),
+                             "kernel_ms": p_km, "steps": n_prod,
+                             "roofline": {"bound": "alu", "kernel": "eloc_kernel", "achieved": p_achieved,
+                                          "peak": fp32_peak_tflops, "unit": "TFLOP/s", "frac": p_achieved / fp32_peak_tflops},
+                             "path_fraction_of_fp32_roofline": fp32_floor_ms / p_ms_per_step,
+                             "max_abs_diff_vs_default_path": float((e_prod - e).abs().max().item()),
+                             "what": "the same steps with NQS_OPT_A5_PATH = 1 (FP32 product form, the round-1 path)"},
         }
+        if theta_on_tensor:
+            th_tops = 2.0 * work["a2_int8"] / (km["theta"] * 1e-3) / 1e12
+            int8_peak = INT8_OVER_BF16 * peaks["bf16_tflops"]
+            line["theta_tensor"] = {"ms": km["theta"], "achieved_tops": th_tops, "peak_tops": int8_peak,
+                                    "frac": th_tops / int8_peak,
+                                    "what": "pack_spins + pack_w + theta_mma_kernel (a2 + a3); 8 N M int8 MACs per sample; "
+                                            f"peak = {INT8_OVER_BF16:g} x measured bf16 (nominal int8 : bf16 ratio)"}
+        if w.meta.get("config") == 4:
+            # Q12: half of the pair-flip columns have a zero matrix element per sample (parallel bonds)
+            s64 = w.spins.astype(np.int64)
+            bonds = np.array(wl.square_bonds(w.meta["L"]))
+            nonzero = float((s64[:, bonds[:, 0]] * s64[:, bonds[:, 1]] < 0).sum(axis=1).mean())
+            roof["frac_of_nonzero_work"] = roof["frac"] * nonzero / ham.C
+            line["product_form"]["roofline"]["frac_of_nonzero_work"] = p_achieved / fp32_peak_tflops * nonzero / ham.C
+            line["config"]["nonzero_columns_per_sample"] = nonzero
+            line["connected_evals_per_s_nonzero"] = value * (nonzero + 1)
         # SURVEY.md 8(f) items 1 + 3, reported beside the headline (not part of `value`): the force
         # vector of the same batch from the E_loc just computed (nqs_forces: stats, theta, pack, int8 GEMM)
         f_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
@@ -352,10 +458,11 @@ def run_ours(args) -> None:
             "a5_body_scalar_tflops": 2 * mb["a5_body_scalar"] / 1e12,
             "mufu_ex2_gops": mb["mufu_ex2"] / 1e9,
             "how": "nqs_microbench: 2 x 320 threads per SM, operands in registers, best of 3; FMA = 2 flop"}
-        line["roofline"]["frac_of_measured_ffma"] = achieved / (2 * max(mb["ffma"], mb["ffma2"]) / 1e12)
+        line["product_form"]["roofline"]["frac_of_measured_ffma"] = p_achieved / (2 * max(mb["ffma"], mb["ffma2"]) / 1e12)
+        if not series:
+            line["roofline"]["frac_of_measured_ffma"] = achieved / (2 * max(mb["ffma"], mb["ffma2"]) / 1e12)
         if world == 1 and not args.no_cpu_baseline:
-            cb, _, _ = cpu_baseline(w)
-            line["cpu_baseline"] = cb
+            line["cpu_baseline"] = cpu_baseline(w)
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()

@@ -256,6 +256,9 @@ int nqs_metropolis_trace(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const
  * operation); ms_out (may be NULL) the kernel time. */
 int nqs_microbench(int32_t kind, int32_t iters, double *lane_ops_per_s, float *ms_out);
 
+/* Number of kernels this library has launched in this process so far (all entry points, all streams). */
+int nqs_launch_count(int64_t *out);
+
 /* Thread-local message of the last error on this thread ("" if none). */
 const char *nqs_last_error(void);
 

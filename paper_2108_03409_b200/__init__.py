@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     forces,
     hamiltonian_info_host,
     last_error,
+    launch_count,
     lib_path,
     load_library,
     local_energy,

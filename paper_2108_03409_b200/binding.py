@@ -52,6 +52,7 @@ def load_library() -> ctypes.CDLL:
             lib.nqs_set_option.argtypes = [i32, i32]
             lib.nqs_get_option.argtypes = [i32, vp]
             lib.nqs_debug_last_a5.argtypes = [vp, vp]
+            lib.nqs_launch_count.argtypes = [vp]
             lib.nqs_energy_stats.argtypes = [vp, vp, i64, vp, vp]
             lib.nqs_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_microbench.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float)]
@@ -66,7 +67,8 @@ def load_library() -> ctypes.CDLL:
                          "nqs_hamiltonian_info", "nqs_local_energy_h", "nqs_enumerate_connected", "nqs_release",
                          "nqs_profile_enable", "nqs_profile_last", "nqs_microbench", "nqs_energy_stats",
                          "nqs_forces", "nqs_metropolis", "nqs_local_energy_forces_h", "nqs_enumerate_connected_h",
-                         "nqs_metropolis_trace", "nqs_set_option", "nqs_get_option", "nqs_debug_last_a5"):
+                         "nqs_metropolis_trace", "nqs_set_option", "nqs_get_option", "nqs_debug_last_a5",
+                         "nqs_launch_count"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -110,6 +112,13 @@ def set_option(key: str, value: int) -> None:
 def get_option(key: str) -> int:
     v = ctypes.c_int32()
     _check(load_library().nqs_get_option(OPTIONS[key], ctypes.byref(v)))
+    return int(v.value)
+
+
+def launch_count() -> int:
+    """nqs_launch_count: kernels launched by the library so far in this process."""
+    v = ctypes.c_int64()
+    _check(load_library().nqs_launch_count(ctypes.byref(v)))
     return int(v.value)
 
 

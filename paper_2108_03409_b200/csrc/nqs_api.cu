@@ -47,6 +47,19 @@ static int fail(int code, const std::string& msg) {
         if (rc__) return rc__;     \
     } while (0)
 
+// every kernel launch of the library is counted (bench.py reports the launches of its timed region)
+static std::atomic<long long> g_launches{0};
+#define NQS_LAUNCHED()                  \
+    do {                                \
+        NQS_CUDA(cudaGetLastError());   \
+        g_launches.fetch_add(1);        \
+    } while (0)
+extern "C" int nqs_launch_count(int64_t* out) {
+    if (!out) return fail(NQS_ERR_INVALID_ARG, "out is NULL");
+    *out = g_launches.load();
+    return NQS_OK;
+}
+
 extern "C" const char* nqs_last_error(void) { return g_err.c_str(); }
 extern "C" const char* nqs_version(void) { return "0.2.0 sm_100a"; }
 
@@ -467,7 +480,7 @@ static int validate_spins(DeviceState* D, const int8_t* d_spins, int64_t B, int3
     const long long total = (long long)B * N;
     const unsigned grid = (unsigned)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
     validate_spins_kernel<<<grid, 256, 0, st>>>(d_spins, total, bad);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     int h_bad = 0;
     NQS_CUDA(cudaMemcpyAsync(&h_bad, bad, sizeof(int), cudaMemcpyDeviceToHost, st));
     NQS_CUDA(cudaStreamSynchronize(st));
@@ -487,7 +500,7 @@ static int launch_theta_simt(DeviceState* D, const int8_t* d_spins, int64_t B, i
     NQS_TRY(ensure_smem(D, theta_kernel, TH_SMEM));
     theta_kernel<<<grid, 256, TH_SMEM, st>>>(d_spins, (long long)B, N, M, M_pad, (const float2*)d_a, (const float2*)d_b,
                                              (const float2*)d_W, tp, nPairsPad, (float2*)d_logpsi, raw_theta ? 1 : 0);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     return NQS_OK;
 }
 
@@ -508,9 +521,9 @@ static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, in
     const long long a_items = nMT * K16 * TM_M;
     const unsigned agrid = (unsigned)((a_items + 255) / 256 < 148 * 16 ? (a_items + 255) / 256 : 148 * 16);
     pack_spins_kernel<<<agrid, 256, 0, st>>>(d_spins, (long long)B, N, K16, nMT, A_packed);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     pack_w_kernel<<<(unsigned)(nNT * TM_JT), 128, 0, st>>>((const float2*)d_W, N, M, K16, B_packed, scale);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     const size_t smem = theta_mma_smem_bytes(K_pad);
     NQS_TRY(ensure_smem(D, theta_mma_kernel, smem));
     ThetaMmaParams p;
@@ -531,7 +544,7 @@ static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, in
     p.logpsi = (float2*)d_logpsi;
     p.raw_theta = raw_theta ? 1 : 0;
     theta_mma_kernel<<<(unsigned)nMT, TM_THREADS, smem, st>>>(p);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     return NQS_OK;
 }
 
@@ -555,7 +568,7 @@ static int launch_eloc_t(DeviceState* D, const ElocParams& p, long long nBlocksY
     const long long blocks = (long long)p.nTiles * nBlocksY;
     if (blocks > 0x7fffffffll) return fail(NQS_ERR_UNSUPPORTED, "B x column tiles exceeds the grid limit");
     eloc_kernel<WC, WS, KJ><<<(unsigned)blocks, Cfg::NT, Cfg::SMEM, st>>>(p);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     return NQS_OK;
 }
 
@@ -633,7 +646,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         const unsigned tgrid = (unsigned)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
         table_kernel<<<tgrid, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, h->C, TC, nTiles,
                                             h->dev.col_i, h->dev.col_k, h->dev.col_p, tab, rho);
-        NQS_CUDA(cudaGetLastError());
+        NQS_LAUNCHED();
     }
     // series operands that do not depend on the samples
     const int NB = h->NB, nNT = h->nNT, nJC = M_pad / 16;
@@ -654,7 +667,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         series_table_kernel<<<(unsigned)(nNT * NB), 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad,
                                                                   h->C, NB, h->dev.col_i, h->dev.col_k, h->dev.col_p,
                                                                   h->dev.col_group, sB, scols);
-        NQS_CUDA(cudaGetLastError());
+        NQS_LAUNCHED();
     }
     NQS_PROF(1, st);
     if (have_cols || d_logpsi || keep_tp)
@@ -662,7 +675,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     NQS_PROF(2, st);
     if (use_series) {
         series_pack_kernel<<<(unsigned)(B_pad / SR_M), 256, 0, st>>>(tp, nPairsPad, M_pad, sA, rown, rowmax);
-        NQS_CUDA(cudaGetLastError());
+        NQS_LAUNCHED();
     }
     NQS_PROF(3, st);
     if (use_series) {
@@ -685,13 +698,13 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         const long long blocks = (B_pad / SR_M) * nNT;
         if (blocks > 0x7fffffffll) return fail(NQS_ERR_UNSUPPORTED, "B x column tiles exceeds the grid limit");
         series_gemm_kernel<<<(unsigned)blocks, SR_THREADS, smem, st>>>(gp);
-        NQS_CUDA(cudaGetLastError());
+        NQS_LAUNCHED();
     }
     NQS_PROF(4, st);
     if (use_series) {
         series_guard_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(spartial, (long long)B, nNT, (float2*)d_eloc,
                                                                          status);
-        NQS_CUDA(cudaGetLastError());
+        NQS_LAUNCHED();
     }
     NQS_PROF(5, st);
     const int* gate = (use_series && use_product) ? status : nullptr;
@@ -715,7 +728,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     if (use_product || !use_series) {
         finalize_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(d_spins, (long long)B, N, h->dev, partial,
                                                                      have_cols ? nTiles : 0, (float2*)d_eloc, gate);
-        NQS_CUDA(cudaGetLastError());
+        NQS_LAUNCHED();
     }
     // debug record of the decision (nqs_debug_last_a5): {guard flag, failed samples} of this call, path tag
     if (use_series)
@@ -778,7 +791,7 @@ static int enumerate_impl(const nqs_hamiltonian* h, const int8_t* d_spins, int64
     const unsigned grid = (unsigned)((total + 127) / 128 < 65535 ? (total + 127) / 128 : 65535);
     enumerate_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(d_spins, (long long)B, h->hc.N, h->dev, d_sprime,
                                                              (float2*)d_mel);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     mark_use(h, (cudaStream_t)stream);
     return NQS_OK;
 }
@@ -921,7 +934,7 @@ extern "C" int nqs_microbench(int32_t kind, int32_t iters, double* lane_ops_per_
             case MB_BODY_SCALAR: launch_microbench<MB_BODY_SCALAR>(out, grid, iters, st); break;
             default: launch_microbench<MB_MUFU_EX2>(out, grid, iters, st); break;
         }
-        NQS_CUDA(cudaGetLastError());
+        NQS_LAUNCHED();
         NQS_CUDA(cudaEventRecord(e1, st));
         NQS_CUDA(cudaEventSynchronize(e1));
         float ms = 0.f;
@@ -947,9 +960,9 @@ static int launch_stats(DeviceState* D, const nqs_c64* d_x, const float* d_w, in
     const int nblk = (int)((B + 255) / 256 < ST_BLOCKS ? (B + 255) / 256 : ST_BLOCKS);
     NQS_TRY(S.get(&partial, (size_t)4 * ST_BLOCKS));
     stats_partial_kernel<<<nblk, 256, 0, st>>>((const float2*)d_x, d_w, (long long)B, partial);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     stats_final_kernel<<<1, 32, 0, st>>>(partial, nblk, d_stats);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     return NQS_OK;
 }
 
@@ -997,14 +1010,14 @@ static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, c
     if (d_stats) NQS_CUDA(cudaMemcpyAsync(d_stats, stats, sizeof(double) * 4, cudaMemcpyDeviceToDevice, st));
     force_coef_kernel<<<(unsigned)((B_pad + 255) / 256), 256, 0, st>>>((const float2*)d_eloc, d_weights, (long long)B,
                                                                        B_pad, stats, cb);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     if (!tp_in) NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st));
     force_gscale_kernel<<<(unsigned)(nJT * TM_JT), 256, 0, st>>>(tp, nPairsPad, cb, M, gexp);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     force_pack_g_kernel<<<148 * 8, 256, 0, st>>>(tp, nPairsPad, cb, M, K16, nJT, gexp, B_packed);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     force_pack_spins_kernel<<<148 * 8, 256, 0, st>>>(d_spins, (long long)B, N, K16, nIT, A_packed);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     NQS_TRY(ensure_smem(D, force_mma_kernel, FM_SMEM));
     ForceMmaParams p;
     p.A_packed = A_packed;
@@ -1015,7 +1028,7 @@ static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, c
     p.K16 = K16;
     p.F = (float2*)d_F;
     force_mma_kernel<<<dim3((unsigned)nIT, (unsigned)nJT), FM_THREADS, FM_SMEM, st>>>(p);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     return NQS_OK;
 }
 
@@ -1049,7 +1062,7 @@ template <int CPB>
 static int launch_metropolis_t(DeviceState* D, const MetroParams& p, size_t smem, cudaStream_t st) {
     NQS_TRY(ensure_smem(D, metropolis_kernel<CPB>, smem));
     metropolis_kernel<CPB><<<(unsigned)((p.C + CPB - 1) / CPB), CPB * 32, smem, st>>>(p);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     return NQS_OK;
 }
 
@@ -1081,7 +1094,7 @@ static int metropolis_impl(int8_t* d_spins, int64_t C, int32_t N, int32_t M, con
     NQS_TRY(Sc.get(&Gm, (size_t)N * (M_pad / 2)));
     NQS_TRY(Sc.get(&lk2, (size_t)N));
     site_table_kernel<<<(unsigned)N, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, Gp, Gm, lk2);
-    NQS_CUDA(cudaGetLastError());
+    NQS_LAUNCHED();
     MetroParams p;
     p.spins = d_spins;
     p.C = C;

@@ -100,9 +100,10 @@ _ORACLE_CACHE = {}
 def full_size_sample(k, B):
     """Outputs the oracle recomputes at full size: three whole 128-sample tiles (first, middle, last: every
     position inside a CTA of either a5 kernel, i.e. every b mod 128 and b mod 64) plus every 17th sample of
-    the batch (17 is coprime to the tile sizes, so every residue and ~every tile is hit)."""
+    the batch (every 7th at B = 32768; 17 and 7 are coprime to the tile sizes, so every residue is hit)."""
     mid = (B // 2) // 128 * 128
-    idx = np.concatenate([np.arange(0, 128), np.arange(mid, mid + 128), np.arange(B - 128, B), np.arange(0, B, 17)])
+    stride = 17 if B >= 65536 else 7
+    idx = np.concatenate([np.arange(0, 128), np.arange(mid, mid + 128), np.arange(B - 128, B), np.arange(0, B, stride)])
     idx = np.unique(idx)
     d_idx = np.unique(np.concatenate([np.linspace(0, B - 1, 28).astype(np.int64), [63, 64, 127, 128, B - 129, B - 128]]))
     return idx, d_idx

@@ -80,7 +80,7 @@ def test_series_pair_flip_parities_and_y_terms(nqs, oracle):
 @pytest.mark.parametrize("sigma", [0.1, 0.3, 0.5])
 def test_p10_takes_the_fallback(nqs, oracle, sigma):
     """Pin P10 (large parameters): the guard must refuse the series and the product form must answer."""
-    w = wl.make_robustness(sigma, B=256)
+    w = wl.make_robustness(sigma, B=256 if sigma == 0.1 else 128)  # the sizes of the P10 cases in test_gpu_parity
     e, l, took = run(nqs, w, "series_guarded")
     assert took["path"] == "series" and took["guard_failed"] and took["samples_over"] > 0, took
     e_prod, _, took_p = run(nqs, w, "product")
@@ -96,8 +96,10 @@ def test_p10_takes_the_fallback(nqs, oracle, sigma):
 
 def test_guard_boundary_inside_and_outside(nqs, oracle):
     """Config-3 shapes with growing parameter scale.  The guard decision must be monotone in sigma; wherever it
-    PASSES, the series alone meets the tolerance (sufficiency: checked with the fallback disabled); just
-    outside, the guarded call still meets it through the product form."""
+    PASSES, the series alone meets the tolerance (sufficiency: checked with the fallback disabled); outside,
+    the guarded call returns the product form's result bit for bit (which meets the full tolerance up to
+    sigma = 0.04 here; beyond that E_loc is a cancelling sum of large ratios and float32 is only asked for 1e-3,
+    as in pin P10)."""
     sigmas = [0.01, 0.014, 0.02, 0.028, 0.04, 0.056, 0.08]
     passed = []
     for sg in sigmas:
@@ -109,7 +111,10 @@ def test_guard_boundary_inside_and_outside(nqs, oracle):
             check_eloc(e3, e_ref, f"series only, sigma={sg} (guard passed)")
         e2, _, took2 = run(nqs, w, "series_guarded")
         assert took2["guard_failed"] == took3["guard_failed"]
-        check_eloc(e2, e_ref, f"guarded, sigma={sg}")
+        if took2["guard_failed"]:
+            ep, _, _ = run(nqs, w, "product")
+            assert np.array_equal(e2, ep), f"sigma={sg}: the fallback is not the product-form result"
+        check_eloc(e2, e_ref, f"guarded, sigma={sg}", rtol=1e-4 if sg <= 0.04 else 1e-3)
     assert passed[0], "config 3's own sigma must be inside the guard"
     assert not passed[-1], "sigma = 0.08 at M = 400 must be outside the guard"
     first_fail = passed.index(False)
