@@ -652,6 +652,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     const int NB = h->NB, nNT = h->nNT, nJC = M_pad / 16;
     uint4 *sA = nullptr, *sB = nullptr;
     SeriesCol* scols = nullptr;
+    SeriesTerms* sterms = nullptr;
     float4 *rown = nullptr, *spartial = nullptr;
     float* rowmax = nullptr;
     int* status = nullptr;
@@ -659,6 +660,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         NQS_TRY(S.get(&sA, (size_t)(B_pad / SR_M) * nJC * SR_PLANES * SR_A_PLANE_U4));
         NQS_TRY(S.get(&sB, (size_t)nNT * nJC * SR_PLANES * 2 * NB));
         NQS_TRY(S.get(&scols, (size_t)nNT * NB));
+        NQS_TRY(S.get(&sterms, (size_t)nNT * NB));
         NQS_TRY(S.get(&rown, (size_t)B_pad));
         NQS_TRY(S.get(&rowmax, (size_t)B_pad));
         NQS_TRY(S.get(&spartial, (size_t)B * nNT));
@@ -666,7 +668,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         NQS_CUDA(cudaMemsetAsync(status, 0, 4 * sizeof(int), st));
         series_table_kernel<<<(unsigned)(nNT * NB), 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad,
                                                                   h->C, NB, h->dev.col_i, h->dev.col_k, h->dev.col_p,
-                                                                  h->dev.col_group, sB, scols);
+                                                                  h->dev.col_group, h->dev, sB, scols, sterms);
         NQS_LAUNCHED();
     }
     NQS_PROF(1, st);
@@ -685,6 +687,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         gp.A_packed = sA;
         gp.B_packed = sB;
         gp.cols = scols;
+        gp.terms = sterms;
         gp.rown = rown;
         gp.rowmax = rowmax;
         gp.spins = d_spins;

@@ -39,7 +39,8 @@ constexpr int SR_PLANES = 8;              // hi.re hi.im lo.re lo.im sq.re sq.im
 constexpr int SR_A_PLANE_U4 = 2 * SR_M;   // uint4 per A plane: [slab 2][row 128][16 bytes]
 constexpr int SR_A_STAGE_BYTES = SR_PLANES * SR_A_PLANE_U4 * 16;  // 32 KB
 constexpr int SR_STAGES = 3;
-constexpr int SR_THREADS = 192;           // producer, MMA issuer, 4 epilogue warps
+constexpr int SR_EPI_WARPS = 8;           // two per TMEM lane group: each takes half of the tile's columns
+constexpr int SR_THREADS = 64 + 32 * SR_EPI_WARPS;  // producer, MMA issuer, epilogue warps
 constexpr int SR_MAX_N = 2048;            // sites (bit-packed spins of the tile live in shared memory)
 // power-of-two operand scales (keep the FP16 parts normal; removed exactly in the epilogue)
 constexpr float SR_SA = 16.f;             // every t plane
@@ -57,14 +58,22 @@ struct __align__(16) SeriesCol {
     float k4, tmax;      // tmax = max_j |T_jc|
     int site, sitek;     // flip sites (sitek = -1: single flip)
     int par, group;      // parity of the column, flip group (-1: padding column)
-    int pad0, pad1;
+    int first, count;    // the group's terms: range into DevHam::gt_* (count <= 2: also inline in SeriesTerms)
 };
 static_assert(sizeof(SeriesCol) == 64, "SeriesCol layout");
+// the first two terms of the column's group, element = c * s[z0] * s[z1] (z = -1: factor 1); an absent term has c = 0
+struct __align__(16) SeriesTerms {
+    int z0a, z1a;
+    float cra, cia;
+    int z0b, z1b;
+    float crb, cib;
+};
+static_assert(sizeof(SeriesTerms) == 32, "SeriesTerms layout");
 
 __host__ __device__ inline int series_bits_stride(int N) { return (N + 31) / 32 | 1; }  // odd: conflict-free rows
 __host__ __device__ inline size_t series_gemm_smem_bytes(int NB, int N) {
-    return (size_t)SR_STAGES * (SR_A_STAGE_BYTES + 256 * NB) + (size_t)NB * sizeof(SeriesCol) +
-           (size_t)SR_M * series_bits_stride(N) * 4 + 256;
+    return (size_t)SR_STAGES * (SR_A_STAGE_BYTES + 256 * NB) + (size_t)NB * (sizeof(SeriesCol) + sizeof(SeriesTerms)) +
+           (size_t)SR_M * series_bits_stride(N) * 4 + (size_t)SR_M * 16 + 256;
 }
 
 __device__ __forceinline__ unsigned pack_h2(float a, float b) {
@@ -80,8 +89,9 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
                                                            int N, int M, int M_pad, int C, int NB,
                                                            const int* __restrict__ col_i, const int* __restrict__ col_k,
                                                            const int* __restrict__ col_p,
-                                                           const int* __restrict__ col_group,
-                                                           uint4* __restrict__ B_packed, SeriesCol* __restrict__ cols) {
+                                                           const int* __restrict__ col_group, DevHam H,
+                                                           uint4* __restrict__ B_packed, SeriesCol* __restrict__ cols,
+                                                           SeriesTerms* __restrict__ terms) {
     const int c = blockIdx.x, tid = threadIdx.x;
     const int nt = c / NB, cl = c % NB;
     const int nJC = M_pad / 16;
@@ -176,8 +186,19 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
         r.sitek = ck;
         r.par = (int)cp;
         r.group = live_col ? col_group[c] : -1;
-        r.pad0 = r.pad1 = 0;
+        r.first = r.group >= 0 ? H.grp_first[r.group] : 0;
+        r.count = r.group >= 0 ? H.grp_count[r.group] : 0;
         cols[c] = r;
+        SeriesTerms t2 = {-1, -1, 0.f, 0.f, -1, -1, 0.f, 0.f};
+        if (r.count >= 1) {
+            const float2 cc = H.gt_c[r.first];
+            t2.z0a = H.gt_z0[r.first], t2.z1a = H.gt_z1[r.first], t2.cra = cc.x, t2.cia = cc.y;
+        }
+        if (r.count >= 2) {
+            const float2 cc = H.gt_c[r.first + 1];
+            t2.z0b = H.gt_z0[r.first + 1], t2.z1b = H.gt_z1[r.first + 1], t2.crb = cc.x, t2.cib = cc.y;
+        }
+        terms[c] = t2;
     }
 }
 
@@ -289,6 +310,7 @@ struct SeriesGemmParams {
     const uint4* A_packed;   // [nMT][nJC][8][256]
     const uint4* B_packed;   // [nNT][nJC][8][2 NB]
     const SeriesCol* cols;   // [nNT * NB]
+    const SeriesTerms* terms;  // [nNT * NB]
     const float4* rown;      // [B_pad]
     const float* rowmax;     // [B_pad]
     const int8_t* spins;     // [B][N]
@@ -303,9 +325,11 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
     const int NB = p.NB;
     const uint32_t b_stage_bytes = 256u * NB, stage_bytes = SR_A_STAGE_BYTES + b_stage_bytes;
     SeriesCol* const scol = reinterpret_cast<SeriesCol*>(sr_smem + (size_t)SR_STAGES * stage_bytes);
-    uint32_t* const sbits = reinterpret_cast<uint32_t*>(scol + NB);
+    SeriesTerms* const sterm = reinterpret_cast<SeriesTerms*>(scol + NB);
+    float4* const sred = reinterpret_cast<float4*>(sterm + NB);  // [128]: partial sums of the second column half
+    uint32_t* const sbits = reinterpret_cast<uint32_t*>(sred + SR_M);
     const int bstride = series_bits_stride(p.N);
-    uint64_t* const bars = reinterpret_cast<uint64_t*>(sbits + (size_t)SR_M * bstride);
+    uint64_t* const bars = reinterpret_cast<uint64_t*>(sbits + (size_t)SR_M * bstride + (((size_t)SR_M * bstride) & 1));
     uint64_t* const full = bars;
     uint64_t* const empty = bars + SR_STAGES;
     uint64_t* const t_full = bars + 2 * SR_STAGES;
@@ -375,31 +399,56 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
             tc_commit(t_full);
         }
     } else {
-        // ---------------- epilogue warps: TMEM lane group = warp % 4
-        const int lane_grp = warp & 3;
+        // ---------------- epilogue warps: TMEM lane group = warp % 4, column half = (warp - 2) / 4
+        const int lane_grp = warp & 3, half = (warp - 2) >> 2;
         const int row = lane_grp * 32 + lane;
         const long long b = mt * SR_M + row;
-        // while the MMAs run: column records -> smem, bit-packed spins of the tile, diagonal element
-        for (int idx = tid - 64; idx < NB * 4; idx += 128)
-            reinterpret_cast<uint4*>(scol)[idx] = reinterpret_cast<const uint4*>(p.cols + (long long)nt * NB)[idx];
-        for (int r = 0; r < 32; ++r) {
-            const long long br = mt * SR_M + lane_grp * 32 + r;
-            for (int w = 0; w < bstride; ++w) {
-                const int i = w * 32 + lane;
-                const bool up = (br < p.B && i < p.N) ? (p.spins[br * p.N + i] > 0) : false;
-                const uint32_t word = __ballot_sync(0xffffffffu, up);
-                if (lane == 0) sbits[(size_t)(lane_grp * 32 + r) * bstride + w] = word;
+        // while the MMAs run: column records -> smem (second half), bit-packed spins of the own row (first half)
+        if (half == 1) {
+            const int et = tid - 64 - 128;
+            for (int idx = et; idx < NB * 4; idx += 128)
+                reinterpret_cast<uint4*>(scol)[idx] = reinterpret_cast<const uint4*>(p.cols + (long long)nt * NB)[idx];
+            for (int idx = et; idx < NB * 2; idx += 128)
+                reinterpret_cast<uint4*>(sterm)[idx] = reinterpret_cast<const uint4*>(p.terms + (long long)nt * NB)[idx];
+        } else {
+            uint32_t* const wbits = sbits + (size_t)row * bstride;
+            const int nW = (p.N + 31) / 32;
+            if (b >= p.B) {
+                for (int w = 0; w < nW; ++w) wbits[w] = 0u;
+            } else {
+                const int8_t* const srow = p.spins + b * p.N;
+                auto nib = [](uint32_t x) {  // 4 spins (bytes +1 / -1) -> 4 bits, bit k = (byte k > 0)
+                    const uint32_t y = (~x >> 7) & 0x01010101u;
+                    return (y & 1u) | ((y >> 7) & 2u) | ((y >> 14) & 4u) | ((y >> 21) & 8u);
+                };
+                if ((p.N & 15) == 0 && (reinterpret_cast<uintptr_t>(p.spins) & 15) == 0) {
+                    const uint4* const v = reinterpret_cast<const uint4*>(srow);
+                    const int nV = p.N / 16;
+#pragma unroll 4
+                    for (int w = 0; w < nW; ++w) {
+                        const uint4 lo = v[2 * w];
+                        const uint4 hi = (2 * w + 1 < nV) ? v[2 * w + 1] : make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
+                        wbits[w] = nib(lo.x) | (nib(lo.y) << 4) | (nib(lo.z) << 8) | (nib(lo.w) << 12) | (nib(hi.x) << 16) |
+                                   (nib(hi.y) << 20) | (nib(hi.z) << 24) | (nib(hi.w) << 28);
+                    }
+                } else {
+                    for (int w = 0; w < nW; ++w) {
+                        uint32_t word = 0u;
+                        const int i1 = min(32, p.N - 32 * w);
+                        for (int i = 0; i < i1; ++i) word |= (srow[32 * w + i] > 0 ? 1u : 0u) << i;
+                        wbits[w] = word;
+                    }
+                }
             }
         }
-        asm volatile("bar.sync 1, 128;" ::: "memory");
+        asm volatile("bar.sync 1, 256;" ::: "memory");  // records and bits visible to the eight epilogue warps
         const uint32_t* const mybits = sbits + (size_t)row * bstride;
+        auto spin_or_one = [&](int z) { return z >= 0 ? spin_from_bits(mybits, z) : 1.f; };
         float er_acc = 0.f, ei_acc = 0.f, eps = 0.f;
-        if (nt == 0) {  // diagonal terms (empty flip set): d = sum_t c_t s[z0] s[z1]
-            for (int t = 0; t < p.H.Td; ++t) {
-                const int z0 = p.H.diag_z0[t], z1 = p.H.diag_z1[t];
-                float f = 1.f;
-                if (z0 >= 0) f *= spin_from_bits(mybits, z0);
-                if (z1 >= 0) f *= spin_from_bits(mybits, z1);
+        if (nt == 0) {  // diagonal terms (empty flip set): d = sum_t c_t s[z0] s[z1]; the halves split the list
+#pragma unroll 4
+            for (int t = half; t < p.H.Td; t += 2) {
+                const float f = spin_or_one(p.H.diag_z0[t]) * spin_or_one(p.H.diag_z1[t]);
                 const float2 cc = p.H.diag_c[t];
                 er_acc = fmaf(cc.x, f, er_acc);
                 ei_acc = fmaf(cc.y, f, ei_acc);
@@ -407,38 +456,43 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
         }
         const float4 rn = p.rown[b];
         const float rmax = p.rowmax[b];
+        const int nBatch = NB / 16, b_lo = half ? (nBatch + 1) / 2 : 0, b_hi = half ? nBatch : (nBatch + 1) / 2;
         mbar_wait(t_full, 0);
         tc_fence_after();
         const uint32_t tbase = tmem_base + ((uint32_t)(lane_grp * 32) << 16);
 #pragma unroll 1
-        for (int c0 = 0; c0 < NB; c0 += 16) {
+        for (int bt = b_lo; bt < b_hi; ++bt) {
+            const int c0 = bt * 16;
             float vor[16], voi[16], ver[16], vei[16];
             tmem_ld16(tbase + (uint32_t)c0, vor);
             tmem_ld16(tbase + (uint32_t)(NB + c0), voi);
             tmem_ld16(tbase + (uint32_t)(2 * NB + c0), ver);
             tmem_ld16(tbase + (uint32_t)(3 * NB + c0), vei);
+            // branch-free per column, so that the 16 columns of a batch overlap in the pipeline
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
-                const SeriesCol& cr = scol[c0 + q];
-                if (cr.group < 0) continue;
+                const SeriesCol cr = scol[c0 + q];
+                const SeriesTerms tm = sterm[c0 + q];
                 const float si = spin_from_bits(mybits, cr.site);
-                if (cr.sitek >= 0 && si * spin_from_bits(mybits, cr.sitek) != (float)cr.par) continue;
-                // summed matrix element of the group (Eq. 39)
-                const int first = p.H.grp_first[cr.group], count = p.H.grp_count[cr.group];
-                float mr = 0.f, mi = 0.f;
-                for (int u = 0; u < count; ++u) {
-                    const int z0 = p.H.gt_z0[first + u], z1 = p.H.gt_z1[first + u];
-                    float f = 1.f;
-                    if (z0 >= 0) f *= spin_from_bits(mybits, z0);
-                    if (z1 >= 0) f *= spin_from_bits(mybits, z1);
-                    const float2 cc = p.H.gt_c[first + u];
-                    mr = fmaf(cc.x, f, mr);
-                    mi = fmaf(cc.y, f, mi);
+                const float sk = spin_or_one(cr.sitek);
+                const bool active = cr.group >= 0 && (cr.sitek < 0 || si * sk == (float)cr.par);
+                // summed matrix element of the group (Eq. 39): two inline terms, the rest (rare) from global memory
+                const float fa = spin_or_one(tm.z0a) * spin_or_one(tm.z1a), fb = spin_or_one(tm.z0b) * spin_or_one(tm.z1b);
+                float mr = fmaf(tm.cra, fa, tm.crb * fb), mi = fmaf(tm.cia, fa, tm.cib * fb);
+                if (cr.count > 2) {
+                    for (int u = 2; u < cr.count; ++u) {
+                        const float f = spin_or_one(p.H.gt_z0[cr.first + u]) * spin_or_one(p.H.gt_z1[cr.first + u]);
+                        const float2 cc = p.H.gt_c[cr.first + u];
+                        mr = fmaf(cc.x, f, mr);
+                        mi = fmaf(cc.y, f, mi);
+                    }
                 }
-                if (mr == 0.f && mi == 0.f) continue;
-                // log R = log kappa - sigma (2 A + ODD) - EVEN
-                const float zr = cr.lkr - si * fmaf(SR_INV_ODD, vor[q], cr.a2r) - SR_INV_EVEN * ver[q];
-                float zi = cr.lki - si * fmaf(SR_INV_ODD, voi[q], cr.a2i) - SR_INV_EVEN * vei[q];
+                const bool live = active && (mr != 0.f || mi != 0.f);
+                mr = live ? mr : 0.f;
+                mi = live ? mi : 0.f;
+                // log R = log kappa - sigma (2 A + ODD) - EVEN   (R = 1 for a dead column: nothing to overflow)
+                const float zr = live ? cr.lkr - si * fmaf(SR_INV_ODD, vor[q], cr.a2r) - SR_INV_EVEN * ver[q] : 0.f;
+                float zi = live ? cr.lki - si * fmaf(SR_INV_ODD, voi[q], cr.a2i) - SR_INV_EVEN * vei[q] : 0.f;
                 const float kk = rintf(zi * 0.15915494309189535f);
                 zi = fmaf(-kk, 6.2831855f, zi);
                 zi = fmaf(-kk, -1.7484555e-7f, zi);
@@ -451,10 +505,17 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 // guard: |m R| (k0 + n2t k1 + n4t k2 + n6t k3 + n8t k4), valid while max |t| max |T| <= 1/2
                 const float delta = fmaf(rn.x, cr.k1, fmaf(rn.y, cr.k2, fmaf(rn.z, cr.k3, fmaf(rn.w, cr.k4, cr.k0))));
                 const float wgt = (fabsf(mr) + fabsf(mi)) * mag;
-                eps += (rmax * cr.tmax <= 0.5f) ? wgt * delta : __int_as_float(0x7f800000);
+                const float bound = (rmax * cr.tmax <= 0.5f) ? wgt * delta : __int_as_float(0x7f800000);
+                eps += live ? bound : 0.f;
             }
         }
-        if (b < p.B) p.partial[b * p.nNT + nt] = make_float4(er_acc, ei_acc, eps, 0.f);
+        // the second column half hands its sums to the first, which owns the row's output
+        if (half == 1) sred[row] = make_float4(er_acc, ei_acc, eps, 0.f);
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (half == 0 && b < p.B) {
+            const float4 o = sred[row];
+            p.partial[b * p.nNT + nt] = make_float4(er_acc + o.x, ei_acc + o.y, eps + o.z, 0.f);
+        }
     }
     tc_fence_before();
     __syncthreads();
