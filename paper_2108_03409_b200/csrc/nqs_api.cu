@@ -492,23 +492,36 @@ static int validate_spins(DeviceState* D, const int8_t* d_spins, int64_t B, int3
 // ----------------------------------------------------------------------------------------
 // a2 / a3 launches
 // ----------------------------------------------------------------------------------------
+// what one pass of the theta kernel writes
+struct ThetaOut {
+    float4* tp = nullptr;        // tanh(theta) (or theta itself with raw) as [M_pad][nPairsPad] pair records
+    nqs_c64* logpsi = nullptr;   // [B]
+    bool raw = false;
+    uint4* sA = nullptr;         // series operand planes (tensor-core kernel only), with rown / rowmax
+    float4* rown = nullptr;
+    float* rowmax = nullptr;
+    const int* gate = nullptr;   // device word: run only if (gate[0] & 1)
+};
+
 static int launch_theta_simt(DeviceState* D, const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad,
-                             const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, float4* tp,
-                             long long nPairsPad, nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta) {
-    const long long rows = tp ? nPairsPad * 2 : B;
+                             const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, long long nPairsPad,
+                             const ThetaOut& o, cudaStream_t st) {
+    const long long rows = o.tp ? nPairsPad * 2 : B;
     const unsigned grid = (unsigned)((rows + 63) / 64);
     NQS_TRY(ensure_smem(D, theta_kernel, TH_SMEM));
     theta_kernel<<<grid, 256, TH_SMEM, st>>>(d_spins, (long long)B, N, M, M_pad, (const float2*)d_a, (const float2*)d_b,
-                                             (const float2*)d_W, tp, nPairsPad, (float2*)d_logpsi, raw_theta ? 1 : 0);
+                                             (const float2*)d_W, o.tp, nPairsPad, (float2*)o.logpsi, o.raw ? 1 : 0,
+                                             o.gate);
     NQS_LAUNCHED();
     return NQS_OK;
 }
 
-// a2 on the tensor cores: pack spins and the int8 digits of W, then theta_mma_kernel (tcgen05).
+// a2 on the tensor cores: pack spins and the int8 digits of W, then theta_mma_kernel (tcgen05); all three
+// kernels honour o.gate.
 static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad,
-                            const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, float4* tp,
-                            long long nPairsPad, nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta) {
-    const long long rows = tp ? nPairsPad * 2 : B;
+                            const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, long long nPairsPad,
+                            const ThetaOut& o, cudaStream_t st) {
+    const long long rows = (o.tp || o.sA) ? nPairsPad * 2 : B;
     const long long nMT = (rows + TM_M - 1) / TM_M;
     const int K_pad = (int)round_up(N, TM_KC), K16 = K_pad / 16;
     const int nNT = (M_pad + TM_JT - 1) / TM_JT;
@@ -520,9 +533,9 @@ static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, in
     NQS_TRY(S.get(&scale, (size_t)nNT * TM_JT));
     const long long a_items = nMT * K16 * TM_M;
     const unsigned agrid = (unsigned)((a_items + 255) / 256 < 148 * 16 ? (a_items + 255) / 256 : 148 * 16);
-    pack_spins_kernel<<<agrid, 256, 0, st>>>(d_spins, (long long)B, N, K16, nMT, A_packed);
+    pack_spins_kernel<<<agrid, 256, 0, st>>>(d_spins, (long long)B, N, K16, nMT, A_packed, o.gate);
     NQS_LAUNCHED();
-    pack_w_kernel<<<(unsigned)(nNT * TM_JT), 128, 0, st>>>((const float2*)d_W, N, M, K16, B_packed, scale);
+    pack_w_kernel<<<(unsigned)(nNT * TM_JT), 128, 0, st>>>((const float2*)d_W, N, M, K16, B_packed, scale, o.gate);
     NQS_LAUNCHED();
     const size_t smem = theta_mma_smem_bytes(K_pad);
     NQS_TRY(ensure_smem(D, theta_mma_kernel, smem));
@@ -539,10 +552,14 @@ static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, in
     p.M_pad = M_pad;
     p.K16 = K16;
     p.nNT = nNT;
-    p.tp = tp;
     p.nPairsPad = nPairsPad;
-    p.logpsi = (float2*)d_logpsi;
-    p.raw_theta = raw_theta ? 1 : 0;
+    p.tp = o.tp;
+    p.logpsi = (float2*)o.logpsi;
+    p.raw_theta = o.raw ? 1 : 0;
+    p.sA = o.sA;
+    p.rown = o.rown;
+    p.rowmax = o.rowmax;
+    p.gate = o.gate;
     theta_mma_kernel<<<(unsigned)nMT, TM_THREADS, smem, st>>>(p);
     NQS_LAUNCHED();
     return NQS_OK;
@@ -554,11 +571,11 @@ static bool theta_use_mma(int32_t N) {
 }
 
 static int launch_theta(DeviceState* D, const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad,
-                        const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, float4* tp, long long nPairsPad,
-                        nqs_c64* d_logpsi, cudaStream_t st, bool raw_theta = false) {
-    if (theta_use_mma(N))
-        return launch_theta_mma(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st, raw_theta);
-    return launch_theta_simt(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st, raw_theta);
+                        const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, long long nPairsPad,
+                        const ThetaOut& o, cudaStream_t st) {
+    if (theta_use_mma(N)) return launch_theta_mma(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st);
+    if (o.sA) return fail(NQS_ERR_UNSUPPORTED, "series planes need the tensor-core theta kernel");
+    return launch_theta_simt(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st);
 }
 
 template <int WC, int WS>
@@ -592,8 +609,9 @@ extern "C" int nqs_log_psi(const int8_t* d_spins, int64_t B, int32_t N, int32_t 
     NQS_TRY(device_state(&D));
     if (B == 0) return NQS_OK;
     NQS_TRY(validate_spins(D, d_spins, B, N, (cudaStream_t)stream));
-    return launch_theta(D, d_spins, B, N, M, (int)round_up(M, KJ), d_a, d_b, d_W, nullptr, 0, d_logpsi,
-                        (cudaStream_t)stream);
+    ThetaOut o;
+    o.logpsi = d_logpsi;
+    return launch_theta(D, d_spins, B, N, M, (int)round_up(M, KJ), d_a, d_b, d_W, 0, o, (cudaStream_t)stream);
 }
 
 // ----------------------------------------------------------------------------------------
@@ -633,10 +651,13 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     const bool use_series = series_ok && (opt == 2 || opt == 3 || (opt == 0 && big));
     const bool use_product = have_cols && !(use_series && opt == 3);
 
+    // the tensor-core theta kernel writes the series planes itself; tanh(theta) is then only needed by the
+    // product form (in a gated second pass if the guard fails) or by the caller (keep_tp)
+    const bool fused_pack = use_series && theta_use_mma(N);
     Scratch S(D, st);
     float4 *tp = nullptr, *tab = nullptr, *rho = nullptr;
     float2* partial = nullptr;
-    if (have_cols || keep_tp) NQS_TRY(S.get(&tp, (size_t)M_pad * nPairsPad));
+    if (use_product || keep_tp || (use_series && !fused_pack)) NQS_TRY(S.get(&tp, (size_t)M_pad * nPairsPad));
     NQS_PROF(0, st);
     if (use_product) {
         NQS_TRY(S.get(&tab, (size_t)nTiles * M_pad * TC));
@@ -672,10 +693,18 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         NQS_LAUNCHED();
     }
     NQS_PROF(1, st);
-    if (have_cols || d_logpsi || keep_tp)
-        NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, d_logpsi, st));
+    // tanh(theta) itself: now if the caller keeps it or the product form runs unconditionally; with the fused
+    // series planes it is otherwise produced only in the gated second pass after the guard
+    const bool tp_now = keep_tp || !use_series || !fused_pack;
+    if (have_cols || d_logpsi || keep_tp) {
+        ThetaOut o;
+        o.logpsi = d_logpsi;
+        o.tp = tp_now ? tp : nullptr;
+        if (fused_pack) o.sA = sA, o.rown = rown, o.rowmax = rowmax;
+        NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
+    }
     NQS_PROF(2, st);
-    if (use_series) {
+    if (use_series && !fused_pack) {
         series_pack_kernel<<<(unsigned)(B_pad / SR_M), 256, 0, st>>>(tp, nPairsPad, M_pad, sA, rown, rowmax);
         NQS_LAUNCHED();
     }
@@ -711,6 +740,12 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     }
     NQS_PROF(5, st);
     const int* gate = (use_series && use_product) ? status : nullptr;
+    if (use_product && !tp_now) {  // fallback pass: tanh(theta) for the product form, only if the guard failed
+        ThetaOut o;
+        o.tp = tp;
+        o.gate = gate;
+        NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
+    }
     if (use_product) {
         ElocParams p;
         p.tp = tp;
@@ -1014,7 +1049,11 @@ static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, c
     force_coef_kernel<<<(unsigned)((B_pad + 255) / 256), 256, 0, st>>>((const float2*)d_eloc, d_weights, (long long)B,
                                                                        B_pad, stats, cb);
     NQS_LAUNCHED();
-    if (!tp_in) NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st));
+    if (!tp_in) {
+        ThetaOut o;
+        o.tp = tp;
+        NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
+    }
     force_gscale_kernel<<<(unsigned)(nJT * TM_JT), 256, 0, st>>>(tp, nPairsPad, cb, M, gexp);
     NQS_LAUNCHED();
     force_pack_g_kernel<<<148 * 8, 256, 0, st>>>(tp, nPairsPad, cb, M, K16, nJT, gexp, B_packed);
@@ -1113,7 +1152,10 @@ static int metropolis_impl(int8_t* d_spins, int64_t C, int32_t N, int32_t M, con
     // chunks of two sweeps; theta is recomputed from the current spins before each chunk
     const int chunk = 2 * N;
     for (int s0 = 0; s0 == 0 || s0 < S; s0 += chunk) {
-        NQS_TRY(launch_theta(D, d_spins, C, N, M, M_pad, d_a, d_b, d_W, tp, nPairsPad, nullptr, st, true));
+        ThetaOut o;
+        o.tp = tp;
+        o.raw = true;
+        NQS_TRY(launch_theta(D, d_spins, C, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
         p.S = S - s0 < chunk ? S - s0 : chunk;
         p.sites = d_sites + (long long)s0 * C;
         p.u = d_u + (long long)s0 * C;

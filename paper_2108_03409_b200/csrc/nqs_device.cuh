@@ -95,6 +95,51 @@ __device__ __forceinline__ void lncosh_tanh(float x, float y, float& lr, float& 
     ti = s * c * sech2 * inv;
 }
 
+// The same for TWO arguments at once, (x.x + i y.x) and (x.y + i y.y), on packed FFMA2 operands.  Small |z|
+// (|z|^2 < 0.36, every hidden unit of the five configurations): Taylor series in w = z^2,
+//   log cosh z = w (1/2 - w/12 + w^2/45 - ...)  (8 terms),   tanh z = z (1 - w/3 + 2 w^2/15 - ...)  (9 terms),
+// pure FMA, no cancellation: absolute error <= 3e-8 on log cosh (unbiased: 3e-7 on a sum of 1600 units against the
+// 1e-5 tolerance of log psi), relative error <= 1.2e-7 on tanh (float32 emulation over the full range, round 2).
+// Anything else (|z|^2 >= 0.36, NaN) takes lncosh_tanh above, lane by lane.
+__device__ __forceinline__ void lncosh_tanh2(float2 x, float2 y, float2& lr, float2& li, float2& tr, float2& ti) {
+    const float2 yy = __fmul2_rn(y, y);
+    const float2 wr = __ffma2_rn(x, x, neg2(yy));
+    const float2 wi = __fmul2_rn(__fadd2_rn(x, x), y);
+    const float2 nwi = neg2(wi);
+    // Horner in w with real coefficients: (pr, pi) <- (pr, pi) w + c
+    float2 pr, pi, nr;
+#define NQS_HORNER(c)                              \
+    nr = __ffma2_rn(pr, wr, bc2(c));               \
+    nr = __ffma2_rn(pi, nwi, nr);                  \
+    pi = __ffma2_rn(pi, wr, __fmul2_rn(pr, wi));   \
+    pr = nr;
+    pr = __ffma2_rn(bc2(-9.09896491907074e-05f), wr, bc2(2.565805740408915e-04f));
+    pi = __fmul2_rn(bc2(-9.09896491907074e-05f), wi);
+    NQS_HORNER(-7.386029608251831e-04f)
+    NQS_HORNER(2.1869488536155205e-03f)
+    NQS_HORNER(-6.746031746031746e-03f)
+    NQS_HORNER(2.2222222222222223e-02f)
+    NQS_HORNER(-8.333333333333333e-02f)
+    NQS_HORNER(0.5f)
+    lr = __ffma2_rn(pi, nwi, __fmul2_rn(pr, wr));
+    li = __ffma2_rn(pi, wr, __fmul2_rn(pr, wi));
+    pr = __ffma2_rn(bc2(5.90027440945586e-04f), wr, bc2(-1.4558343870513183e-03f));
+    pi = __fmul2_rn(bc2(5.90027440945586e-04f), wi);
+    NQS_HORNER(3.592128036572481e-03f)
+    NQS_HORNER(-8.863235529902197e-03f)
+    NQS_HORNER(2.1869488536155203e-02f)
+    NQS_HORNER(-5.396825396825397e-02f)
+    NQS_HORNER(0.13333333333333333f)
+    NQS_HORNER(-0.3333333333333333f)
+    NQS_HORNER(1.0f)
+#undef NQS_HORNER
+    tr = __ffma2_rn(pi, neg2(y), __fmul2_rn(pr, x));
+    ti = __ffma2_rn(pi, x, __fmul2_rn(pr, y));
+    const float m0 = fmaf(x.x, x.x, yy.x), m1 = fmaf(x.y, x.y, yy.y);
+    if (!(m0 < 0.36f)) lncosh_tanh(x.x, y.x, lr.x, li.x, tr.x, ti.x);
+    if (!(m1 < 0.36f)) lncosh_tanh(x.y, y.y, lr.y, li.y, tr.y, ti.y);
+}
+
 // ---- mbarrier / bulk-copy (TMA engine, non-tensor) helpers: PTX for sm_90+/sm_100a ----
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 

@@ -81,8 +81,10 @@ __global__ void __launch_bounds__(256) theta_kernel(const int8_t* __restrict__ s
                                                     int M_pad, const float2* __restrict__ a,
                                                     const float2* __restrict__ bvec, const float2* __restrict__ W,
                                                     float4* __restrict__ tp, long long nPairsPad,
-                                                    float2* __restrict__ logpsi, int raw_theta) {
+                                                    float2* __restrict__ logpsi, int raw_theta,
+                                                    const int* __restrict__ gate) {
     extern __shared__ __align__(16) unsigned char th_smem[];
+    if (gate && !(gate[0] & 1)) return;
     float(*sS)[64] = reinterpret_cast<float(*)[64]>(th_smem);
     float2(*sW)[64] = reinterpret_cast<float2(*)[64]>(th_smem + sizeof(float) * TH_KI * 64);
     float4(*sT)[33] = reinterpret_cast<float4(*)[33]>(th_smem + (sizeof(float) + sizeof(float2)) * TH_KI * 64);

@@ -46,6 +46,7 @@ constexpr int SR_MAX_N = 2048;            // sites (bit-packed spins of the tile
 constexpr float SR_SA = 16.f;             // every t plane
 constexpr float SR_SB1 = 64.f;            // T and T^3/3 planes  -> ODD  is scaled by 2^10
 constexpr float SR_SB2 = 2048.f;          // T^2/2 plane         -> EVEN is scaled by 2^15
+static_assert(SR_SA == TM_SERIES_SA, "theta_mma_kernel writes the t planes with this scale");
 constexpr float SR_INV_ODD = 1.f / (SR_SA * SR_SB1);
 constexpr float SR_INV_EVEN = 1.f / (SR_SA * SR_SB2);
 constexpr float SR_GUARD_FRACTION = 0.5f; // of the tolerance 1e-4 max(1, |E_loc|)

@@ -19,6 +19,8 @@
 // 2..9 = epilogue (tcgen05.ld -> theta -> log cosh, tanh -> log psi, tp).  Two CTAs per SM share
 // the 512 TMEM columns, so one CTA's MMAs overlap the other's epilogue.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "nqs_device.cuh"
 
 namespace nqs {
@@ -43,7 +45,8 @@ __host__ __device__ inline size_t theta_mma_smem_bytes(int K_pad) {
 // ---------------------------------------------------------------------------------------
 // A_packed[mtile][k16][row 0..127][16 bytes] = spins[mtile*128 + row][16*k16 .. +16), zero padded
 __global__ void pack_spins_kernel(const int8_t* __restrict__ spins, long long B, int N, int K16, long long nMT,
-                                  uint4* __restrict__ A_packed) {
+                                  uint4* __restrict__ A_packed, const int* __restrict__ gate) {
+    if (gate && !(gate[0] & 1)) return;
     const long long total = nMT * K16 * TM_M;
     const bool vec = (N % 16 == 0) && ((reinterpret_cast<uintptr_t>(spins) & 15) == 0);
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
@@ -73,7 +76,9 @@ __global__ void pack_spins_kernel(const int8_t* __restrict__ spins, long long B,
 //   Q = d0 + 128 d1 + 128^2 d2 + 128^3 d3.
 // B_packed[ntile][k16][n = 8*jl + 4*part + digit][16 bytes];  scale[j] = 2^(e-27).
 __global__ void __launch_bounds__(128) pack_w_kernel(const float2* __restrict__ W, int N, int M, int K16,
-                                                     uint4* __restrict__ B_packed, float* __restrict__ scale) {
+                                                     uint4* __restrict__ B_packed, float* __restrict__ scale,
+                                                     const int* __restrict__ gate) {
+    if (gate && !(gate[0] & 1)) return;
     const int j = blockIdx.x;
     const int tid = threadIdx.x;
     __shared__ float smax[4];
@@ -169,9 +174,28 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, int (&v)[32]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
+__device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, int (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
 // ---------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------
+// Series operands of the a5 GEMM (nqs_series.cuh), written straight from the epilogue when sA != nullptr:
+//   sA[mtile][jchunk16][plane 8][slab 2][row 128][8 halves]   planes: 16 t (hi.re hi.im lo.re lo.im), 16 t^2 (re im),
+//   16 t^3 (re im);   rown[b] = (n2t, n4t, n6t, n8t), nPt = sqrt(sum_j |t_bj|^P);   rowmax[b] = max_j |t_bj|
+constexpr float TM_SERIES_SA = 16.f;  // == SR_SA of nqs_series.cuh (static_assert there)
+
 struct ThetaMmaParams {
     const uint4* A_packed;   // [nMT][K16][128]
     const uint4* B_packed;   // [nNT][K16][256]
@@ -185,10 +209,21 @@ struct ThetaMmaParams {
     long long nPairsPad;
     float2* logpsi;          // [B] or nullptr
     int raw_theta;           // 1: tp receives theta itself instead of tanh(theta) (nqs_metropolis)
+    uint4* sA;               // series operand planes or nullptr
+    float4* rown;            // [rows] (with sA)
+    float* rowmax;           // [rows] (with sA)
+    const int* gate;         // nullptr, or: run only if (gate[0] & 1) -- the series guard failed (fallback pass)
 };
+
+__device__ __forceinline__ unsigned tm_pack_h2(float2 v) {
+    const __half2 h = __float22half2_rn(v);
+    return *reinterpret_cast<const unsigned*>(&h);
+}
+__device__ __forceinline__ float2 tm_unpack_h2(unsigned u) { return __half22float2(*reinterpret_cast<const __half2*>(&u)); }
 
 __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMmaParams p) {
     extern __shared__ __align__(128) unsigned char tm_smem[];
+    if (p.gate && !(p.gate[0] & 1)) return;
     const int K16 = p.K16;
     unsigned char* const sA = tm_smem;
     unsigned char* const sB = tm_smem + (size_t)K16 * TM_A_K16_BYTES;
@@ -199,7 +234,8 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
     uint64_t* const t_full = bars + 1 + 2 * TM_STAGES;
     uint64_t* const t_empty = bars + 2 + 2 * TM_STAGES;
     uint32_t* const tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 + 2 * TM_STAGES);
-    double* const lp_x = reinterpret_cast<double*>(sB);  // reused after the main loop: [128][2]
+    double* const lp_x = reinterpret_cast<double*>(sB);           // reused after the main loop: [128][2]
+    float* const nrm_x = reinterpret_cast<float*>(lp_x + 2 * TM_M);  // [128][5]
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long mt = blockIdx.x;
@@ -263,61 +299,102 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
             }
         }
     } else {
-        // ---------------- epilogue: 8 warps; TMEM lanes 32*(warp%4).., column half (warp-2)/4
+        // ---------------- epilogue: 8 warps; TMEM lanes 32*(warp%4).., column half (warp-2)/4 = 16 hidden units
         const int ew = warp - 2;
         const int lane_grp = warp & 3, half = ew >> 2;
         const int row = lane_grp * 32 + lane;
         const long long b = mt * TM_M + row;
         const long long pair = b >> 1;
         const bool odd = lane & 1;
+        const int nJC = p.M_pad / 16;
         double lpr = 0.0, lpi = 0.0;
+        float2 n2 = make_float2(0.f, 0.f), n4 = n2, n6 = n2, n8 = n2;  // the two halves of a unit pair accumulate apart
+        float tmx = 0.f;
         for (int nt = 0; nt < p.nNT; ++nt) {
             mbar_wait(t_full, nt & 1);
             tc_fence_after();
 #pragma unroll 1
-            for (int q4 = 0; q4 < 4; ++q4) {  // 4 hidden units per TMEM load
-                int v[32];
-                const uint32_t col = (uint32_t)(half * 128 + q4 * 32);
-                tmem_ld32(tmem_base + ((uint32_t)(lane_grp * 32) << 16) + col, v);
-                float tr[4], ti[4];
-                const int jbase = nt * TM_JT + half * 16 + q4 * 4;
+            for (int sb = 0; sb < 2; ++sb) {  // 8 hidden units per pass = one 16-byte slab of every series plane
+                int v0[32], v1[32];
+                const uint32_t col = (uint32_t)(half * 128 + sb * 64);
+                tmem_ld32_nowait(tmem_base + ((uint32_t)(lane_grp * 32) << 16) + col, v0);
+                tmem_ld32_nowait(tmem_base + ((uint32_t)(lane_grp * 32) << 16) + col + 32, v1);
+                tmem_ld_wait();
+                const int jbase = nt * TM_JT + half * 16 + sb * 8;
+                float2 tr[4], ti[4];
+                float lsr = 0.f, lsi = 0.f;
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int j = jbase + u;
-                    const bool live = j < p.M;
-                    const float sc = p.scale[j];
-                    const float2 bj = live ? p.bvec[j] : make_float2(0.f, 0.f);
-                    const int* w = &v[u * 8];
-                    const float hr = (float)(w[3] * 128 + w[2]), lr_ = (float)(w[1] * 128 + w[0]);
-                    const float hi_ = (float)(w[7] * 128 + w[6]), li_ = (float)(w[5] * 128 + w[4]);
-                    const float thr = fmaf(hr * 16384.f, sc, fmaf(lr_, sc, bj.x));
-                    const float thi = fmaf(hi_ * 16384.f, sc, fmaf(li_, sc, bj.y));
+                for (int pq = 0; pq < 4; ++pq) {  // unit pair (jbase + 2 pq, + 1)
+                    float2 thr, thi;
+                    bool live[2];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int u = 2 * pq + h;
+                        const int j = jbase + u;
+                        live[h] = j < p.M;
+                        const float sc = p.scale[j];
+                        const float2 bj = live[h] ? p.bvec[j] : make_float2(0.f, 0.f);
+                        const int* w = (u < 4) ? &v0[u * 8] : &v1[(u - 4) * 8];
+                        const float hr = (float)(w[3] * 128 + w[2]), lr_ = (float)(w[1] * 128 + w[0]);
+                        const float hi_ = (float)(w[7] * 128 + w[6]), li_ = (float)(w[5] * 128 + w[4]);
+                        const float re = fmaf(hr * 16384.f, sc, fmaf(lr_, sc, bj.x));
+                        const float im = fmaf(hi_ * 16384.f, sc, fmaf(li_, sc, bj.y));
+                        if (h == 0) thr.x = re, thi.x = im;
+                        else thr.y = re, thi.y = im;
+                    }
                     if (p.raw_theta) {
-                        tr[u] = live ? thr : 0.f;
-                        ti[u] = live ? thi : 0.f;
+                        tr[pq] = make_float2(live[0] ? thr.x : 0.f, live[1] ? thr.y : 0.f);
+                        ti[pq] = make_float2(live[0] ? thi.x : 0.f, live[1] ? thi.y : 0.f);
                         continue;
                     }
-                    float lr, li;
-                    lncosh_tanh(thr, thi, lr, li, tr[u], ti[u]);
-                    if (live) {
-                        lpr += (double)lr;
-                        lpi += (double)li;
-                    } else {
-                        tr[u] = 0.f;
-                        ti[u] = 0.f;
-                    }
+                    float2 lr, li;
+                    lncosh_tanh2(thr, thi, lr, li, tr[pq], ti[pq]);
+                    if (live[0]) lsr += lr.x, lsi += li.x;
+                    else tr[pq].x = 0.f, ti[pq].x = 0.f;
+                    if (live[1]) lsr += lr.y, lsi += li.y;
+                    else tr[pq].y = 0.f, ti[pq].y = 0.f;
                 }
+                lpr += (double)lsr;  // eight small float32 terms first, then float64 across the M / 8 groups
+                lpi += (double)lsi;
                 if (p.tp) {
 #pragma unroll
-                    for (int u = 0; u < 4; u += 2) {
-                        // even lane writes unit u (needs the odd lane's values), odd lane writes u+1
-                        const float sr = odd ? tr[u] : tr[u + 1], si = odd ? ti[u] : ti[u + 1];
+                    for (int pq = 0; pq < 4; ++pq) {
+                        // even lane writes unit 2 pq (needs the odd lane's values), odd lane writes 2 pq + 1
+                        const float sr = odd ? tr[pq].x : tr[pq].y, si = odd ? ti[pq].x : ti[pq].y;
                         const float rr = __shfl_xor_sync(0xffffffffu, sr, 1), ri = __shfl_xor_sync(0xffffffffu, si, 1);
-                        const int j = jbase + u + (odd ? 1 : 0);
-                        const float4 rec = odd ? make_float4(rr, tr[u + 1], ri, ti[u + 1])
-                                               : make_float4(tr[u], rr, ti[u], ri);
+                        const int j = jbase + 2 * pq + (odd ? 1 : 0);
+                        const float4 rec = odd ? make_float4(rr, tr[pq].y, ri, ti[pq].y)
+                                               : make_float4(tr[pq].x, rr, ti[pq].x, ri);
                         if (j < p.M_pad) p.tp[(long long)j * p.nPairsPad + pair] = rec;
                     }
+                }
+                if (p.sA && jbase < p.M_pad) {
+                    unsigned wd[8][4];
+#pragma unroll
+                    for (int pq = 0; pq < 4; ++pq) {
+                        const float2 r = tr[pq], i = ti[pq];
+                        const float2 m2 = __ffma2_rn(r, r, __fmul2_rn(i, i));
+                        const float2 m4 = __fmul2_rn(m2, m2);
+                        n2 = __fadd2_rn(n2, m2);
+                        n4 = __fadd2_rn(n4, m4);
+                        n6 = __ffma2_rn(m4, m2, n6);
+                        n8 = __ffma2_rn(m4, m4, n8);
+                        tmx = fmaxf(tmx, fmaxf(m2.x, m2.y));
+                        const float2 sr = __fmul2_rn(r, bc2(TM_SERIES_SA)), si = __fmul2_rn(i, bc2(TM_SERIES_SA));
+                        wd[0][pq] = tm_pack_h2(sr);
+                        wd[1][pq] = tm_pack_h2(si);
+                        wd[2][pq] = tm_pack_h2(__fadd2_rn(sr, neg2(tm_unpack_h2(wd[0][pq]))));
+                        wd[3][pq] = tm_pack_h2(__fadd2_rn(si, neg2(tm_unpack_h2(wd[1][pq]))));
+                        const float2 qr = __ffma2_rn(r, r, neg2(__fmul2_rn(i, i))), qi = __fmul2_rn(__fadd2_rn(r, r), i);
+                        wd[4][pq] = tm_pack_h2(__fmul2_rn(qr, bc2(TM_SERIES_SA)));
+                        wd[5][pq] = tm_pack_h2(__fmul2_rn(qi, bc2(TM_SERIES_SA)));
+                        const float2 cr = __ffma2_rn(sr, qr, neg2(__fmul2_rn(si, qi))), ci = __ffma2_rn(sr, qi, __fmul2_rn(si, qr));
+                        wd[6][pq] = tm_pack_h2(cr);
+                        wd[7][pq] = tm_pack_h2(ci);
+                    }
+                    uint4* dst = p.sA + ((mt * nJC + (jbase >> 4)) * 8) * (2 * TM_M) + ((jbase >> 3) & 1) * TM_M + row;
+#pragma unroll
+                    for (int pl = 0; pl < 8; ++pl) dst[pl * 2 * TM_M] = make_uint4(wd[pl][0], wd[pl][1], wd[pl][2], wd[pl][3]);
                 }
             }
             tc_fence_before();
@@ -325,7 +402,7 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
             if (lane == 0) mbar_arrive(t_empty);
         }
         // visible bias, split between the two column halves of a row
-        if (b < p.B) {
+        if (b < p.B && p.logpsi) {
             float ar = 0.f, ai = 0.f;
             const int i_lo = half ? p.N / 2 : 0, i_hi = half ? p.N : p.N / 2;
             for (int i = i_lo; i < i_hi; ++i) {
@@ -342,10 +419,22 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
         if (half == 1) {
             lp_x[2 * row] = lpr;
             lp_x[2 * row + 1] = lpi;
+            nrm_x[5 * row + 0] = n2.x + n2.y;
+            nrm_x[5 * row + 1] = n4.x + n4.y;
+            nrm_x[5 * row + 2] = n6.x + n6.y;
+            nrm_x[5 * row + 3] = n8.x + n8.y;
+            nrm_x[5 * row + 4] = tmx;
         }
         asm volatile("bar.sync 1, 256;" ::: "memory");
-        if (half == 0 && b < p.B && p.logpsi)
-            p.logpsi[b] = make_float2((float)(lpr + lp_x[2 * row]), (float)(lpi + lp_x[2 * row + 1]));
+        if (half == 0) {
+            if (b < p.B && p.logpsi)
+                p.logpsi[b] = make_float2((float)(lpr + lp_x[2 * row]), (float)(lpi + lp_x[2 * row + 1]));
+            if (p.sA) {
+                p.rown[b] = make_float4(sqrtf(n2.x + n2.y + nrm_x[5 * row + 0]), sqrtf(n4.x + n4.y + nrm_x[5 * row + 1]),
+                                        sqrtf(n6.x + n6.y + nrm_x[5 * row + 2]), sqrtf(n8.x + n8.y + nrm_x[5 * row + 3]));
+                p.rowmax[b] = sqrtf(fmaxf(tmx, nrm_x[5 * row + 4]));
+            }
+        }
     }
     tc_fence_before();
     __syncthreads();
