@@ -18,3 +18,4 @@ from .oracle import (  # noqa: F401
     num_threads,
     set_num_threads,
 )
+from .fisher import fisher, fisher_from_derivatives  # noqa: F401,E402

@@ -136,8 +136,10 @@ __device__ __forceinline__ void lncosh_tanh2(float2 x, float2 y, float2& lr, flo
     tr = __ffma2_rn(pi, neg2(y), __fmul2_rn(pr, x));
     ti = __ffma2_rn(pi, x, __fmul2_rn(pr, y));
     const float m0 = fmaf(x.x, x.x, yy.x), m1 = fmaf(x.y, x.y, yy.y);
-    if (!(m0 < 0.36f)) lncosh_tanh(x.x, y.x, lr.x, li.x, tr.x, ti.x);
-    if (!(m1 < 0.36f)) lncosh_tanh(x.y, y.y, lr.y, li.y, tr.y, ti.y);
+    if (!(m0 < 0.36f && m1 < 0.36f)) {  // rare: one branch for the pair
+        if (!(m0 < 0.36f)) lncosh_tanh(x.x, y.x, lr.x, li.x, tr.x, ti.x);
+        if (!(m1 < 0.36f)) lncosh_tanh(x.y, y.y, lr.y, li.y, tr.y, ti.y);
+    }
 }
 
 // ---- mbarrier / bulk-copy (TMA engine, non-tensor) helpers: PTX for sm_90+/sm_100a ----

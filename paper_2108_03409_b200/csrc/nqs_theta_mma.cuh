@@ -311,6 +311,11 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
         float2 n2 = make_float2(0.f, 0.f), n4 = n2, n6 = n2, n8 = n2;  // the two halves of a unit pair accumulate apart
         float tmx = 0.f;
         for (int nt = 0; nt < p.nNT; ++nt) {
+            // scale and bias of this warp's 16 hidden units: lane u (and u + 16) holds unit u, fetched before the
+            // accumulator wait and handed round by shuffles
+            const int jmine = nt * TM_JT + half * 16 + (lane & 15);
+            const float my_sc = p.scale[jmine];
+            const float2 my_b = jmine < p.M ? p.bvec[jmine] : make_float2(0.f, 0.f);
             mbar_wait(t_full, nt & 1);
             tc_fence_after();
 #pragma unroll 1
@@ -332,8 +337,9 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
                         const int u = 2 * pq + h;
                         const int j = jbase + u;
                         live[h] = j < p.M;
-                        const float sc = p.scale[j];
-                        const float2 bj = live[h] ? p.bvec[j] : make_float2(0.f, 0.f);
+                        const int src = sb * 8 + u;
+                        const float sc = __shfl_sync(0xffffffffu, my_sc, src);
+                        const float2 bj = make_float2(__shfl_sync(0xffffffffu, my_b.x, src), __shfl_sync(0xffffffffu, my_b.y, src));
                         const int* w = (u < 4) ? &v0[u * 8] : &v1[(u - 4) * 8];
                         const float hr = (float)(w[3] * 128 + w[2]), lr_ = (float)(w[1] * 128 + w[0]);
                         const float hi_ = (float)(w[7] * 128 + w[6]), li_ = (float)(w[5] * 128 + w[4]);
