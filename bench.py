@@ -428,6 +428,24 @@ def run_ours(args) -> None:
         line["vmc_step"] = {"ms_per_call": v_ms, "samples_per_s": w.B / (v_ms * 1e-3),
                             "what": "nqs_local_energy_forces_h: E_loc, mean/variance and force vector of one batch, "
                                     "theta and tanh(theta) computed once; median of 5, L2 flushed"}
+        # SURVEY.md 8(f) items 1 + 3: the quantum Fisher matrix S = <<O* O>>_c of the same batch (K <= 8192 parameters)
+        K = w.N + w.M + w.M * w.N
+        if K <= 8192:
+            s_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+            for k in range(7):
+                if k >= 2:
+                    flush.fill_(k)
+                    s_ev[k - 2][0].record()
+                nqs.fisher(spins, a, b, W)
+                if k >= 2:
+                    s_ev[k - 2][1].record()
+            torch.cuda.synchronize()
+            s_ms = float(np.median([s0.elapsed_time(s1) for s0, s1 in s_ev]))
+            macs = 12.0 * w.B * K * (K + 128) / 2.0  # upper-triangle tiles, 3 split products x 4 real MACs
+            line["fisher"] = {"ms_per_call": s_ms, "parameters": K, "achieved_tflops": 2.0 * macs / (s_ms * 1e-3) / 1e12,
+                              "frac_of_bf16_peak": 2.0 * macs / (s_ms * 1e-3) / 1e12 / peaks["bf16_tflops"],
+                              "what": "nqs_fisher (Eq. 10-11): theta, <O> (int8 GEMM), operand packing and the FP16 tcgen05 "
+                                      "GEMM over the samples of the upper-triangle tile pairs; median of 5, L2 flushed"}
         # one Metropolis sweep (N proposals per chain) of B chains, proposals and
         # uniforms drawn on the device beforehand (not timed), chains continue from the batch
         gen = torch.Generator(device=dev)

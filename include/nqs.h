@@ -219,6 +219,25 @@ int nqs_local_energy_forces_h(const nqs_hamiltonian *h, const int8_t *d_spins, i
                               double *d_stats, void *stream);
 
 /* ---------------------------------------------------------------------------------------
+ * Quantum Fisher matrix of the RBM (Eq. 10-11; Algorithm 1 line 9; get_global_covariance, :515):
+ *   S_{k,k'} = << O_k^* O_k' >>_c = sum_b w_b (O_k(s_b) - <O_k>)^* (O_k'(s_b) - <O_k'>) / sum_b w_b,
+ *   <O_k> = sum_b w_b O_k(s_b) / sum_b w_b,   O_k as in nqs_forces, K = N + M + M*N parameters in the order a, b, W.
+ *   d_weights [B] float32 or NULL (uniform), as in nqs_energy_stats.
+ *   d_S [K,K] complex64 out, row-major (Hermitian, both triangles written);  d_Obar [K] complex64 out or NULL: <O_k>.
+ * The contraction over the samples runs on the tensor cores: FP16 tcgen05 GEMM with FP32 accumulation of the
+ * centred derivatives split error-free into two FP16 parts (22 bits); <O_k> comes from the exact int8 contraction
+ * of nqs_forces.  Entry errors are of order 1e-6 sqrt(S_kk S_k'k') (float32 tanh, FP32 accumulation over B / 16
+ * MMA steps).  K <= 8192 (NQS_ERR_UNSUPPORTED above: S would exceed 512 MB), B <= 2^25.  Asynchronous on `stream`.
+ * nqs_vmc_step_h: nqs_local_energy_forces_h plus S and <O> of the same batch (Algorithm 1 lines 6-9 in one call),
+ * theta / tanh(theta) computed once.  d_logpsi, d_Obar and d_stats may be NULL.
+ * ------------------------------------------------------------------------------------- */
+int nqs_fisher(const int8_t *d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64 *d_a, const nqs_c64 *d_b,
+               const nqs_c64 *d_W, const float *d_weights, nqs_c64 *d_S, nqs_c64 *d_Obar, void *stream);
+int nqs_vmc_step_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t B, int32_t M, const nqs_c64 *d_a,
+                   const nqs_c64 *d_b, const nqs_c64 *d_W, const float *d_weights, nqs_c64 *d_eloc,
+                   nqs_c64 *d_logpsi, nqs_c64 *d_F, nqs_c64 *d_S, nqs_c64 *d_Obar, double *d_stats, void *stream);
+
+/* ---------------------------------------------------------------------------------------
  * Metropolis sampling of p(s) = |psi(s)|^2 / <psi|psi> with single-spin-flip
  * proposals, C independent chains advanced in lock-step (:490-494); one sweep = N steps (:341).
  *   d_spins    [C,N] int8 DEVICE in/out: the chains' states (start -> after S steps)

@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     debug_last_a5,
     enumerate_connected,
     enumerate_connected_h,
+    fisher,
     get_option,
     set_option,
     forces,

@@ -53,6 +53,8 @@ def load_library() -> ctypes.CDLL:
             lib.nqs_get_option.argtypes = [i32, vp]
             lib.nqs_debug_last_a5.argtypes = [vp, vp]
             lib.nqs_launch_count.argtypes = [vp]
+            lib.nqs_fisher.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+            lib.nqs_vmc_step_h.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_energy_stats.argtypes = [vp, vp, i64, vp, vp]
             lib.nqs_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_microbench.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float)]
@@ -68,7 +70,7 @@ def load_library() -> ctypes.CDLL:
                          "nqs_profile_enable", "nqs_profile_last", "nqs_microbench", "nqs_energy_stats",
                          "nqs_forces", "nqs_metropolis", "nqs_local_energy_forces_h", "nqs_enumerate_connected_h",
                          "nqs_metropolis_trace", "nqs_set_option", "nqs_get_option", "nqs_debug_last_a5",
-                         "nqs_launch_count"):
+                         "nqs_launch_count", "nqs_fisher", "nqs_vmc_step_h"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -254,6 +256,49 @@ class Hamiltonian:
                 ctypes.c_void_p(eloc.data_ptr()), ctypes.c_void_p(logpsi.data_ptr()), ctypes.c_void_p(F.data_ptr()),
                 ctypes.c_void_p(stats.data_ptr()), _stream()))
         return eloc, logpsi, F, stats
+
+
+    def vmc_step(self, spins, a, b, W, weights=None):
+        """nqs_vmc_step_h: (E_loc [B], log psi [B], F [K], S [K,K], <O> [K], stats [4] float64), K = N + M + M*N."""
+        import torch
+
+        B, N, M = _shapes(spins, a, b, W)
+        if N != self.N:
+            raise ValueError("N mismatch with the compiled Hamiltonian")
+        dev, K = spins.device, N + M + M * N
+        eloc = torch.empty(B, dtype=torch.complex64, device=dev)
+        logpsi = torch.empty(B, dtype=torch.complex64, device=dev)
+        F = torch.empty(K, dtype=torch.complex64, device=dev)
+        S = torch.empty((K, K), dtype=torch.complex64, device=dev)
+        Obar = torch.empty(K, dtype=torch.complex64, device=dev)
+        stats = torch.empty(4, dtype=torch.float64, device=dev)
+        with torch.cuda.device(dev):
+            _check(load_library().nqs_vmc_step_h(
+                self._h, _dev(spins, torch.int8, "spins"), B, M, _dev(a, torch.complex64, "a"),
+                _dev(b, torch.complex64, "b"), _dev(W, torch.complex64, "W"),
+                _dev(weights, torch.float32, "weights") if weights is not None else None,
+                ctypes.c_void_p(eloc.data_ptr()), ctypes.c_void_p(logpsi.data_ptr()), ctypes.c_void_p(F.data_ptr()),
+                ctypes.c_void_p(S.data_ptr()), ctypes.c_void_p(Obar.data_ptr()), ctypes.c_void_p(stats.data_ptr()),
+                _stream()))
+        return eloc, logpsi, F, S, Obar, stats
+
+
+def fisher(spins, a, b, W, weights=None):
+    """nqs_fisher: (S [K,K], <O> [K]) complex64 CUDA tensors, K = N + M + M*N in the order a, b, W."""
+    import torch
+
+    B, N, M = _shapes(spins, a, b, W)
+    K = N + M + M * N
+    if weights is not None and tuple(weights.shape) != (B,):
+        raise ValueError("weights must have shape [B]")
+    S = torch.empty((K, K), dtype=torch.complex64, device=spins.device)
+    Obar = torch.empty(K, dtype=torch.complex64, device=spins.device)
+    with torch.cuda.device(spins.device):
+        _check(load_library().nqs_fisher(
+            _dev(spins, torch.int8, "spins"), B, N, M, _dev(a, torch.complex64, "a"), _dev(b, torch.complex64, "b"),
+            _dev(W, torch.complex64, "W"), _dev(weights, torch.float32, "weights") if weights is not None else None,
+            ctypes.c_void_p(S.data_ptr()), ctypes.c_void_p(Obar.data_ptr()), _stream()))
+    return S, Obar
 
 
 def energy_stats(x, weights=None):

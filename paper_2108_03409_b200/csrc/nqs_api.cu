@@ -1,6 +1,6 @@
 // C ABI of libnqs_b200.so (declared in include/nqs.h): argument checks, workspace, launches.
 // Every step of the path runs in the kernels of nqs_kernels.cuh / nqs_series.cuh / nqs_theta_mma.cuh /
-// nqs_forces.cuh / nqs_sampler.cuh; there is no CPU fallback.
+// nqs_forces.cuh / nqs_fisher.cuh / nqs_sampler.cuh; there is no CPU fallback.
 #include <cuda_runtime.h>
 
 #include <atomic>
@@ -18,6 +18,7 @@
 #include "../../include/nqs.h"
 #include "nqs_hamiltonian.h"
 #include "nqs_kernels.cuh"
+#include "nqs_fisher.cuh"
 #include "nqs_forces.cuh"
 #include "nqs_microbench.cuh"
 #include "nqs_sampler.cuh"
@@ -1014,46 +1015,21 @@ extern "C" int nqs_energy_stats(const nqs_c64* d_x, const float* d_weights, int6
     return launch_stats(D, d_x, d_weights, B, d_stats, (cudaStream_t)stream);
 }
 
-// tp_in != NULL: tanh(theta) of this batch from local_energy_impl (owned by the caller's Scratch)
-static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
-                       const nqs_c64* d_b, const nqs_c64* d_W, const nqs_c64* d_eloc, const float* d_weights,
-                       nqs_c64* d_F, double* d_stats, void* stream, float4* tp_in) {
-    NQS_TRY(check_common(d_spins, B, N, M, d_a, d_b, d_W));
-    if (B == 0) return NQS_OK;
-    if (!d_eloc || !d_F) return fail(NQS_ERR_INVALID_ARG, "nqs_forces: NULL d_eloc / d_F");
-    if (B > (1ll << 25)) return fail(NQS_ERR_UNSUPPORTED, "nqs_forces: B > 2^25 (int32 accumulation range)");
-    DeviceState* D = nullptr;
-    NQS_TRY(device_state(&D));
-    cudaStream_t st = (cudaStream_t)stream;
-    const int M_pad = (int)round_up(M, KJ);
+// F[k] = sum_b conj(O_k(s_b)) cb[b] for all K = N + M + M N parameters: the exact int8 contraction over the
+// samples of nqs_forces.cuh.  tp = tanh(theta) pair records, cb [B_pad] (0 for the padding samples).
+// spT_out != NULL: the transposed int8 spins it packs ([nIT][K16][128] uint4) are handed to `keeper`.
+static int force_contract(DeviceState* D, const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const float4* tp,
+                          const float2* cb, nqs_c64* d_F, cudaStream_t st, uint4** spT_out, Scratch* keeper) {
     const long long B_pad = round_up(B, 256);
     const long long nPairsPad = B_pad / 2;
     const int K16 = (int)(B_pad / 16);
     const int nIT = (N + 1 + TM_M - 1) / TM_M, nJT = (M + 1 + TM_JT - 1) / TM_JT;
-
     Scratch S(D, st);
-    float4* tp = tp_in;
-    float2* cb = nullptr;
-    double* stats = nullptr;
     int* gexp = nullptr;
     uint4 *A_packed = nullptr, *B_packed = nullptr;
-    if (!tp) NQS_TRY(S.get(&tp, (size_t)M_pad * nPairsPad));
-    NQS_TRY(S.get(&cb, (size_t)B_pad));
-    NQS_TRY(S.get(&stats, 4));
     NQS_TRY(S.get(&gexp, (size_t)nJT * TM_JT));
     NQS_TRY(S.get(&A_packed, (size_t)nIT * K16 * TM_M));
     NQS_TRY(S.get(&B_packed, (size_t)nJT * K16 * TM_N));
-
-    NQS_TRY(launch_stats(D, d_eloc, d_weights, B, stats, st));
-    if (d_stats) NQS_CUDA(cudaMemcpyAsync(d_stats, stats, sizeof(double) * 4, cudaMemcpyDeviceToDevice, st));
-    force_coef_kernel<<<(unsigned)((B_pad + 255) / 256), 256, 0, st>>>((const float2*)d_eloc, d_weights, (long long)B,
-                                                                       B_pad, stats, cb);
-    NQS_LAUNCHED();
-    if (!tp_in) {
-        ThetaOut o;
-        o.tp = tp;
-        NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
-    }
     force_gscale_kernel<<<(unsigned)(nJT * TM_JT), 256, 0, st>>>(tp, nPairsPad, cb, M, gexp);
     NQS_LAUNCHED();
     force_pack_g_kernel<<<148 * 8, 256, 0, st>>>(tp, nPairsPad, cb, M, K16, nJT, gexp, B_packed);
@@ -1071,7 +1047,116 @@ static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, c
     p.F = (float2*)d_F;
     force_mma_kernel<<<dim3((unsigned)nIT, (unsigned)nJT), FM_THREADS, FM_SMEM, st>>>(p);
     NQS_LAUNCHED();
+    if (spT_out) {
+        *spT_out = A_packed;
+        S.disown(A_packed);
+        keeper->adopt(A_packed);
+    }
     return NQS_OK;
+}
+
+// tp_in != NULL: tanh(theta) of this batch from local_energy_impl (owned by the caller's Scratch)
+static int forces_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
+                       const nqs_c64* d_b, const nqs_c64* d_W, const nqs_c64* d_eloc, const float* d_weights,
+                       nqs_c64* d_F, double* d_stats, void* stream, float4* tp_in) {
+    NQS_TRY(check_common(d_spins, B, N, M, d_a, d_b, d_W));
+    if (B == 0) return NQS_OK;
+    if (!d_eloc || !d_F) return fail(NQS_ERR_INVALID_ARG, "nqs_forces: NULL d_eloc / d_F");
+    if (B > (1ll << 25)) return fail(NQS_ERR_UNSUPPORTED, "nqs_forces: B > 2^25 (int32 accumulation range)");
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M_pad = (int)round_up(M, KJ);
+    const long long B_pad = round_up(B, 256);
+    const long long nPairsPad = B_pad / 2;
+
+    Scratch S(D, st);
+    float4* tp = tp_in;
+    float2* cb = nullptr;
+    double* stats = nullptr;
+    if (!tp) NQS_TRY(S.get(&tp, (size_t)M_pad * nPairsPad));
+    NQS_TRY(S.get(&cb, (size_t)B_pad));
+    NQS_TRY(S.get(&stats, 4));
+    NQS_TRY(launch_stats(D, d_eloc, d_weights, B, stats, st));
+    if (d_stats) NQS_CUDA(cudaMemcpyAsync(d_stats, stats, sizeof(double) * 4, cudaMemcpyDeviceToDevice, st));
+    force_coef_kernel<<<(unsigned)((B_pad + 255) / 256), 256, 0, st>>>((const float2*)d_eloc, d_weights, (long long)B,
+                                                                       B_pad, stats, cb);
+    NQS_LAUNCHED();
+    if (!tp_in) {
+        ThetaOut o;
+        o.tp = tp;
+        NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
+    }
+    return force_contract(D, d_spins, B, N, M, tp, cb, d_F, st, nullptr, nullptr);
+}
+
+// S = <<O* O>>_c (nqs_fisher.cuh).  tp_in != NULL: tanh(theta) of this batch (owned by the caller's Scratch).
+static int fisher_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a, const nqs_c64* d_b,
+                       const nqs_c64* d_W, const float* d_weights, nqs_c64* d_S, nqs_c64* d_Obar, void* stream,
+                       float4* tp_in) {
+    NQS_TRY(check_common(d_spins, B, N, M, d_a, d_b, d_W));
+    if (B == 0) return NQS_OK;
+    if (!d_S) return fail(NQS_ERR_INVALID_ARG, "nqs_fisher: NULL d_S");
+    const long long K = (long long)N + M + (long long)M * N;
+    if (K > FS_MAX_K) return fail(NQS_ERR_UNSUPPORTED, "nqs_fisher: more than 8192 parameters (S would exceed 512 MB)");
+    if (B > (1ll << 25)) return fail(NQS_ERR_UNSUPPORTED, "nqs_fisher: B > 2^25");
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M_pad = (int)round_up(M, KJ);
+    const long long B_pad = round_up(B, 256);
+    const long long nPairsPad = B_pad / 2;
+    const int K16 = (int)(B_pad / 16);
+    const int nKT = (int)((K + FS_T - 1) / FS_T);
+
+    Scratch S(D, st);
+    float4* tp = tp_in;
+    float2 *cb = nullptr, *Fc = nullptr;
+    float* sw = nullptr;
+    double* stats = nullptr;
+    uint4 *spT = nullptr, *X = nullptr;
+    if (!tp) NQS_TRY(S.get(&tp, (size_t)M_pad * nPairsPad));
+    NQS_TRY(S.get(&cb, (size_t)B_pad));
+    NQS_TRY(S.get(&sw, (size_t)B_pad));
+    NQS_TRY(S.get(&stats, 4));
+    NQS_TRY(S.get(&Fc, (size_t)K));
+    NQS_TRY(S.get(&X, (size_t)nKT * K16 * FS_PLANES * FS_PLANE_U4));
+    NQS_TRY(launch_stats(D, nullptr, d_weights, B, stats, st));
+    fisher_mean_coef_kernel<<<(unsigned)((B_pad + 255) / 256), 256, 0, st>>>(d_weights, (long long)B, B_pad, stats, cb, sw);
+    NQS_LAUNCHED();
+    if (!tp_in) {
+        ThetaOut o;
+        o.tp = tp;
+        NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
+    }
+    NQS_TRY(force_contract(D, d_spins, B, N, M, tp, cb, (nqs_c64*)Fc, st, &spT, &S));
+    // power-of-two operand scale: |X| ~ |O - <O>| / sqrt(B) is brought to O(1) (exactly removed in the epilogue)
+    int e = 0;
+    (void)frexpf(sqrtf((float)B), &e);
+    float scale = ldexpf(4.f, e);
+    if (scale > 16384.f) scale = 16384.f;
+    const long long nB8 = B_pad / 8;
+    fisher_pack_kernel<<<148 * 16, 256, 0, st>>>(tp, nPairsPad, spT, K16, sw, Fc, N, M, (int)K, nKT, nB8, scale, X);
+    NQS_LAUNCHED();
+    NQS_TRY(ensure_smem(D, fisher_gemm_kernel, FS_SMEM));
+    FisherGemmParams p;
+    p.X_packed = X;
+    p.nBC = K16;
+    p.K = (int)K;
+    p.nKT = nKT;
+    p.inv_scale2 = 1.f / (scale * scale);
+    p.S = (float2*)d_S;
+    p.Obar = (float2*)d_Obar;
+    p.Fc = Fc;
+    fisher_gemm_kernel<<<(unsigned)(nKT * (nKT + 1) / 2), FS_THREADS, FS_SMEM, st>>>(p);
+    NQS_LAUNCHED();
+    return NQS_OK;
+}
+
+extern "C" int nqs_fisher(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
+                          const nqs_c64* d_b, const nqs_c64* d_W, const float* d_weights, nqs_c64* d_S,
+                          nqs_c64* d_Obar, void* stream) {
+    return fisher_impl(d_spins, B, N, M, d_a, d_b, d_W, d_weights, d_S, d_Obar, stream, nullptr);
 }
 
 extern "C" int nqs_forces(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
@@ -1095,6 +1180,26 @@ extern "C" int nqs_local_energy_forces_h(const nqs_hamiltonian* h, const int8_t*
     float4* tp = nullptr;
     NQS_TRY(local_energy_impl(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream, &tp, &keeper));
     return forces_impl(d_spins, B, h->hc.N, M, d_a, d_b, d_W, d_eloc, d_weights, d_F, d_stats, stream, tp);
+}
+
+// Algorithm 1 lines 6-9 in one call: E_loc, statistics, force vector F and Fisher matrix S of one batch.
+extern "C" int nqs_vmc_step_h(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int32_t M, const nqs_c64* d_a,
+                              const nqs_c64* d_b, const nqs_c64* d_W, const float* d_weights, nqs_c64* d_eloc,
+                              nqs_c64* d_logpsi, nqs_c64* d_F, nqs_c64* d_S, nqs_c64* d_Obar, double* d_stats,
+                              void* stream) {
+    if (B < 0) return fail(NQS_ERR_INVALID_ARG, "nqs_vmc_step_h: B < 0");
+    if (B == 0) return NQS_OK;
+    if (!d_F || !d_S) return fail(NQS_ERR_INVALID_ARG, "nqs_vmc_step_h: NULL d_F / d_S");
+    if (!h) return fail(NQS_ERR_INVALID_ARG, "hamiltonian handle is NULL");
+    const long long K = (long long)h->hc.N + M + (long long)M * h->hc.N;
+    if (K > FS_MAX_K) return fail(NQS_ERR_UNSUPPORTED, "nqs_vmc_step_h: more than 8192 parameters");
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
+    Scratch keeper(D, (cudaStream_t)stream);
+    float4* tp = nullptr;
+    NQS_TRY(local_energy_impl(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream, &tp, &keeper));
+    NQS_TRY(forces_impl(d_spins, B, h->hc.N, M, d_a, d_b, d_W, d_eloc, d_weights, d_F, d_stats, stream, tp));
+    return fisher_impl(d_spins, B, h->hc.N, M, d_a, d_b, d_W, d_weights, d_S, d_Obar, stream, tp);
 }
 
 // ----------------------------------------------------------------------------------------

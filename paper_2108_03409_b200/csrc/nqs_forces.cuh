@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(256) stats_partial_kernel(const float2* __rest
     __shared__ double sh[4][256];
     double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
     for (long long b = blockIdx.x * 256ll + threadIdx.x; b < B; b += (long long)gridDim.x * 256) {
-        const float2 e = x[b];
+        const float2 e = x ? x[b] : make_float2(0.f, 0.f);  // x == nullptr: only the sum of the weights
         const double wb = w ? (double)w[b] : 1.0, er = e.x, ei = e.y;
         s0 += wb;
         s1 += wb * er;
