@@ -10,9 +10,11 @@
  *   log psi(s) = sum_i a_i s_i + sum_j log cosh(b_j + sum_i W_ji s_i)      Eq. 38, :385-390
  *                (index reading Q1 of DESIGN.md: j hidden, i visible, W is [M,N])
  *   E_loc(s)   = sum_s' <s|H|s'> psi(s') / psi(s)                           Eq. 4,  :63-68, :89
- *   H          = sum_t c_t P_t,  P_t a product of at most two Pauli matrices on distinct
- *                sites; its action on a basis configuration is the map of      Eq. 39, :418-426
- *                s -> (s', <s|P_t|s'>) ("branch-free": one non-zero per row, :473).
+ *   H          = sum_t c_t P_t,  P_t a product of Pauli matrices on distinct sites (a "Pauli
+ *                string": K slots per term, K = 2 for the five configurations, any K for the
+ *                k-site strings of SURVEY.md 8(f) item 4 / PAPER.md:473 "tensor products of
+ *                branch-free operators"); its action on a basis configuration is the map of
+ *                s -> (s', <s|P_t|s'>) ("branch-free": one non-zero per row).   Eq. 39, :418-426
  *
  * Inputs are the SAME BYTES the GPU gets (int8 spins, complex64 parameters); they are
  * promoted exactly to double.  All arithmetic is double / double complex.
@@ -129,9 +131,9 @@ static inline cplx pauli_factor(int p, int sk, int *flips) {
  * definition mode: Eq. 4 + Eq. 39 + Eq. 38, term by term (Algorithm 1 lines 6-8)
  * ------------------------------------------------------------------------------------- */
 void oracle_local_energy_definition(const int8_t *spins, int64_t B, int N, int M, const float *a,
-                                    const float *b, const float *W, int T, const int32_t *sites,
+                                    const float *b, const float *W, int T, int K, const int32_t *sites,
                                     const uint8_t *paulis, const float *coeffs, double *out_eloc,
-                                    double *out_logpsi) {
+                                    double *out_logpsi) { /* sites, paulis: [T,K] */
 #pragma omp parallel
     {
         int8_t *sp = (int8_t *)malloc((size_t)N);
@@ -143,11 +145,11 @@ void oracle_local_energy_definition(const int8_t *spins, int64_t B, int N, int M
             for (int t = 0; t < T; ++t) {
                 cplx m = c64(coeffs, t);
                 memcpy(sp, s, (size_t)N);
-                for (int k = 0; k < 2; ++k) {
-                    int site = sites[2 * t + k];
+                for (int k = 0; k < K; ++k) {
+                    int site = sites[(int64_t)K * t + k];
                     if (site < 0) continue; /* unused slot */
                     int flips = 0;
-                    m *= pauli_factor(paulis[2 * t + k], s[site], &flips);
+                    m *= pauli_factor(paulis[(int64_t)K * t + k], s[site], &flips);
                     if (flips) sp[site] = (int8_t)(-sp[site]);
                 }
                 if (m == 0.0) continue; /* "non-zero matrix elements", :458 (reading Q5) */
@@ -168,25 +170,26 @@ void oracle_local_energy_definition(const int8_t *spins, int64_t B, int N, int M
 /* ---------------------------------------------------------------------------------------
  * fast mode: flip grouping + low-rank theta update, same float64 arithmetic
  * ------------------------------------------------------------------------------------- */
-typedef struct { int f0, f1; int first, count; } group_t; /* flip set {f0,f1}, f1=-1 if single, f0=-1 diag */
+#define ORACLE_MAX_SLOTS 16
+typedef struct { int nf; int f[ORACLE_MAX_SLOTS]; int first, count; } group_t; /* sorted flip set; nf = 0: diagonal */
 
-static int key_of(const int32_t *sites, const uint8_t *paulis, int t, int *f0, int *f1) {
-    int f[2], nf = 0;
-    for (int k = 0; k < 2; ++k) {
-        int site = sites[2 * t + k];
-        int p = paulis[2 * t + k];
+/* the flip set of term t: the sites carrying X or Y, sorted */
+static int key_of(const int32_t *sites, const uint8_t *paulis, int K, int t, int *f) {
+    int nf = 0;
+    for (int k = 0; k < K; ++k) {
+        int site = sites[(int64_t)K * t + k];
+        int p = paulis[(int64_t)K * t + k];
         if (site >= 0 && (p == P_X || p == P_Y)) f[nf++] = site;
     }
-    if (nf == 2 && f[0] > f[1]) { int tmp = f[0]; f[0] = f[1]; f[1] = tmp; }
-    *f0 = nf > 0 ? f[0] : -1;
-    *f1 = nf > 1 ? f[1] : -1;
+    for (int i = 1; i < nf; ++i) /* insertion sort */
+        for (int j = i; j > 0 && f[j - 1] > f[j]; --j) { int tmp = f[j]; f[j] = f[j - 1]; f[j - 1] = tmp; }
     return nf;
 }
 
 void oracle_local_energy_fast(const int8_t *spins, int64_t B, int N, int M, const float *a,
-                              const float *b, const float *W, int T, const int32_t *sites,
+                              const float *b, const float *W, int T, int K, const int32_t *sites,
                               const uint8_t *paulis, const float *coeffs, double *out_eloc,
-                              double *out_logpsi) {
+                              double *out_logpsi) { /* sites, paulis: [T,K], K <= ORACLE_MAX_SLOTS */
     /* group terms by flip set: order[] lists term ids group by group (O(T^2), T is small) */
     int *order = (int *)malloc(sizeof(int) * (size_t)(T > 0 ? T : 1));
     group_t *groups = (group_t *)malloc(sizeof(group_t) * (size_t)(T > 0 ? T : 1));
@@ -194,14 +197,15 @@ void oracle_local_energy_fast(const int8_t *spins, int64_t B, int N, int M, cons
     int G = 0, pos = 0;
     for (int t = 0; t < T; ++t) {
         if (done[t]) continue;
-        int f0, f1;
-        key_of(sites, paulis, t, &f0, &f1);
-        groups[G].f0 = f0; groups[G].f1 = f1; groups[G].first = pos; groups[G].count = 0;
+        groups[G].nf = key_of(sites, paulis, K, t, groups[G].f);
+        groups[G].first = pos; groups[G].count = 0;
         for (int u = t; u < T; ++u) {
-            int g0, g1;
+            int g[ORACLE_MAX_SLOTS];
             if (done[u]) continue;
-            key_of(sites, paulis, u, &g0, &g1);
-            if (g0 == f0 && g1 == f1) { order[pos++] = u; done[u] = 1; groups[G].count++; }
+            int ng = key_of(sites, paulis, K, u, g);
+            if (ng == groups[G].nf && memcmp(g, groups[G].f, sizeof(int) * (size_t)ng) == 0) {
+                order[pos++] = u; done[u] = 1; groups[G].count++;
+            }
         }
         ++G;
     }
@@ -229,22 +233,27 @@ void oracle_local_energy_fast(const int8_t *spins, int64_t B, int N, int M, cons
                 for (int q = 0; q < groups[g].count; ++q) {
                     int t = order[groups[g].first + q];
                     cplx mt = c64(coeffs, t);
-                    for (int k = 0; k < 2; ++k) {
-                        int site = sites[2 * t + k];
+                    for (int k = 0; k < K; ++k) {
+                        int site = sites[(int64_t)K * t + k];
                         if (site < 0) continue;
                         int flips;
-                        mt *= pauli_factor(paulis[2 * t + k], s[site], &flips);
+                        mt *= pauli_factor(paulis[(int64_t)K * t + k], s[site], &flips);
                     }
                     m += mt;
                 }
-                if (groups[g].f0 < 0) { E += m; continue; } /* diagonal: s' = s, ratio 1 */
+                if (groups[g].nf == 0) { E += m; continue; } /* diagonal: s' = s, ratio 1 */
                 if (m == 0.0) continue;
-                int f0 = groups[g].f0, f1 = groups[g].f1;
-                cplx dlog = -2.0 * c64(a, f0) * (double)s[f0];
-                if (f1 >= 0) dlog += -2.0 * c64(a, f1) * (double)s[f1];
+                cplx dlog = 0.0;
+                for (int q = 0; q < groups[g].nf; ++q) {
+                    int f = groups[g].f[q];
+                    dlog += -2.0 * c64(a, f) * (double)s[f];
+                }
                 for (int j = 0; j < M; ++j) {
-                    cplx thp = theta[j] - 2.0 * c64(W, (int64_t)j * N + f0) * (double)s[f0];
-                    if (f1 >= 0) thp -= 2.0 * c64(W, (int64_t)j * N + f1) * (double)s[f1];
+                    cplx thp = theta[j];
+                    for (int q = 0; q < groups[g].nf; ++q) {
+                        int f = groups[g].f[q];
+                        thp -= 2.0 * c64(W, (int64_t)j * N + f) * (double)s[f];
+                    }
                     dlog += lncosh_stable(thp) - L[j];
                 }
                 E += m * cexp(dlog);
@@ -268,7 +277,7 @@ void oracle_local_energy_fast(const int8_t *spins, int64_t B, int N, int M, cons
  * Eq. 39 as data: connected configurations and matrix elements, term by term (no grouping).
  * sprime [B,T,N] int8, mel [B,T] complex128.  Used to check the GPU enumerator.
  * ------------------------------------------------------------------------------------- */
-void oracle_connected(const int8_t *spins, int64_t B, int N, int T, const int32_t *sites,
+void oracle_connected(const int8_t *spins, int64_t B, int N, int T, int K, const int32_t *sites,
                       const uint8_t *paulis, const float *coeffs, int8_t *sprime, double *mel) {
     for (int64_t n = 0; n < B; ++n) {
         const int8_t *s = spins + n * N;
@@ -276,11 +285,11 @@ void oracle_connected(const int8_t *spins, int64_t B, int N, int T, const int32_
             int8_t *sp = sprime + ((n * T) + t) * N;
             memcpy(sp, s, (size_t)N);
             cplx m = c64(coeffs, t);
-            for (int k = 0; k < 2; ++k) {
-                int site = sites[2 * t + k];
+            for (int k = 0; k < K; ++k) {
+                int site = sites[(int64_t)K * t + k];
                 if (site < 0) continue;
                 int flips = 0;
-                m *= pauli_factor(paulis[2 * t + k], s[site], &flips);
+                m *= pauli_factor(paulis[(int64_t)K * t + k], s[site], &flips);
                 if (flips) sp[site] = (int8_t)(-sp[site]);
             }
             mel[2 * (n * T + t)] = creal(m);

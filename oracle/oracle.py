@@ -43,9 +43,9 @@ def _load():
         lib.oracle_log_psi.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp]
         lib.oracle_log_psi.restype = None
         for fn in (lib.oracle_local_energy_definition, lib.oracle_local_energy_fast):
-            fn.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp]
+            fn.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp]
             fn.restype = None
-        lib.oracle_connected.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp]
+        lib.oracle_connected.argtypes = [vp, i64, i32, i32, i32, vp, vp, vp, vp, vp]
         lib.oracle_connected.restype = None
         lib.oracle_mean_variance.argtypes = [vp, vp, i64, vp]
         lib.oracle_mean_variance.restype = None
@@ -80,10 +80,13 @@ def _params(spins, a, b, W):
 
 
 def _terms(sites, paulis, coeffs):
+    """Term arrays [T,K]: K slots per term (K = 2 for the five configurations; k-site Pauli strings use more)."""
     sites, paulis, coeffs = _c(sites, np.int32), _c(paulis, np.uint8), _c(coeffs, np.complex64)
     T = coeffs.shape[0]
-    assert sites.shape == (T, 2) and paulis.shape == (T, 2)
-    return sites, paulis, coeffs, T
+    K = sites.shape[1] if sites.ndim == 2 else 2
+    sites, paulis = sites.reshape(T, K), paulis.reshape(T, K)
+    assert 1 <= K <= 16
+    return sites, paulis, coeffs, T, K
 
 
 def num_threads() -> int:
@@ -112,10 +115,10 @@ def log_psi(spins, a, b, W, stable: bool = False) -> np.ndarray:
 
 def _eloc(fn, spins, a, b, W, sites, paulis, coeffs):
     spins, a, b, W, B, N, M = _params(spins, a, b, W)
-    sites, paulis, coeffs, T = _terms(sites, paulis, coeffs)
+    sites, paulis, coeffs, T, K = _terms(sites, paulis, coeffs)
     eloc = np.empty(B, dtype=np.complex128)
     logpsi = np.empty(B, dtype=np.complex128)
-    fn(_p(spins), B, N, M, _p(a), _p(b), _p(W), T, _p(sites), _p(paulis), _p(coeffs), _p(eloc), _p(logpsi))
+    fn(_p(spins), B, N, M, _p(a), _p(b), _p(W), T, K, _p(sites), _p(paulis), _p(coeffs), _p(eloc), _p(logpsi))
     return eloc, logpsi
 
 
@@ -133,10 +136,10 @@ def connected(spins, sites, paulis, coeffs):
     """Eq. 39 as data, term by term: s' int8 [B,T,N] and matrix elements complex128 [B,T]."""
     spins = _c(spins, np.int8)
     B, N = spins.shape
-    sites, paulis, coeffs, T = _terms(sites, paulis, coeffs)
+    sites, paulis, coeffs, T, K = _terms(sites, paulis, coeffs)
     sp = np.empty((B, T, N), dtype=np.int8)
     mel = np.empty((B, T), dtype=np.complex128)
-    _load().oracle_connected(_p(spins), B, N, T, _p(sites), _p(paulis), _p(coeffs), _p(sp), _p(mel))
+    _load().oracle_connected(_p(spins), B, N, T, K, _p(sites), _p(paulis), _p(coeffs), _p(sp), _p(mel))
     return sp, mel
 
 

@@ -23,9 +23,9 @@ def dense_hamiltonian(N: int, sites, paulis, coeffs) -> np.ndarray:
     assert N <= 12
     dim = 1 << N
     H = np.zeros((dim, dim), dtype=np.complex128)
-    for (s0, s1), (p0, p1), c in zip(np.asarray(sites), np.asarray(paulis), np.asarray(coeffs)):
+    for srow, prow, c in zip(np.asarray(sites), np.asarray(paulis), np.asarray(coeffs)):  # [T,K]: K slots per term
         factors = [PAULI[0]] * N
-        for site, p in ((int(s0), int(p0)), (int(s1), int(p1))):
+        for site, p in zip((int(v) for v in srow), (int(v) for v in prow)):
             if site >= 0:
                 assert factors[site] is PAULI[0], "two operators on one site"
                 factors[site] = PAULI[p]

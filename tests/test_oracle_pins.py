@@ -53,6 +53,47 @@ def test_p1_bruteforce_random_terms(oracle, N, M, T, sigma, seed):
         _assert_logpsi(lp, psi, 1e-11, f"log psi {fn.__name__}")
 
 
+@pytest.mark.parametrize("N,M,T,K,sigma,seed", [(5, 4, 30, 3, 0.3, 15), (7, 6, 40, 4, 0.25, 16), (8, 5, 50, 6, 0.2, 17),
+                                                 (9, 7, 25, 8, 0.15, 18)])
+def test_p1_bruteforce_k_site_pauli_strings(oracle, N, M, T, K, sigma, seed):
+    """k-site Pauli strings ("tensor products of branch-free operators"): term
+    arrays [T,K] with up to K operators per term, up to four of them flipping, against the dense Kronecker-product H
+    (which knows no flip / sign rule).  Several Y factors in one string pin the (-i)^n phase; strings with the same
+    flip set pin the grouping of fast mode."""
+    w = wl.make_random(N, M, 1 << N, 4, sigma, seed)
+    ham = wl.random_strings(N, T, K, np.random.default_rng([seed, 3]))
+    assert ham.sites.shape == (T, K)
+    e_ref, psi, H = local_energy_all(N, w.a, w.b, w.W, ham.sites, ham.paulis, ham.coeffs)
+    assert np.abs(H).max() > 0
+    for fn in (oracle.local_energy_definition, oracle.local_energy_fast):
+        e, lp = fn(w.spins, w.a, w.b, w.W, ham.sites, ham.paulis, ham.coeffs)
+        _assert_close(e, e_ref, 1e-10, f"E_loc {fn.__name__} K={K}")
+        _assert_logpsi(lp, psi, 1e-11, f"log psi {fn.__name__} K={K}")
+    # Eq. 39 as data: every term's (s', element) is an entry of the dense matrix row
+    sp, mel = oracle.connected(w.spins[:8], ham.sites, ham.paulis, ham.coeffs)
+    states = all_states(N)
+    index = {tuple(row): k for k, row in enumerate(states)}
+    for bidx in range(8):
+        row = np.zeros(1 << N, np.complex128)
+        for t in range(T):
+            row[index[tuple(sp[bidx, t].astype(np.float64))]] += mel[bidx, t]
+        assert np.allclose(row, H[index[tuple(w.spins[bidx].astype(np.float64))]], atol=1e-12)
+
+
+def test_p1_three_and_four_site_strings_by_hand(oracle):
+    """XXX, YYY, XYZ, ZZZZ and XZZX on a 5-site chain with fixed coefficients: a term list a reader can check."""
+    N, M = 5, 3
+    w = wl.make_random(N, M, 1 << N, 1, 0.3, 19)
+    X, Y, Z = 1, 2, 3
+    sites = np.array([[0, 1, 2, -1], [1, 2, 3, -1], [0, 2, 4, -1], [0, 1, 2, 3], [1, 2, 3, 4]], np.int32)
+    paulis = np.array([[X, X, X, 0], [Y, Y, Y, 0], [X, Y, Z, 0], [Z, Z, Z, Z], [X, Z, Z, X]], np.uint8)
+    coeffs = np.array([0.5, -0.25 + 0.5j, 1.5, -1.0, 0.75j], np.complex64)
+    e_ref, _, _ = local_energy_all(N, w.a, w.b, w.W, sites, paulis, coeffs)
+    for fn in (oracle.local_energy_definition, oracle.local_energy_fast):
+        e, _ = fn(w.spins, w.a, w.b, w.W, sites, paulis, coeffs)
+        _assert_close(e, e_ref, 1e-11, fn.__name__)
+
+
 @pytest.mark.parametrize("pauli", [1, 2, 3])
 def test_p1_single_pauli_terms(oracle, pauli):
     """One single-site Pauli with a complex coefficient: a column-convention or sigma^y sign

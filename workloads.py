@@ -134,6 +134,33 @@ def random_terms(N: int, T: int, rng: np.random.Generator, allow_identity: bool 
     return ham
 
 
+def random_strings(N: int, T: int, K: int, rng: np.random.Generator, max_flips: int = 4) -> Hamiltonian:
+    """Random Pauli strings on up to K distinct sites (term arrays [T,K]):
+    every Pauli type, complex coefficients, at most `max_flips` X/Y factors per string (the flip set), unused
+    slots (-1) anywhere in the row."""
+    sites = np.full((T, K), -1, dtype=np.int32)
+    paulis = np.zeros((T, K), dtype=np.uint8)
+    coeffs = np.zeros((T,), dtype=np.complex64)
+    for t in range(T):
+        m = int(rng.integers(0, min(K, N) + 1))  # number of sites the string acts on (0: constant term)
+        where = rng.choice(K, size=m, replace=False)
+        which = rng.choice(N, size=m, replace=False)
+        flips = 0
+        for slot, site in zip(where, which):
+            p = int(rng.integers(0, 4))
+            if p in (PAULI_X, PAULI_Y):
+                if flips == max_flips:
+                    p = PAULI_Z
+                else:
+                    flips += 1
+            sites[t, slot] = site
+            paulis[t, slot] = p
+        coeffs[t] = complex(rng.standard_normal(), rng.standard_normal())
+    ham = Hamiltonian(sites, paulis, coeffs)
+    ham.name = f"strings({T},K={K})"
+    return ham
+
+
 # ----------------------------------------------------------------------------------------
 # parameters and spins
 # ----------------------------------------------------------------------------------------
