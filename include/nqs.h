@@ -9,7 +9,7 @@
  *
  *   E_loc(s)   = sum_s' <s|H|s'> psi(s') / psi(s)                            Eq. 4, :63-68, :89
  *       for H = sum_t c_t P_t with P_t a product of at most two Pauli matrices on distinct
- *       sites ("branch-free" operators, :473); the connected configurations s' and matrix
+ *       sites ("branch-free" operators, :473; up to eight with the *_k entry points); the connected configurations s' and matrix
  *       elements <s|P_t|s'> are generated on the fly on the device (Eq. 39, :418-426;
  *       Algorithm 1 lines 6-8, :163-194; the four-call sequence at :464-469).
  *
@@ -114,6 +114,22 @@ int nqs_log_psi_host(const int8_t *h_spins, int64_t B, int32_t N, int32_t M, con
 int nqs_hamiltonian_create(int32_t N, int32_t T, const int32_t *h_sites, const uint8_t *h_paulis,
                            const nqs_c64 *h_coeffs, nqs_hamiltonian **out);
 int nqs_hamiltonian_destroy(nqs_hamiltonian *h);
+
+/* k-site Pauli strings ("tensor products of branch-free operators"): the same
+ * with K slots per term -- h_sites [T,K] int32 (-1 = unused slot), h_paulis [T,K] uint8 -- 1 <= K <= 8, all sites of
+ * a term distinct.  A term may carry any number of Z / I factors and at most FOUR X / Y factors (a flip set of m
+ * sites costs 2^(m-1) table columns, one per pattern of relative signs; NQS_ERR_UNSUPPORTED beyond four).  Handles
+ * made this way work with every *_h entry point; nqs_hamiltonian_info_k reports the flip sets as [G,4] (-1 padded).
+ * nqs_local_energy_k is nqs_local_energy for such a term list. */
+int nqs_hamiltonian_create_k(int32_t N, int32_t T, int32_t K, const int32_t *h_sites, const uint8_t *h_paulis,
+                             const nqs_c64 *h_coeffs, nqs_hamiltonian **out);
+int nqs_hamiltonian_compile_host_k(int32_t N, int32_t T, int32_t K, const int32_t *h_sites, const uint8_t *h_paulis,
+                                   const nqs_c64 *h_coeffs, nqs_hamiltonian **out);
+int nqs_hamiltonian_info_k(const nqs_hamiltonian *h, int32_t info[5], int32_t *flip_sites4);
+int nqs_local_energy_k(const int8_t *d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64 *d_a,
+                       const nqs_c64 *d_b, const nqs_c64 *d_W, int32_t T, int32_t K, const int32_t *h_sites,
+                       const uint8_t *h_paulis, const nqs_c64 *h_coeffs, nqs_c64 *d_eloc, nqs_c64 *d_logpsi,
+                       void *stream);
 
 /* Host-side description of the compiled form (no device work; usable without a GPU when the
  * handle was made with nqs_hamiltonian_compile_host):

@@ -53,6 +53,10 @@ def load_library() -> ctypes.CDLL:
             lib.nqs_get_option.argtypes = [i32, vp]
             lib.nqs_debug_last_a5.argtypes = [vp, vp]
             lib.nqs_launch_count.argtypes = [vp]
+            lib.nqs_hamiltonian_create_k.argtypes = [i32, i32, i32, vp, vp, vp, ctypes.POINTER(vp)]
+            lib.nqs_hamiltonian_compile_host_k.argtypes = [i32, i32, i32, vp, vp, vp, ctypes.POINTER(vp)]
+            lib.nqs_hamiltonian_info_k.argtypes = [vp, vp, vp]
+            lib.nqs_local_energy_k.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp, vp]
             lib.nqs_fisher.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_vmc_step_h.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_energy_stats.argtypes = [vp, vp, i64, vp, vp]
@@ -70,7 +74,8 @@ def load_library() -> ctypes.CDLL:
                          "nqs_profile_enable", "nqs_profile_last", "nqs_microbench", "nqs_energy_stats",
                          "nqs_forces", "nqs_metropolis", "nqs_local_energy_forces_h", "nqs_enumerate_connected_h",
                          "nqs_metropolis_trace", "nqs_set_option", "nqs_get_option", "nqs_debug_last_a5",
-                         "nqs_launch_count", "nqs_fisher", "nqs_vmc_step_h"):
+                         "nqs_launch_count", "nqs_fisher", "nqs_vmc_step_h", "nqs_hamiltonian_create_k",
+                         "nqs_hamiltonian_compile_host_k", "nqs_hamiltonian_info_k", "nqs_local_energy_k"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -154,9 +159,12 @@ def _np(x, dtype, shape_tail=None):
 
 
 def _terms(sites, paulis, coeffs):
-    sites = _np(sites, np.int32).reshape(-1, 2)
-    paulis = _np(paulis, np.uint8).reshape(-1, 2)
+    """Term arrays [T,K]: K = 2 slots per term, or up to 8 for k-site Pauli strings (the *_k entry points)."""
     coeffs = _np(coeffs, np.complex64).reshape(-1)
+    sites = _np(sites, np.int32)
+    K = sites.shape[1] if sites.ndim == 2 and sites.shape[0] == coeffs.shape[0] else 2
+    sites = sites.reshape(-1, K)
+    paulis = _np(paulis, np.uint8).reshape(-1, K)
     assert sites.shape[0] == paulis.shape[0] == coeffs.shape[0]
     return sites, paulis, coeffs
 
@@ -200,15 +208,21 @@ class Hamiltonian:
         sites, paulis, coeffs = _terms(sites, paulis, coeffs)
         self.N = int(N)
         self.T = int(coeffs.shape[0])
+        self.K = int(sites.shape[1])
         self._h = ctypes.c_void_p()
-        fn = lib.nqs_hamiltonian_compile_host if host_only else lib.nqs_hamiltonian_create
-        _check(fn(self.N, self.T, _hp(sites), _hp(paulis), _hp(coeffs), ctypes.byref(self._h)))
+        if self.K == 2:
+            fn = lib.nqs_hamiltonian_compile_host if host_only else lib.nqs_hamiltonian_create
+            _check(fn(self.N, self.T, _hp(sites), _hp(paulis), _hp(coeffs), ctypes.byref(self._h)))
+        else:
+            fn = lib.nqs_hamiltonian_compile_host_k if host_only else lib.nqs_hamiltonian_create_k
+            _check(fn(self.N, self.T, self.K, _hp(sites), _hp(paulis), _hp(coeffs), ctypes.byref(self._h)))
         info = np.zeros(5, np.int32)
         _check(lib.nqs_hamiltonian_info(self._h, _hp(info), None))
         self.G, self.C, self.n_diag, self.n_group_terms = (int(v) for v in info[:4])
-        flips = np.zeros((max(self.G, 1), 2), np.int32)
-        _check(lib.nqs_hamiltonian_info(self._h, _hp(info), _hp(flips)))
-        self.flip_sites = flips[: self.G].copy()
+        flips = np.zeros((max(self.G, 1), 4), np.int32)
+        _check(lib.nqs_hamiltonian_info_k(self._h, _hp(info), _hp(flips)))
+        self.flip_sites4 = flips[: self.G].copy()
+        self.flip_sites = self.flip_sites4[:, :2].copy()
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
@@ -356,7 +370,8 @@ def metropolis(spins, a, b, W, sites, u, want_accepted: bool = True, trace: bool
 def hamiltonian_info_host(N: int, sites, paulis, coeffs) -> dict:
     """Host-only compile (no GPU needed): grouping of the term list by flip set."""
     h = Hamiltonian(N, sites, paulis, coeffs, host_only=True)
-    out = dict(G=h.G, C=h.C, n_diag=h.n_diag, n_group_terms=h.n_group_terms, flip_sites=h.flip_sites)
+    out = dict(G=h.G, C=h.C, n_diag=h.n_diag, n_group_terms=h.n_group_terms, flip_sites=h.flip_sites,
+               flip_sites4=h.flip_sites4)
     h.close()
     return out
 
@@ -382,12 +397,16 @@ def local_energy(spins, a, b, W, sites, paulis, coeffs, want_logpsi: bool = True
     sites, paulis, coeffs = _terms(sites, paulis, coeffs)
     eloc = torch.empty(B, dtype=torch.complex64, device=spins.device)
     logpsi = torch.empty(B, dtype=torch.complex64, device=spins.device) if want_logpsi else None
+    K = int(sites.shape[1])
+    head = (_dev(spins, torch.int8, "spins"), B, N, M, _dev(a, torch.complex64, "a"), _dev(b, torch.complex64, "b"),
+            _dev(W, torch.complex64, "W"), int(coeffs.shape[0]))
+    tail = (_hp(sites), _hp(paulis), _hp(coeffs), ctypes.c_void_p(eloc.data_ptr()),
+            ctypes.c_void_p(logpsi.data_ptr()) if want_logpsi else None)
     with torch.cuda.device(spins.device):
-        _check(load_library().nqs_local_energy(
-            _dev(spins, torch.int8, "spins"), B, N, M, _dev(a, torch.complex64, "a"), _dev(b, torch.complex64, "b"),
-            _dev(W, torch.complex64, "W"), int(coeffs.shape[0]), _hp(sites), _hp(paulis), _hp(coeffs),
-            ctypes.c_void_p(eloc.data_ptr()), ctypes.c_void_p(logpsi.data_ptr()) if want_logpsi else None,
-            _stream()))
+        if K == 2:
+            _check(load_library().nqs_local_energy(*head, *tail, _stream()))
+        else:
+            _check(load_library().nqs_local_energy_k(*head, K, *tail, _stream()))
     return (eloc, logpsi) if want_logpsi else eloc
 
 

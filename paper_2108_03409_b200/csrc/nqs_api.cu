@@ -230,24 +230,34 @@ static int upload(nqs_hamiltonian* h, DeviceState* D, bool pooled, cudaStream_t 
         ints.insert(ints.end(), v.begin(), v.end());
         return o;
     };
-    std::vector<int32_t> f0(G), f1(G), first(G), count(G);
+    std::vector<int32_t> f0(G), f1(G), f2(G), f3(G), first(G), count(G);
     for (int g = 0; g < G; ++g) {
-        f0[g] = hc.groups[g].f0;
-        f1[g] = hc.groups[g].f1;
+        f0[g] = hc.groups[g].f[0];
+        f1[g] = hc.groups[g].f[1];
+        f2[g] = hc.groups[g].f[2];
+        f3[g] = hc.groups[g].f[3];
         first[g] = hc.groups[g].term_first;
         count[g] = hc.groups[g].term_count;
     }
     std::vector<int32_t> ci(C_pad, 0), ck(C_pad, -1), cp(C_pad, 1), cg(C_pad, -1);
+    std::vector<int32_t> cs2(C_pad, -1), cp2(C_pad, 1), cs3(C_pad, -1), cp3(C_pad, 1);
     for (int c = 0; c < h->C; ++c) {
         ci[c] = hc.col_i[c];
         ck[c] = hc.col_k[c];
         cp[c] = hc.col_p[c];
+        cs2[c] = hc.col_s2[c];
+        cp2[c] = hc.col_p2[c];
+        cs3[c] = hc.col_s3[c];
+        cp3[c] = hc.col_p3[c];
         cg[c] = hc.col_group[c];
     }
     const size_t o_dz0 = push(hc.diag_z0), o_dz1 = push(hc.diag_z1);
     const size_t o_f0 = push(f0), o_f1 = push(f1), o_first = push(first), o_count = push(count);
     const size_t o_gz0 = push(hc.gt_z0), o_gz1 = push(hc.gt_z1);
     const size_t o_ci = push(ci), o_ck = push(ck), o_cp = push(cp), o_cg = push(cg);
+    const size_t o_f2 = push(f2), o_f3 = push(f3);
+    const size_t o_cs2 = push(cs2), o_cp2 = push(cp2), o_cs3 = push(cs3), o_cp3 = push(cp3);
+    const size_t o_dxo = push(hc.diag_zx_off), o_dx = push(hc.diag_zx), o_gxo = push(hc.gt_zx_off), o_gx = push(hc.gt_zx);
     size_t int_bytes = (ints.size() * sizeof(int) + 15) / 16 * 16;
     std::vector<nqs_c64> cs;
     cs.insert(cs.end(), hc.diag_c.begin(), hc.diag_c.end());
@@ -289,6 +299,17 @@ static int upload(nqs_hamiltonian* h, DeviceState* D, bool pooled, cudaStream_t 
     Dv.col_k = di + o_ck;
     Dv.col_p = di + o_cp;
     Dv.col_group = di + o_cg;
+    Dv.grp_f2 = di + o_f2;
+    Dv.grp_f3 = di + o_f3;
+    Dv.col_s2 = di + o_cs2;
+    Dv.col_p2 = di + o_cp2;
+    Dv.col_s3 = di + o_cs3;
+    Dv.col_p3 = di + o_cp3;
+    Dv.has_zx = hc.has_zx ? 1 : 0;
+    Dv.diag_zx_off = di + o_dxo;
+    Dv.diag_zx = di + o_dx;
+    Dv.gt_zx_off = di + o_gxo;
+    Dv.gt_zx = di + o_gx;
     return NQS_OK;
 }
 
@@ -308,13 +329,13 @@ static void destroy_handle(nqs_hamiltonian* h) {
 }
 
 // mode 0 host only, 1 blocking upload (user handle), 2 pooled, stream-ordered upload (cache entry)
-static int create_impl(int32_t N, int32_t T, const int32_t* s, const uint8_t* p, const nqs_c64* c, int mode,
+static int create_impl(int32_t N, int32_t T, int32_t K, const int32_t* s, const uint8_t* p, const nqs_c64* c, int mode,
                        cudaStream_t st, nqs_hamiltonian** out) {
     if (!out) return fail(NQS_ERR_INVALID_ARG, "nqs_hamiltonian_create: out is NULL");
     *out = nullptr;
     auto* h = new nqs_hamiltonian();
     std::string err;
-    int rc = compile_hamiltonian(N, T, s, p, c, h->hc, err);
+    int rc = compile_hamiltonian(N, T, K, s, p, c, h->hc, err);
     if (rc != NQS_OK) {
         delete h;
         return fail(rc, err);
@@ -335,11 +356,19 @@ static int create_impl(int32_t N, int32_t T, const int32_t* s, const uint8_t* p,
 
 extern "C" int nqs_hamiltonian_create(int32_t N, int32_t T, const int32_t* h_sites, const uint8_t* h_paulis,
                                       const nqs_c64* h_coeffs, nqs_hamiltonian** out) {
-    return create_impl(N, T, h_sites, h_paulis, h_coeffs, 1, nullptr, out);
+    return create_impl(N, T, 2, h_sites, h_paulis, h_coeffs, 1, nullptr, out);
 }
 extern "C" int nqs_hamiltonian_compile_host(int32_t N, int32_t T, const int32_t* h_sites, const uint8_t* h_paulis,
                                             const nqs_c64* h_coeffs, nqs_hamiltonian** out) {
-    return create_impl(N, T, h_sites, h_paulis, h_coeffs, 0, nullptr, out);
+    return create_impl(N, T, 2, h_sites, h_paulis, h_coeffs, 0, nullptr, out);
+}
+extern "C" int nqs_hamiltonian_create_k(int32_t N, int32_t T, int32_t K, const int32_t* h_sites, const uint8_t* h_paulis,
+                                        const nqs_c64* h_coeffs, nqs_hamiltonian** out) {
+    return create_impl(N, T, K, h_sites, h_paulis, h_coeffs, 1, nullptr, out);
+}
+extern "C" int nqs_hamiltonian_compile_host_k(int32_t N, int32_t T, int32_t K, const int32_t* h_sites,
+                                              const uint8_t* h_paulis, const nqs_c64* h_coeffs, nqs_hamiltonian** out) {
+    return create_impl(N, T, K, h_sites, h_paulis, h_coeffs, 0, nullptr, out);
 }
 extern "C" int nqs_hamiltonian_destroy(nqs_hamiltonian* h) {
     destroy_handle(h);
@@ -354,9 +383,16 @@ extern "C" int nqs_hamiltonian_info(const nqs_hamiltonian* h, int32_t info[5], i
     info[4] = h->hc.N;
     if (flip_sites)
         for (size_t g = 0; g < h->hc.groups.size(); ++g) {
-            flip_sites[2 * g] = h->hc.groups[g].f0;
-            flip_sites[2 * g + 1] = h->hc.groups[g].f1;
+            flip_sites[2 * g] = h->hc.groups[g].f[0];
+            flip_sites[2 * g + 1] = h->hc.groups[g].f[1];
         }
+    return NQS_OK;
+}
+extern "C" int nqs_hamiltonian_info_k(const nqs_hamiltonian* h, int32_t info[5], int32_t* flip_sites4) {
+    NQS_TRY(nqs_hamiltonian_info(h, info, nullptr));
+    if (flip_sites4)
+        for (size_t g = 0; g < h->hc.groups.size(); ++g)
+            for (int q = 0; q < 4; ++q) flip_sites4[4 * g + q] = h->hc.groups[g].f[q];
     return NQS_OK;
 }
 
@@ -367,35 +403,36 @@ extern "C" int nqs_hamiltonian_info(const nqs_hamiltonian* h, int32_t info[5], i
 // ----------------------------------------------------------------------------------------
 using HamRef = std::shared_ptr<nqs_hamiltonian>;
 struct CacheEntry {
-    int device, N, T;
+    int device, N, T, K;
     std::vector<unsigned char> key;
     HamRef h;
 };
 static std::mutex g_cache_mu;
 static std::list<CacheEntry> g_cache;
 
-static int cached_hamiltonian(int32_t N, int32_t T, const int32_t* s, const uint8_t* p, const nqs_c64* c,
+static int cached_hamiltonian(int32_t N, int32_t T, int32_t K, const int32_t* s, const uint8_t* p, const nqs_c64* c,
                               cudaStream_t st, HamRef* out) {
-    if (T < 0 || (T > 0 && (!s || !p || !c))) return fail(NQS_ERR_INVALID_ARG, "term arrays are NULL or T < 0");
+    if (T < 0 || K < 1 || K > HAM_MAX_SLOTS || (T > 0 && (!s || !p || !c)))
+        return fail(NQS_ERR_INVALID_ARG, "term arrays are NULL, T < 0 or K outside 1..8");
     int dev = 0;
     NQS_CUDA(cudaGetDevice(&dev));
-    std::vector<unsigned char> key((size_t)T * (8 + 2 + 8));
+    std::vector<unsigned char> key((size_t)T * (4 * K + K + 8));
     if (T > 0) {
-        memcpy(key.data(), s, (size_t)T * 8);
-        memcpy(key.data() + (size_t)T * 8, p, (size_t)T * 2);
-        memcpy(key.data() + (size_t)T * 10, c, (size_t)T * 8);
+        memcpy(key.data(), s, (size_t)T * 4 * K);
+        memcpy(key.data() + (size_t)T * 4 * K, p, (size_t)T * K);
+        memcpy(key.data() + (size_t)T * 5 * K, c, (size_t)T * 8);
     }
     std::lock_guard<std::mutex> lk(g_cache_mu);
     for (auto it = g_cache.begin(); it != g_cache.end(); ++it)
-        if (it->device == dev && it->N == N && it->T == T && it->key == key) {
+        if (it->device == dev && it->N == N && it->T == T && it->K == K && it->key == key) {
             g_cache.splice(g_cache.begin(), g_cache, it);
             *out = g_cache.front().h;
             return NQS_OK;
         }
     nqs_hamiltonian* h = nullptr;
-    NQS_TRY(create_impl(N, T, s, p, c, 2, st, &h));
+    NQS_TRY(create_impl(N, T, K, s, p, c, 2, st, &h));
     HamRef ref(h, destroy_handle);
-    g_cache.push_front(CacheEntry{dev, N, T, std::move(key), ref});
+    g_cache.push_front(CacheEntry{dev, N, T, K, std::move(key), ref});
     if (g_cache.size() > 8) g_cache.pop_back();  // the blob goes when the last holder lets go
     *out = ref;
     return NQS_OK;
@@ -667,7 +704,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         const long long total = (long long)M_pad * C_pad;
         const unsigned tgrid = (unsigned)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
         table_kernel<<<tgrid, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, h->C, TC, nTiles,
-                                            h->dev.col_i, h->dev.col_k, h->dev.col_p, tab, rho);
+                                            h->dev, tab, rho);
         NQS_LAUNCHED();
     }
     // series operands that do not depend on the samples
@@ -689,8 +726,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         NQS_TRY(S.get(&status, 4));
         NQS_CUDA(cudaMemsetAsync(status, 0, 4 * sizeof(int), st));
         series_table_kernel<<<(unsigned)(nNT * NB), 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad,
-                                                                  h->C, NB, h->dev.col_i, h->dev.col_k, h->dev.col_p,
-                                                                  h->dev.col_group, h->dev, sB, scols, sterms);
+                                                                  h->C, NB, h->dev, sB, scols, sterms);
         NQS_LAUNCHED();
     }
     NQS_PROF(1, st);
@@ -806,16 +842,24 @@ extern "C" int nqs_local_energy_h(const nqs_hamiltonian* h, const int8_t* d_spin
     return local_energy_impl(h, d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream, nullptr, nullptr);
 }
 
-extern "C" int nqs_local_energy(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
-                                const nqs_c64* d_b, const nqs_c64* d_W, int32_t T, const int32_t* h_sites,
-                                const uint8_t* h_paulis, const nqs_c64* h_coeffs, nqs_c64* d_eloc,
-                                nqs_c64* d_logpsi, void* stream) {
+extern "C" int nqs_local_energy_k(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
+                                  const nqs_c64* d_b, const nqs_c64* d_W, int32_t T, int32_t K, const int32_t* h_sites,
+                                  const uint8_t* h_paulis, const nqs_c64* h_coeffs, nqs_c64* d_eloc,
+                                  nqs_c64* d_logpsi, void* stream) {
     NQS_TRY(check_common(d_spins, B, N, M, d_a, d_b, d_W));
     DeviceState* D = nullptr;
     NQS_TRY(device_state(&D));
     HamRef h;
-    NQS_TRY(cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, (cudaStream_t)stream, &h));
+    NQS_TRY(cached_hamiltonian(N, T, K, h_sites, h_paulis, h_coeffs, (cudaStream_t)stream, &h));
     return nqs_local_energy_h(h.get(), d_spins, B, M, d_a, d_b, d_W, d_eloc, d_logpsi, stream);
+}
+
+extern "C" int nqs_local_energy(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* d_a,
+                                const nqs_c64* d_b, const nqs_c64* d_W, int32_t T, const int32_t* h_sites,
+                                const uint8_t* h_paulis, const nqs_c64* h_coeffs, nqs_c64* d_eloc,
+                                nqs_c64* d_logpsi, void* stream) {
+    return nqs_local_energy_k(d_spins, B, N, M, d_a, d_b, d_W, T, 2, h_sites, h_paulis, h_coeffs, d_eloc, d_logpsi,
+                              stream);
 }
 
 static int enumerate_impl(const nqs_hamiltonian* h, const int8_t* d_spins, int64_t B, int8_t* d_sprime,
@@ -846,7 +890,7 @@ extern "C" int nqs_enumerate_connected(const int8_t* d_spins, int64_t B, int32_t
     if (B < 0 || N <= 0) return fail(NQS_ERR_INVALID_ARG, "nqs_enumerate_connected: B < 0 or N <= 0");
     if (B == 0) {  // sizing call: no device needed
         nqs_hamiltonian* hh = nullptr;
-        NQS_TRY(create_impl(N, T, h_sites, h_paulis, h_coeffs, 0, nullptr, &hh));
+        NQS_TRY(create_impl(N, T, 2, h_sites, h_paulis, h_coeffs, 0, nullptr, &hh));
         if (G_out) *G_out = (int32_t)hh->hc.groups.size();
         destroy_handle(hh);
         return NQS_OK;
@@ -854,7 +898,7 @@ extern "C" int nqs_enumerate_connected(const int8_t* d_spins, int64_t B, int32_t
     DeviceState* D = nullptr;
     NQS_TRY(device_state(&D));
     HamRef h;
-    NQS_TRY(cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, (cudaStream_t)stream, &h));
+    NQS_TRY(cached_hamiltonian(N, T, 2, h_sites, h_paulis, h_coeffs, (cudaStream_t)stream, &h));
     if (G_out) *G_out = (int32_t)h->hc.groups.size();
     return enumerate_impl(h.get(), d_spins, B, d_sprime, d_mel, stream);
 }
@@ -900,7 +944,7 @@ extern "C" int nqs_local_energy_host(const int8_t* h_spins, int64_t B, int32_t N
     HostStage S;
     NQS_TRY(S.init());
     HamRef h;
-    NQS_TRY(cached_hamiltonian(N, T, h_sites, h_paulis, h_coeffs, S.st, &h));
+    NQS_TRY(cached_hamiltonian(N, T, 2, h_sites, h_paulis, h_coeffs, S.st, &h));
     if (B == 0) return NQS_OK;
     void *ds, *da, *db, *dW, *de, *dl = nullptr;
     NQS_TRY(S.to_device(h_spins, (size_t)B * N, &ds));

@@ -24,6 +24,19 @@ struct DevHam {
     const int* col_k;
     const int* col_p;
     const int* col_group;
+    // k-site Pauli strings: third / fourth flip site of a group and of a column (-1: none)
+    // with the column's relative signs, and the z sites of a term beyond the first two (has_zx: any at all)
+    const int* grp_f2;
+    const int* grp_f3;
+    const int* col_s2;
+    const int* col_p2;
+    const int* col_s3;
+    const int* col_p3;
+    int has_zx;
+    const int* diag_zx_off;
+    const int* diag_zx;
+    const int* gt_zx_off;
+    const int* gt_zx;
 };
 
 __device__ __forceinline__ float2 bc2(float x) { return make_float2(x, x); }
@@ -39,11 +52,49 @@ __device__ __forceinline__ float2 group_element(const DevHam& H, const int8_t* _
         float f = 1.f;
         if (z0 >= 0) f *= (float)srow[z0];
         if (z1 >= 0) f *= (float)srow[z1];
+        if (H.has_zx)
+            for (int x = H.gt_zx_off[first + q]; x < H.gt_zx_off[first + q + 1]; ++x) f *= (float)srow[H.gt_zx[x]];
         const float2 c = H.gt_c[first + q];
         mr = fmaf(c.x, f, mr);
         mi = fmaf(c.y, f, mi);
     }
     return make_float2(mr, mi);
+}
+
+// Is column c (flip sites ci [, ck, s2, s3] with relative signs cp, p2, p3) the one that applies to `srow`?
+__device__ __forceinline__ bool column_active(const DevHam& H, const int8_t* __restrict__ srow, int c, int si) {
+    const int ck = H.col_k[c];
+    if (ck < 0) return true;
+    if ((int)srow[ck] * si != H.col_p[c]) return false;
+    const int s2 = H.col_s2[c];
+    if (s2 < 0) return true;
+    if ((int)srow[s2] * si != H.col_p2[c]) return false;
+    const int s3 = H.col_s3[c];
+    return s3 < 0 || (int)srow[s3] * si == H.col_p3[c];
+}
+
+// V_j = W[j, i] + p W[j, k] + p2 W[j, s2] + p3 W[j, s3] of a column (absent sites: -1), likewise for the bias a
+__device__ __forceinline__ float2 column_sum(const DevHam& H, int c, const float2* __restrict__ row) {
+    float2 v = row[H.col_i[c]];
+    const int k = H.col_k[c];
+    if (k >= 0) {
+        const float p = (float)H.col_p[c];
+        v.x = fmaf(p, row[k].x, v.x);
+        v.y = fmaf(p, row[k].y, v.y);
+        const int s2 = H.col_s2[c];
+        if (s2 >= 0) {
+            const float p2 = (float)H.col_p2[c];
+            v.x = fmaf(p2, row[s2].x, v.x);
+            v.y = fmaf(p2, row[s2].y, v.y);
+            const int s3 = H.col_s3[c];
+            if (s3 >= 0) {
+                const float p3 = (float)H.col_p3[c];
+                v.x = fmaf(p3, row[s3].x, v.x);
+                v.y = fmaf(p3, row[s3].y, v.y);
+            }
+        }
+    }
+    return v;
 }
 
 // Sum of the diagonal terms (empty flip set): d = sum_t c_t * s[z0] * s[z1].
@@ -54,6 +105,8 @@ __device__ __forceinline__ float2 diagonal_element(const DevHam& H, const int8_t
         float f = 1.f;
         if (z0 >= 0) f *= (float)srow[z0];
         if (z1 >= 0) f *= (float)srow[z1];
+        if (H.has_zx)
+            for (int x = H.diag_zx_off[t]; x < H.diag_zx_off[t + 1]; ++x) f *= (float)srow[H.diag_zx[x]];
         const float2 c = H.diag_c[t];
         dr = fmaf(c.x, f, dr);
         di = fmaf(c.y, f, di);

@@ -15,28 +15,23 @@ namespace nqs {
 
 static inline nqs_c64 cmul(nqs_c64 a, nqs_c64 b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
 
-int compile_hamiltonian(int32_t N, int32_t T, const int32_t* sites, const uint8_t* paulis,
+int compile_hamiltonian(int32_t N, int32_t T, int32_t K, const int32_t* sites, const uint8_t* paulis,
                         const nqs_c64* coeffs, HostCompiled& out, std::string& err) {
-    if (N <= 0 || T < 0 || (T > 0 && (!sites || !paulis || !coeffs))) {
-        err = "compile_hamiltonian: bad N/T or NULL term arrays";
+    if (N <= 0 || T < 0 || K < 1 || K > HAM_MAX_SLOTS || (T > 0 && (!sites || !paulis || !coeffs))) {
+        err = "compile_hamiltonian: bad N / T / K (1..8 slots per term) or NULL term arrays";
         return NQS_ERR_INVALID_ARG;
     }
     out = HostCompiled();
     out.N = N;
     out.T = T;
 
-    struct Parsed { int32_t f[2]; int nf; int32_t z[2]; int nz; nqs_c64 c; };
+    struct Parsed { std::vector<int32_t> f, z; nqs_c64 c; };
     std::vector<Parsed> parsed(T);
     for (int t = 0; t < T; ++t) {
-        Parsed p{{-1, -1}, 0, {-1, -1}, 0, coeffs[t]};
-        int32_t s0 = sites[2 * t], s1 = sites[2 * t + 1];
-        if (s0 >= 0 && s0 == s1) {
-            err = "term " + std::to_string(t) + ": the same site in both slots";
-            return NQS_ERR_INVALID_TERM;
-        }
-        for (int k = 0; k < 2; ++k) {
-            int32_t site = sites[2 * t + k];
-            uint8_t pk = paulis[2 * t + k];
+        Parsed p{{}, {}, coeffs[t]};
+        for (int k = 0; k < K; ++k) {
+            const int32_t site = sites[(size_t)t * K + k];
+            const uint8_t pk = paulis[(size_t)t * K + k];
             if (pk > 3) {
                 err = "term " + std::to_string(t) + ": Pauli code > 3";
                 return NQS_ERR_INVALID_TERM;
@@ -52,79 +47,95 @@ int compile_hamiltonian(int32_t N, int32_t T, const int32_t* sites, const uint8_
                 err = "term " + std::to_string(t) + ": site out of range";
                 return NQS_ERR_INVALID_TERM;
             }
-            if (pk == NQS_X || pk == NQS_Y) p.f[p.nf++] = site;
+            for (int k2 = 0; k2 < k; ++k2)
+                if (sites[(size_t)t * K + k2] == site) {
+                    err = "term " + std::to_string(t) + ": the same site in two slots";
+                    return NQS_ERR_INVALID_TERM;
+                }
+            if (pk == NQS_X || pk == NQS_Y) p.f.push_back(site);
             if (pk == NQS_Y) p.c = cmul(p.c, nqs_c64{0.f, -1.f});
-            if (pk == NQS_Y || pk == NQS_Z) p.z[p.nz++] = site;
+            if (pk == NQS_Y || pk == NQS_Z) p.z.push_back(site);
         }
-        if (p.nf == 2 && p.f[0] > p.f[1]) std::swap(p.f[0], p.f[1]);
-        parsed[t] = p;
+        if ((int)p.f.size() > HAM_MAX_FLIPS) {
+            err = "term " + std::to_string(t) + ": more than four X / Y factors (flip sets of up to 4 sites are supported)";
+            return NQS_ERR_UNSUPPORTED;
+        }
+        std::sort(p.f.begin(), p.f.end());
+        parsed[t] = std::move(p);
     }
 
+    auto push_z = [&](const Parsed& p, std::vector<int32_t>& z0, std::vector<int32_t>& z1, std::vector<int32_t>& zx) {
+        z0.push_back(p.z.size() > 0 ? p.z[0] : -1);
+        z1.push_back(p.z.size() > 1 ? p.z[1] : -1);
+        for (size_t q = 2; q < p.z.size(); ++q) zx.push_back(p.z[q]);
+        if (p.z.size() > 2) out.has_zx = true;
+    };
+
     // group by flip set, in order of first appearance
-    std::map<std::pair<int32_t, int32_t>, int> index;
+    std::map<std::vector<int32_t>, int> index;
     std::vector<std::vector<int>> members;
+    out.diag_zx_off.push_back(0);
     for (int t = 0; t < T; ++t) {
         const Parsed& p = parsed[t];
-        if (p.nf == 0) {
-            out.diag_z0.push_back(p.z[0]);
-            out.diag_z1.push_back(p.z[1]);
+        if (p.f.empty()) {
+            push_z(p, out.diag_z0, out.diag_z1, out.diag_zx);
+            out.diag_zx_off.push_back((int32_t)out.diag_zx.size());
             out.diag_c.push_back(p.c);
             continue;
         }
-        auto key = std::make_pair(p.f[0], p.f[1]);
-        auto it = index.find(key);
+        auto it = index.find(p.f);
         if (it == index.end()) {
-            it = index.emplace(key, (int)out.groups.size()).first;
-            out.groups.push_back(HostGroup{p.f[0], p.f[1], 0, 0, {-1, -1}});
+            it = index.emplace(p.f, (int)out.groups.size()).first;
+            HostGroup G{{-1, -1, -1, -1}, (int32_t)p.f.size(), 0, 0};
+            for (size_t q = 0; q < p.f.size(); ++q) G.f[q] = p.f[q];
+            out.groups.push_back(G);
             members.emplace_back();
         }
         members[it->second].push_back(t);
     }
+    out.gt_zx_off.push_back(0);
     for (size_t g = 0; g < out.groups.size(); ++g) {
         HostGroup& G = out.groups[g];
         G.term_first = (int32_t)out.gt_c.size();
         G.term_count = (int32_t)members[g].size();
+        bool outside = false;  // some term has a z factor on a site outside the flip set
         for (int t : members[g]) {
-            out.gt_z0.push_back(parsed[t].z[0]);
-            out.gt_z1.push_back(parsed[t].z[1]);
+            push_z(parsed[t], out.gt_z0, out.gt_z1, out.gt_zx);
+            out.gt_zx_off.push_back((int32_t)out.gt_zx.size());
             out.gt_c.push_back(parsed[t].c);
+            for (int32_t z : parsed[t].z)
+                if (std::find(G.f, G.f + G.nf, z) == G.f + G.nf) outside = true;
         }
-        if (G.f1 < 0) {  // single flip: one column
-            G.col[0] = (int32_t)out.col_i.size();
-            out.col_i.push_back(G.f0);
-            out.col_k.push_back(-1);
-            out.col_p.push_back(+1);
-            out.col_group.push_back((int32_t)g);
-        } else {
-            // pair flip: every term has both slots flipping, so the summed element is a function of
-            // (s_f0, s_f1) only.  Emit the parity column p = s_f0 * s_f1 only if some spin pair of
-            // that parity has a non-zero element (":458 non-zero matrix elements", reading Q5).
-            for (int pi = 0; pi < 2; ++pi) {
-                int par = pi == 0 ? +1 : -1;
-                bool any = false;
-                for (int sa = -1; sa <= 1; sa += 2) {
-                    int sb = par * sa;
-                    float mr = 0.f, mi = 0.f;
-                    for (int q = 0; q < G.term_count; ++q) {
-                        int idx = G.term_first + q;
-                        float f = 1.f;
-                        for (int32_t z : {out.gt_z0[idx], out.gt_z1[idx]}) {
-                            if (z == G.f0) f *= (float)sa;
-                            else if (z == G.f1) f *= (float)sb;
-                        }
-                        mr += out.gt_c[idx].re * f;
-                        mi += out.gt_c[idx].im * f;
+        // one column per pattern of relative signs p_q = s[f_q] s[f_0], q = 1 .. nf-1 (2^(nf-1) patterns).  A
+        // pattern is dropped only if the summed element is zero for both values of s[f_0] and no term looks at a
+        // spin outside the flip set (":458 non-zero matrix elements", reading Q5): the antiparallel-only column
+        // of the Heisenberg bonds.
+        for (int pat = 0; pat < (1 << (G.nf - 1)); ++pat) {
+            int sign[HAM_MAX_FLIPS] = {1, 1, 1, 1};
+            for (int q = 1; q < G.nf; ++q) sign[q] = (pat >> (q - 1)) & 1 ? -1 : 1;
+            bool any = outside;
+            for (int sa = -1; sa <= 1 && !any; sa += 2) {
+                float mr = 0.f, mi = 0.f;
+                for (int t : members[g]) {
+                    float f = 1.f;
+                    for (int32_t z : parsed[t].z) {
+                        const int q = (int)(std::find(G.f, G.f + G.nf, z) - G.f);
+                        f *= (float)(sa * sign[q]);
                     }
-                    if (mr != 0.f || mi != 0.f) any = true;
+                    mr += parsed[t].c.re * f;
+                    mi += parsed[t].c.im * f;
                 }
-                if (any) {
-                    G.col[pi] = (int32_t)out.col_i.size();
-                    out.col_i.push_back(G.f0);
-                    out.col_k.push_back(G.f1);
-                    out.col_p.push_back(par);
-                    out.col_group.push_back((int32_t)g);
-                }
+                if (mr != 0.f || mi != 0.f) any = true;
             }
+            if (!any) continue;
+            out.col_i.push_back(G.f[0]);
+            out.col_k.push_back(G.nf > 1 ? G.f[1] : -1);
+            out.col_p.push_back(sign[1]);
+            out.col_s2.push_back(G.nf > 2 ? G.f[2] : -1);
+            out.col_p2.push_back(sign[2]);
+            out.col_s3.push_back(G.nf > 3 ? G.f[3] : -1);
+            out.col_p3.push_back(sign[3]);
+            out.col_group.push_back((int32_t)g);
         }
     }
     return NQS_OK;

@@ -19,8 +19,7 @@ namespace nqs {
 // rho[c] = (exp(-2A).re, exp(-2A).im, exp(+2A).re, exp(+2A).im), A = a_i + p a_k.
 // ----------------------------------------------------------------------------------------
 __global__ void table_kernel(const float2* __restrict__ W, const float2* __restrict__ a, int N, int M, int M_pad,
-                             int C, int TC, int nTiles, const int* __restrict__ col_i,
-                             const int* __restrict__ col_k, const int* __restrict__ col_p,
+                             int C, int TC, int nTiles, DevHam H,
                              float4* __restrict__ tab, float4* __restrict__ rho) {
     const int C_pad = nTiles * TC;
     const long long total = (long long)M_pad * C_pad;
@@ -30,14 +29,7 @@ __global__ void table_kernel(const float2* __restrict__ W, const float2* __restr
         const int j = (int)(idx / C_pad);
         float4 e = make_float4(1.f, 0.f, 0.f, 0.f);
         if (c < C && j < M) {
-            const int i = col_i[c], k = col_k[c];
-            float2 v = W[(long long)j * N + i];
-            if (k >= 0) {
-                const float2 w2 = W[(long long)j * N + k];
-                const float p = (float)col_p[c];
-                v.x = fmaf(p, w2.x, v.x);
-                v.y = fmaf(p, w2.y, v.y);
-            }
+            const float2 v = column_sum(H, c, W + (long long)j * N);
             const float x = 2.f * v.x, y = 2.f * v.y;
             float sy, cy;
             sincosf(y, &sy, &cy);
@@ -49,13 +41,7 @@ __global__ void table_kernel(const float2* __restrict__ W, const float2* __restr
         if (j == 0) {
             float4 r = make_float4(1.f, 0.f, 1.f, 0.f);
             if (c < C) {
-                const int i = col_i[c], k = col_k[c];
-                float2 A = a[i];
-                if (k >= 0) {
-                    const float p = (float)col_p[c];
-                    A.x = fmaf(p, a[k].x, A.x);
-                    A.y = fmaf(p, a[k].y, A.y);
-                }
+                const float2 A = column_sum(H, c, a);
                 float sy, cy;
                 sincosf(2.f * A.y, &sy, &cy);
                 const float em = expf(-2.f * A.x), ep = expf(2.f * A.x);
@@ -392,8 +378,6 @@ __global__ void __launch_bounds__(WC * WS * 32, (WC * WS <= 10) ? 2 : 1) eloc_ke
     // a4 (part 2) + a6: matrix elements, rho, reduction over the block's columns
     float2* const accs = reinterpret_cast<float2*>(smem_raw);  // [TB][WC], stages are dead now
     const int g = p.H.col_group[c];
-    const int ck = p.H.col_k[c];
-    const int cp = p.H.col_p[c];
     const float4 rho = p.rho[c];
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
@@ -405,8 +389,7 @@ __global__ void __launch_bounds__(WC * WS * 32, (WC * WS <= 10) ? 2 : 1) eloc_ke
             if (g >= 0 && b < p.B) {
                 const int8_t* srow = p.spins + b * p.N;
                 const int si = srow[site];
-                const bool active = (ck < 0) || ((int)srow[ck] * si == cp);
-                if (active) {
+                if (column_active(p.H, srow, c, si)) {
                     const float2 m = group_element(p.H, srow, g);
                     if (m.x != 0.f || m.y != 0.f) {
                         const float rr = si > 0 ? rho.x : rho.z, ri = si > 0 ? rho.y : rho.w;
@@ -472,9 +455,11 @@ __global__ void enumerate_kernel(const int8_t* __restrict__ spins, long long B, 
             mel[idx] = diagonal_element(H, srow);
         } else {
             const int g = slot - 1;
-            const int f0 = H.grp_f0[g], f1 = H.grp_f1[g];
+            const int f0 = H.grp_f0[g], f1 = H.grp_f1[g], f2 = H.grp_f2[g], f3 = H.grp_f3[g];
             out[f0] = (int8_t)(-srow[f0]);
             if (f1 >= 0) out[f1] = (int8_t)(-srow[f1]);
+            if (f2 >= 0) out[f2] = (int8_t)(-srow[f2]);
+            if (f3 >= 0) out[f3] = (int8_t)(-srow[f3]);
             mel[idx] = group_element(H, srow, g);
         }
     }

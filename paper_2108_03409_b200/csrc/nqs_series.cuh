@@ -57,10 +57,12 @@ struct __align__(16) SeriesCol {
     float a2r, a2i;      // 2 A_c,  A = a_i + p a_k
     float k0, k1, k2, k3;  // guard: delta_bc = k0 + n2t k1 + n4t k2 + n6t k3 + n8t k4
     float k4, tmax;      // tmax = max_j |T_jc|
-    int site, sitek;     // flip sites (sitek = -1: single flip)
-    int par, group;      // parity of the column, flip group (-1: padding column)
-    int first, count;    // the group's terms: range into DevHam::gt_* (count <= 2: also inline in SeriesTerms)
+    int site, sitek;     // first / second flip site (sitek = -1: single flip)
+    int par, group;      // bit q: relative sign of flip site q + 1 is -1; flip group (-1: padding column)
+    int sx, count;       // third | fourth << 16 flip site (0xffff: none); number of terms of the group, with
+                         // SR_GENERIC_TERMS set when they are not (all) inline in SeriesTerms
 };
+constexpr int SR_GENERIC_TERMS = 1 << 30;
 static_assert(sizeof(SeriesCol) == 64, "SeriesCol layout");
 // the first two terms of the column's group, element = c * s[z0] * s[z1] (z = -1: factor 1); an absent term has c = 0
 struct __align__(16) SeriesTerms {
@@ -87,18 +89,13 @@ __device__ __forceinline__ unsigned pack_h2(float a, float b) {
 // B_packed[ntile][jchunk16][plane][slab 2][row NB][8 halves]  (one contiguous 256 NB-byte block per stage)
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restrict__ W, const float2* __restrict__ a,
-                                                           int N, int M, int M_pad, int C, int NB,
-                                                           const int* __restrict__ col_i, const int* __restrict__ col_k,
-                                                           const int* __restrict__ col_p,
-                                                           const int* __restrict__ col_group, DevHam H,
+                                                           int N, int M, int M_pad, int C, int NB, DevHam H,
                                                            uint4* __restrict__ B_packed, SeriesCol* __restrict__ cols,
                                                            SeriesTerms* __restrict__ terms) {
     const int c = blockIdx.x, tid = threadIdx.x;
     const int nt = c / NB, cl = c % NB;
     const int nJC = M_pad / 16;
     const bool live_col = c < C;
-    const int ci = live_col ? col_i[c] : 0, ck = live_col ? col_k[c] : -1;
-    const float cp = live_col ? (float)col_p[c] : 1.f;
     double lkr = 0.0, lki = 0.0;
     float n2 = 0.f, n4 = 0.f, n6 = 0.f, n8 = 0.f, tmx = 0.f;
     for (int j8 = tid; j8 < M_pad / 8; j8 += 256) {
@@ -108,12 +105,7 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
             const int j = j8 * 8 + q;
             float Tr = 0.f, Ti = 0.f;
             if (live_col && j < M) {
-                float2 w = W[(long long)j * N + ci];
-                if (ck >= 0) {
-                    const float2 w2 = W[(long long)j * N + ck];
-                    w.x = fmaf(cp, w2.x, w.x);
-                    w.y = fmaf(cp, w2.y, w.y);
-                }
+                const float2 w = column_sum(H, c, W + (long long)j * N);
                 float lr, li;
                 lncosh_tanh(2.f * w.x, 2.f * w.y, lr, li, Tr, Ti);
                 lkr += (double)lr;
@@ -163,14 +155,7 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
         SeriesCol r;
         r.lkr = (float)sd[0][0];
         r.lki = (float)sd[1][0];
-        float2 A = make_float2(0.f, 0.f);
-        if (live_col) {
-            A = a[ci];
-            if (ck >= 0) {
-                A.x = fmaf(cp, a[ck].x, A.x);
-                A.y = fmaf(cp, a[ck].y, A.y);
-            }
-        }
+        const float2 A = live_col ? column_sum(H, c, a) : make_float2(0.f, 0.f);
         r.a2r = 2.f * A.x;
         r.a2i = 2.f * A.y;
         // guard coefficients; u16 = 2^-21 (hi + lo split), u = 2^-10 (one FP16 part,
@@ -183,22 +168,33 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
         r.k3 = (2.f / 3.f) * 9.765625e-4f * n6T;                             // 2 . 2^-10 . 1/3
         r.k4 = 0.5f * n8T;                                                   // truncation: 1/(4 (1 - X)), X <= 1/2
         r.tmax = sqrtf(sf[4][0]);
-        r.site = ci;
-        r.sitek = ck;
-        r.par = (int)cp;
-        r.group = live_col ? col_group[c] : -1;
-        r.first = r.group >= 0 ? H.grp_first[r.group] : 0;
-        r.count = r.group >= 0 ? H.grp_count[r.group] : 0;
-        cols[c] = r;
+        r.site = live_col ? H.col_i[c] : 0;
+        r.sitek = live_col ? H.col_k[c] : -1;
+        r.par = 0;
+        r.sx = 0xffffffff;
+        if (live_col) {
+            const int s2 = H.col_s2[c], s3 = H.col_s3[c];
+            r.par = (H.col_p[c] < 0 ? 1 : 0) | (H.col_p2[c] < 0 ? 2 : 0) | (H.col_p3[c] < 0 ? 4 : 0);
+            r.sx = (s2 >= 0 ? s2 : 0xffff) | ((s3 >= 0 ? s3 : 0xffff) << 16);
+        }
+        r.group = live_col ? H.col_group[c] : -1;
+        const int first = r.group >= 0 ? H.grp_first[r.group] : 0;
+        int count = r.group >= 0 ? H.grp_count[r.group] : 0;
+        // inline fast path: at most two terms, none with more than two z factors
+        bool generic = count > 2;
+        if (H.has_zx)
+            for (int u = 0; u < count; ++u) generic |= H.gt_zx_off[first + u + 1] > H.gt_zx_off[first + u];
         SeriesTerms t2 = {-1, -1, 0.f, 0.f, -1, -1, 0.f, 0.f};
-        if (r.count >= 1) {
-            const float2 cc = H.gt_c[r.first];
-            t2.z0a = H.gt_z0[r.first], t2.z1a = H.gt_z1[r.first], t2.cra = cc.x, t2.cia = cc.y;
+        if (!generic && count >= 1) {
+            const float2 cc = H.gt_c[first];
+            t2.z0a = H.gt_z0[first], t2.z1a = H.gt_z1[first], t2.cra = cc.x, t2.cia = cc.y;
         }
-        if (r.count >= 2) {
-            const float2 cc = H.gt_c[r.first + 1];
-            t2.z0b = H.gt_z0[r.first + 1], t2.z1b = H.gt_z1[r.first + 1], t2.crb = cc.x, t2.cib = cc.y;
+        if (!generic && count >= 2) {
+            const float2 cc = H.gt_c[first + 1];
+            t2.z0b = H.gt_z0[first + 1], t2.z1b = H.gt_z1[first + 1], t2.crb = cc.x, t2.cib = cc.y;
         }
+        r.count = count | (generic ? SR_GENERIC_TERMS : 0);
+        cols[c] = r;
         terms[c] = t2;
     }
 }
@@ -449,7 +445,9 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
         if (nt == 0) {  // diagonal terms (empty flip set): d = sum_t c_t s[z0] s[z1]; the halves split the list
 #pragma unroll 4
             for (int t = half; t < p.H.Td; t += 2) {
-                const float f = spin_or_one(p.H.diag_z0[t]) * spin_or_one(p.H.diag_z1[t]);
+                float f = spin_or_one(p.H.diag_z0[t]) * spin_or_one(p.H.diag_z1[t]);
+                if (p.H.has_zx)
+                    for (int x = p.H.diag_zx_off[t]; x < p.H.diag_zx_off[t + 1]; ++x) f *= spin_from_bits(mybits, p.H.diag_zx[x]);
                 const float2 cc = p.H.diag_c[t];
                 er_acc = fmaf(cc.x, f, er_acc);
                 ei_acc = fmaf(cc.y, f, ei_acc);
@@ -475,15 +473,25 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 const SeriesCol cr = scol[c0 + q];
                 const SeriesTerms tm = sterm[c0 + q];
                 const float si = spin_from_bits(mybits, cr.site);
-                const float sk = spin_or_one(cr.sitek);
-                const bool active = cr.group >= 0 && (cr.sitek < 0 || si * sk == (float)cr.par);
-                // summed matrix element of the group (Eq. 39): two inline terms, the rest (rare) from global memory
+                // the column applies iff every further flip site q has s_q s_i equal to the column's relative sign
+                bool active = cr.group >= 0;
+                if (cr.sitek >= 0) {
+                    active = active && (si * spin_from_bits(mybits, cr.sitek) == ((cr.par & 1) ? -1.f : 1.f));
+                    const int s2 = cr.sx & 0xffff, s3 = (cr.sx >> 16) & 0xffff;
+                    if (s2 != 0xffff) active = active && (si * spin_from_bits(mybits, s2) == ((cr.par & 2) ? -1.f : 1.f));
+                    if (s3 != 0xffff) active = active && (si * spin_from_bits(mybits, s3) == ((cr.par & 4) ? -1.f : 1.f));
+                }
+                // summed matrix element of the group (Eq. 39): two inline terms, or (rare) the general list
                 const float fa = spin_or_one(tm.z0a) * spin_or_one(tm.z1a), fb = spin_or_one(tm.z0b) * spin_or_one(tm.z1b);
                 float mr = fmaf(tm.cra, fa, tm.crb * fb), mi = fmaf(tm.cia, fa, tm.cib * fb);
-                if (cr.count > 2) {
-                    for (int u = 2; u < cr.count; ++u) {
-                        const float f = spin_or_one(p.H.gt_z0[cr.first + u]) * spin_or_one(p.H.gt_z1[cr.first + u]);
-                        const float2 cc = p.H.gt_c[cr.first + u];
+                if (cr.count & SR_GENERIC_TERMS) {
+                    const int first = p.H.grp_first[cr.group], count = cr.count & ~SR_GENERIC_TERMS;
+                    for (int u = 0; u < count; ++u) {
+                        float f = spin_or_one(p.H.gt_z0[first + u]) * spin_or_one(p.H.gt_z1[first + u]);
+                        if (p.H.has_zx)
+                            for (int x = p.H.gt_zx_off[first + u]; x < p.H.gt_zx_off[first + u + 1]; ++x)
+                                f *= spin_from_bits(mybits, p.H.gt_zx[x]);
+                        const float2 cc = p.H.gt_c[first + u];
                         mr = fmaf(cc.x, f, mr);
                         mi = fmaf(cc.y, f, mi);
                     }

@@ -148,3 +148,41 @@ def test_missing_library_fails_loudly(nqs, monkeypatch):
     monkeypatch.setattr(binding, "_LIB_PATH", "/nonexistent/libnqs_b200.so")
     with pytest.raises(FileNotFoundError):
         binding.load_library()
+
+
+# ------------------------------------------------------------------ k-site Pauli strings
+def test_k_site_strings_compile(nqs):
+    X, Y, Z = wl.PAULI_X, wl.PAULI_Y, wl.PAULI_Z
+    sites = np.array([[0, 1, 2, -1], [2, 0, 1, -1], [0, 1, 2, 3], [4, 1, -1, 5], [3, 2, 1, 0], [1, 3, -1, -1]], np.int32)
+    paulis = np.array([[X, X, X, 0], [Y, X, Y, 0], [Z, Z, Z, Z], [X, Z, 0, Z], [X, Y, X, Y], [Z, X, 0, 0]], np.uint8)
+    coeffs = np.array([1.0, 0.5j, -1.0, 2.0, 0.25, 1.0], np.complex64)
+    info = nqs.hamiltonian_info_host(6, sites, paulis, coeffs)
+    # flip sets: {0,1,2} (terms 0, 1), {} (term 2), {4} (term 3), {0,1,2,3} (term 4), {3} (term 5)
+    assert info["G"] == 4 and info["n_diag"] == 1 and info["n_group_terms"] == 5
+    assert info["flip_sites4"].tolist() == [[0, 1, 2, -1], [4, -1, -1, -1], [0, 1, 2, 3], [3, -1, -1, -1]]
+    # columns: a flip set of m sites has 2^(m-1) relative-sign patterns, dropped only if provably zero:
+    #   {0,1,2}: XXX + (i/2) Y X Y over sites (2,0,1): element 1 + (i/2)(-s_2 s_1): never zero -> 4
+    #   {4}: 1;  {0,1,2,3}: XYXY alone: element -(s_2 s_0) * 0.25: never zero -> 8;  {3}: 1
+    assert info["C"] == 4 + 1 + 8 + 1
+    # XXX - XXX cancels identically -> no column; XXX + (XYY over the same sites): 1 - s_1 s_2 -> half the patterns
+    s3 = np.array([[0, 1, 2], [0, 1, 2]], np.int32)
+    assert nqs.hamiltonian_info_host(3, s3, np.array([[X, X, X], [X, X, X]], np.uint8),
+                                     np.array([1.0, -1.0], np.complex64))["C"] == 0
+    assert nqs.hamiltonian_info_host(3, s3, np.array([[X, X, X], [X, Y, Y]], np.uint8),
+                                     np.array([1.0, 1.0], np.complex64))["C"] == 2
+
+
+def test_k_site_strings_invalid_and_unsupported(nqs):
+    X = wl.PAULI_X
+    five = np.array([[0, 1, 2, 3, 4]], np.int32)
+    with pytest.raises(nqs.NqsError) as ei:  # five flipping sites: 16 sign columns per group -- not supported
+        nqs.hamiltonian_info_host(6, five, np.full((1, 5), X, np.uint8), np.ones(1, np.complex64))
+    assert ei.value.code == -4
+    with pytest.raises(nqs.NqsError) as ei:  # the same site in slots 0 and 3
+        nqs.hamiltonian_info_host(6, np.array([[2, 1, 0, 2]], np.int32), np.full((1, 4), X, np.uint8),
+                                  np.ones(1, np.complex64))
+    assert ei.value.code == -2
+    with pytest.raises(nqs.NqsError) as ei:  # nine slots
+        nqs.hamiltonian_info_host(12, np.arange(9, dtype=np.int32)[None, :], np.full((1, 9), 3, np.uint8),
+                                  np.ones(1, np.complex64))
+    assert ei.value.code == -1
