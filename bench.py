@@ -468,6 +468,23 @@ def run_ours(args) -> None:
                               "proposals_per_s": w.B * w.N / (m_ms * 1e-3),
                               "acceptance": float(acc.float().mean().item()) / w.N,
                               "what": "nqs_metropolis, one sweep of all chains, median of 3"}
+        # the shared-site variant: the same sweep with one proposal site per step for all chains
+        m_sites1 = torch.randint(0, w.N, (w.N,), device=dev, dtype=torch.int32, generator=gen)
+        chains = spins.clone()
+        ms_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)]
+        for k in range(4):
+            if k >= 1:
+                ms_ev[k - 1][0].record()
+            acc_s = nqs.metropolis_shared(chains, a, b, W, m_sites1, m_u)
+            if k >= 1:
+                ms_ev[k - 1][1].record()
+        torch.cuda.synchronize()
+        ms_ms = float(np.median([s0.elapsed_time(s1) for s0, s1 in ms_ev]))
+        line["metropolis_shared"] = {"ms_per_sweep": ms_ms, "chains": w.B, "steps_per_sweep": w.N,
+                                     "proposals_per_s": w.B * w.N / (ms_ms * 1e-3),
+                                     "acceptance": float(acc_s.float().mean().item()) / w.N,
+                                     "what": "nqs_metropolis_shared (one proposal site per step for all chains: table rows "
+                                             "staged once per block, chain state in registers), median of 3"}
         del m_sites, m_u, chains
         # pipe rates measured on this box (nqs_microbench; register-only kernels, after the timed region)
         mb = {k: nqs.microbench(k)["lane_ops_per_s"] for k in nqs.MICROBENCH_KINDS}

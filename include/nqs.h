@@ -278,6 +278,17 @@ int nqs_metropolis_trace(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const
                          const nqs_c64 *d_b, const nqs_c64 *d_W, int32_t S, const int32_t *d_sites,
                          const float *d_u, int32_t *d_accepted, uint8_t *d_decisions, void *stream);
 
+/* Shared-site variant: at step t EVERY chain proposes the same site d_sites[t] (d_sites [S] int32 DEVICE; d_u,
+ * d_accepted, d_decisions as in nqs_metropolis_trace, d_decisions may be NULL).  Each chain is still a valid
+ * single-spin-flip Metropolis chain of p(s) (its proposal sequence is a fixed, chain-independent schedule -- e.g. a
+ * random permutation of the sites per sweep -- and its uniforms are its own).  The table rows exp(+-4W)[site] are
+ * then fetched once per thread block and step instead of once per chain, and the chain state lives in registers:
+ * several times the throughput of nqs_metropolis.  M <= 2048 (NQS_ERR_UNSUPPORTED above).  Same arithmetic,
+ * acceptance rule, float32 caveat and theta refresh (every 2 N steps) as nqs_metropolis. */
+int nqs_metropolis_shared(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64 *d_a,
+                          const nqs_c64 *d_b, const nqs_c64 *d_W, int32_t S, const int32_t *d_sites,
+                          const float *d_u, int32_t *d_accepted, uint8_t *d_decisions, void *stream);
+
 /* Pipe-rate micro-benchmark (the roofline is quoted against the nominal peak
  * AND a peak measured on the box).  Runs a register-only kernel (2 blocks of 320 threads per SM,
  * no memory traffic in the loop) `iters` iterations, best of 3 after one warm-up, on a private

@@ -30,6 +30,7 @@ from .binding import (  # noqa: F401
     log_psi,
     log_psi_host,
     metropolis,
+    metropolis_shared,
     microbench,
     profile_enable,
     profile_last,

@@ -57,6 +57,7 @@ def load_library() -> ctypes.CDLL:
             lib.nqs_hamiltonian_compile_host_k.argtypes = [i32, i32, i32, vp, vp, vp, ctypes.POINTER(vp)]
             lib.nqs_hamiltonian_info_k.argtypes = [vp, vp, vp]
             lib.nqs_local_energy_k.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp, vp]
+            lib.nqs_metropolis_shared.argtypes = [vp, i64, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp]
             lib.nqs_fisher.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_vmc_step_h.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_energy_stats.argtypes = [vp, vp, i64, vp, vp]
@@ -75,7 +76,8 @@ def load_library() -> ctypes.CDLL:
                          "nqs_forces", "nqs_metropolis", "nqs_local_energy_forces_h", "nqs_enumerate_connected_h",
                          "nqs_metropolis_trace", "nqs_set_option", "nqs_get_option", "nqs_debug_last_a5",
                          "nqs_launch_count", "nqs_fisher", "nqs_vmc_step_h", "nqs_hamiltonian_create_k",
-                         "nqs_hamiltonian_compile_host_k", "nqs_hamiltonian_info_k", "nqs_local_energy_k"):
+                         "nqs_hamiltonian_compile_host_k", "nqs_hamiltonian_info_k", "nqs_local_energy_k",
+                         "nqs_metropolis_shared"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -365,6 +367,25 @@ def metropolis(spins, a, b, W, sites, u, want_accepted: bool = True, trace: bool
             return accepted, decisions
         _check(load_library().nqs_metropolis(*args, _stream()))
     return accepted
+
+
+def metropolis_shared(spins, a, b, W, sites, u, trace: bool = False):
+    """nqs_metropolis_shared: every chain proposes sites[t] at step t (sites [S] int32, u [S,C] float32).
+    Advances `spins` [C,N] IN PLACE; returns accepted [C] (and the accept bits uint8 [S,C] with trace=True)."""
+    import torch
+
+    C, N, M = _shapes(spins, a, b, W)
+    S = int(sites.shape[0])
+    if tuple(sites.shape) != (S,) or tuple(u.shape) != (S, C):
+        raise ValueError("sites must have shape [S] and u shape [S, C]")
+    accepted = torch.empty(C, dtype=torch.int32, device=spins.device)
+    decisions = torch.empty((S, C), dtype=torch.uint8, device=spins.device) if trace else None
+    with torch.cuda.device(spins.device):
+        _check(load_library().nqs_metropolis_shared(
+            _dev(spins, torch.int8, "spins"), C, N, M, _dev(a, torch.complex64, "a"), _dev(b, torch.complex64, "b"),
+            _dev(W, torch.complex64, "W"), S, _dev(sites, torch.int32, "sites"), _dev(u, torch.float32, "u"),
+            ctypes.c_void_p(accepted.data_ptr()), ctypes.c_void_p(decisions.data_ptr()) if trace else None, _stream()))
+    return (accepted, decisions) if trace else accepted
 
 
 def hamiltonian_info_host(N: int, sites, paulis, coeffs) -> dict:

@@ -1320,6 +1320,77 @@ static int metropolis_impl(int8_t* d_spins, int64_t C, int32_t N, int32_t M, con
     return NQS_OK;
 }
 
+template <int PPL>
+static int launch_metropolis_shared_t(DeviceState* D, const MetroSharedParams& p, cudaStream_t st) {
+    using Cfg = MetroSharedCfg<PPL>;
+    const size_t smem = metropolis_shared_smem_bytes(Cfg::WARPS, p.N, p.M_pad);
+    NQS_TRY(ensure_smem(D, metropolis_shared_kernel<PPL>, smem));
+    metropolis_shared_kernel<PPL><<<(unsigned)((p.C + Cfg::WARPS - 1) / Cfg::WARPS), Cfg::NT, smem, st>>>(p);
+    NQS_LAUNCHED();
+    return NQS_OK;
+}
+
+extern "C" int nqs_metropolis_shared(int8_t* d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64* d_a,
+                                     const nqs_c64* d_b, const nqs_c64* d_W, int32_t S, const int32_t* d_sites,
+                                     const float* d_u, int32_t* d_accepted, uint8_t* d_decisions, void* stream) {
+    NQS_TRY(check_common(d_spins, C, N, M, d_a, d_b, d_W));
+    if (S < 0 || (S > 0 && C > 0 && (!d_sites || !d_u)))
+        return fail(NQS_ERR_INVALID_ARG, "nqs_metropolis_shared: S < 0 or NULL sites / u");
+    DeviceState* D = nullptr;
+    NQS_TRY(device_state(&D));
+    if (C == 0) return NQS_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    NQS_TRY(validate_spins(D, d_spins, C, N, st));
+    const int M_pad = (int)round_up(M, KJ);
+    const int ppl_need = (M_pad / 2 + 31) / 32;
+    if (ppl_need > 32)
+        return fail(NQS_ERR_UNSUPPORTED, "nqs_metropolis_shared: M > 2048 (the chain state lives in registers)");
+    const long long C_pad = round_up(C, 256);
+    const long long nPairsPad = C_pad / 2;
+    Scratch Sc(D, st);
+    float4 *tp = nullptr, *Gp = nullptr, *Gm = nullptr;
+    float* lk2 = nullptr;
+    NQS_TRY(Sc.get(&tp, (size_t)M_pad * nPairsPad));
+    NQS_TRY(Sc.get(&Gp, (size_t)N * (M_pad / 2)));
+    NQS_TRY(Sc.get(&Gm, (size_t)N * (M_pad / 2)));
+    NQS_TRY(Sc.get(&lk2, (size_t)N));
+    site_table_kernel<<<(unsigned)N, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, Gp, Gm, lk2);
+    NQS_LAUNCHED();
+    MetroSharedParams p;
+    p.spins = d_spins;
+    p.C = C;
+    p.N = N;
+    p.M = M;
+    p.M_pad = M_pad;
+    p.tp = tp;
+    p.nPairsPad = nPairsPad;
+    p.Gp = Gp;
+    p.Gm = Gm;
+    p.lk2 = lk2;
+    p.accepted = d_accepted;
+    const int chunk = 2 * N;  // theta is recomputed from the current spins every two sweeps
+    for (int s0 = 0; s0 == 0 || s0 < S; s0 += chunk) {
+        ThetaOut o;
+        o.tp = tp;
+        o.raw = true;
+        NQS_TRY(launch_theta(D, d_spins, C, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
+        p.S = S - s0 < chunk ? S - s0 : chunk;
+        p.sites = d_sites + s0;
+        p.u = d_u + (long long)s0 * C;
+        p.decisions = d_decisions ? d_decisions + (long long)s0 * C : nullptr;
+        p.accumulate = s0 > 0;
+        if (ppl_need <= 1) NQS_TRY(launch_metropolis_shared_t<1>(D, p, st));
+        else if (ppl_need <= 2) NQS_TRY(launch_metropolis_shared_t<2>(D, p, st));
+        else if (ppl_need <= 4) NQS_TRY(launch_metropolis_shared_t<4>(D, p, st));
+        else if (ppl_need <= 8) NQS_TRY(launch_metropolis_shared_t<8>(D, p, st));
+        else if (ppl_need <= 13) NQS_TRY(launch_metropolis_shared_t<13>(D, p, st));
+        else if (ppl_need <= 16) NQS_TRY(launch_metropolis_shared_t<16>(D, p, st));
+        else if (ppl_need <= 25) NQS_TRY(launch_metropolis_shared_t<25>(D, p, st));
+        else NQS_TRY(launch_metropolis_shared_t<32>(D, p, st));
+    }
+    return NQS_OK;
+}
+
 extern "C" int nqs_metropolis(int8_t* d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64* d_a,
                               const nqs_c64* d_b, const nqs_c64* d_W, int32_t S, const int32_t* d_sites,
                               const float* d_u, int32_t* d_accepted, void* stream) {

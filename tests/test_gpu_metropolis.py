@@ -125,6 +125,79 @@ def test_metropolis_config5_full_size_sampled_chains(nqs, oracle):
             "config 5 sampled chains")
 
 
+def gpu_metropolis_shared(nqs, spins, a, b, W, sites, u):
+    import torch
+
+    d = torch.device("cuda:0")
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x)).to(d)  # noqa: E731
+    sp = t(spins.copy())
+    acc, dec = nqs.metropolis_shared(sp, t(a), t(b), t(W), t(sites), t(u), trace=True)
+    torch.cuda.synchronize()
+    return sp.cpu().numpy(), acc.cpu().numpy(), dec.cpu().numpy()
+
+
+@pytest.mark.parametrize("N,M,C,S,sigma,seed", [
+    (8, 8, 256, 64, 0.3, 11),         # one hidden-unit pair record per lane (PPL = 1)
+    (40, 80, 1000, 200, 0.05, 12),    # config-2 shapes, 5 sweeps, chains not a multiple of the 12-chain block
+    (37, 45, 333, 150, 0.2, 13),      # ragged
+    (100, 400, 2048, 100, 0.03, 14),  # config-3 shapes (PPL = 8)
+    (20, 30, 64, 2000, 0.25, 15),     # long chains: 100 sweeps, theta refreshed every 2 N steps
+    (142, 95, 463, 227, 0.25, 16),    # saturated hidden units
+    (50, 700, 100, 120, 0.02, 17),    # PPL = 13
+    (30, 1900, 40, 70, 0.01, 18),     # PPL = 32 (8-warp blocks)
+])
+def test_metropolis_shared_site_vs_oracle(nqs, oracle, N, M, C, S, sigma, seed):
+    """nqs_metropolis_shared: every chain proposes the same site at a step.  Same oracle (the site schedule is
+    broadcast to [S, C]), same per-chain rule."""
+    w = wl.make_random(N, M, C, 4, sigma, 300 + seed)
+    rng = np.random.default_rng([seed, 9])
+    sites1 = rng.integers(0, N, S).astype(np.int32)
+    u = rng.random((S, w.B), dtype=np.float32)
+    sites = np.ascontiguousarray(np.broadcast_to(sites1[:, None], (S, w.B)))
+    final, acc, dec = gpu_metropolis_shared(nqs, w.spins, w.a, w.b, w.W, sites1, u)
+    ref_final, ref_acc, _, ref_dec, ref_mar = oracle.metropolis(w.spins, w.a, w.b, w.W, sites, u, trace=True)
+    parted = compare(w.spins, sites, final, acc, dec, ref_final, ref_acc, ref_dec, ref_mar,
+                     f"shared N={N} M={M} C={w.B} S={S}")
+    assert parted <= 0.5 * w.B
+    assert 0.05 < acc.mean() / S <= 1.0
+
+
+def test_metropolis_shared_config5_full_size_sampled_chains(nqs, oracle):
+    """The launch configuration of the sampler bench (65536 chains, N = 400, M = 1600: PPL = 25, 12-chain blocks)."""
+    w = wl.make_config(5)
+    S = 24
+    rng = np.random.default_rng(57)
+    sites1 = rng.integers(0, w.N, S).astype(np.int32)
+    u = rng.random((S, w.B), dtype=np.float32)
+    final, acc, dec = gpu_metropolis_shared(nqs, w.spins, w.a, w.b, w.W, sites1, u)
+    sites = np.ascontiguousarray(np.broadcast_to(sites1[:, None], (S, w.B)))
+    assert np.array_equal(dec.sum(axis=0), acc) and np.array_equal(replay(w.spins, sites, dec), final)
+    sel = np.sort(np.random.default_rng(58).choice(w.B, size=48, replace=False))
+    sel[0], sel[1], sel[-1] = 0, 11, w.B - 1
+    ref_final, ref_acc, _, ref_dec, ref_mar = oracle.metropolis(w.spins[sel], w.a, w.b, w.W, sites[:, sel], u[:, sel],
+                                                                trace=True)
+    compare(w.spins[sel], sites[:, sel], final[sel], acc[sel], dec[:, sel], ref_final, ref_acc, ref_dec, ref_mar,
+            "config 5 shared-site sampled chains")
+
+
+def test_metropolis_shared_samples_the_born_distribution(nqs):
+    """A fixed site schedule shared by all chains still samples |psi|^2 (each chain is a valid Metropolis chain)."""
+    from dense_reference import all_states, psi_all
+
+    N, M, C, S = 5, 4, 60000, 100
+    w = wl.make_random(N, M, 1 << N, 4, 0.3, 98)
+    p = np.abs(psi_all(N, w.a, w.b, w.W)) ** 2
+    p /= p.sum()
+    rng = np.random.default_rng(99)
+    start = all_states(N).astype(np.int8)[rng.integers(0, 1 << N, C)]
+    sites1 = rng.integers(0, N, S).astype(np.int32)
+    u = rng.random((S, C), dtype=np.float32)
+    final, _, _ = gpu_metropolis_shared(nqs, start, w.a, w.b, w.W, sites1, u)
+    idx = ((1 - final.astype(np.int64)) // 2) @ (1 << np.arange(N - 1, -1, -1))
+    freq = np.bincount(idx, minlength=1 << N) / C
+    assert np.all(np.abs(freq - p) < 4.5 * np.sqrt(p * (1 - p) / C)), np.abs(freq - p).max()
+
+
 def test_metropolis_properties(nqs):
     import torch
 
