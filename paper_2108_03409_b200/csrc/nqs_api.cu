@@ -562,18 +562,18 @@ static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, in
     const long long rows = (o.tp || o.sA) ? nPairsPad * 2 : B;
     const long long nMT = (rows + TM_M - 1) / TM_M;
     const int K_pad = (int)round_up(N, TM_KC), K16 = K_pad / 16;
-    const int nNT = (M_pad + TM_JT - 1) / TM_JT;
+    const int nNT = (M_pad + TH_JT - 1) / TH_JT;
     Scratch S(D, st);
     uint4 *A_packed = nullptr, *B_packed = nullptr;
     float* scale = nullptr;
     NQS_TRY(S.get(&A_packed, (size_t)nMT * K16 * TM_M));
-    NQS_TRY(S.get(&B_packed, (size_t)nNT * K16 * TM_N));
-    NQS_TRY(S.get(&scale, (size_t)nNT * TM_JT));
+    NQS_TRY(S.get(&B_packed, (size_t)nNT * K16 * TH_N));
+    NQS_TRY(S.get(&scale, (size_t)nNT * TH_JT));
     const long long a_items = nMT * K16 * TM_M;
     const unsigned agrid = (unsigned)((a_items + 255) / 256 < 148 * 16 ? (a_items + 255) / 256 : 148 * 16);
     pack_spins_kernel<<<agrid, 256, 0, st>>>(d_spins, (long long)B, N, K16, nMT, A_packed, o.gate);
     NQS_LAUNCHED();
-    pack_w_kernel<<<(unsigned)(nNT * TM_JT), 128, 0, st>>>((const float2*)d_W, N, M, K16, B_packed, scale, o.gate);
+    pack_w_kernel<<<(unsigned)(nNT * TH_JT), 128, 0, st>>>((const float2*)d_W, N, M, K16, B_packed, scale, o.gate);
     NQS_LAUNCHED();
     const size_t smem = theta_mma_smem_bytes(K_pad);
     NQS_TRY(ensure_smem(D, theta_mma_kernel, smem));

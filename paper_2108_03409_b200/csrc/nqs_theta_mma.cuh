@@ -36,8 +36,16 @@ constexpr int TM_B_STAGE_BYTES = TM_B_K16_BYTES * (TM_KC / 16);
 constexpr int TM_THREADS = 320;
 constexpr int TM_MAX_KPAD = 512;
 
+// theta_mma_kernel itself works on tiles of 16 hidden units (128 accumulator columns) and keeps TWO accumulator
+// sets in TMEM, so that the MMAs of tile nt + 1 run while the epilogue warps are still on tile nt
+constexpr int TH_JT = 16;       // hidden units per accumulator tile
+constexpr int TH_N = 128;       // accumulator columns = TH_JT * 2 * 4
+constexpr int TH_STAGES = 6;
+constexpr int TH_B_K16_BYTES = TH_N * 16;
+constexpr int TH_B_STAGE_BYTES = TH_B_K16_BYTES * (TM_KC / 16);  // 8 KB
+
 __host__ __device__ inline size_t theta_mma_smem_bytes(int K_pad) {
-    return (size_t)(K_pad / 16) * TM_A_K16_BYTES + (size_t)TM_STAGES * TM_B_STAGE_BYTES + 256;
+    return (size_t)(K_pad / 16) * TM_A_K16_BYTES + (size_t)TH_STAGES * TH_B_STAGE_BYTES + 256;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -74,7 +82,7 @@ __global__ void pack_spins_kernel(const int8_t* __restrict__ spins, long long B,
 // One block per hidden unit j (padded to nNT*32): power-of-two scale from the row maximum, then
 // W_ji * 2^(27-e) rounded to an integer Q, |Q| <= 2^27, written as digits d0..d3 in [-64, 64]:
 //   Q = d0 + 128 d1 + 128^2 d2 + 128^3 d3.
-// B_packed[ntile][k16][n = 8*jl + 4*part + digit][16 bytes];  scale[j] = 2^(e-27).
+// B_packed[ntile16][k16][n = 8*jl + 4*part + digit][16 bytes] (tiles of TH_JT = 16 units);  scale[j] = 2^(e-27).
 __global__ void __launch_bounds__(128) pack_w_kernel(const float2* __restrict__ W, int N, int M, int K16,
                                                      uint4* __restrict__ B_packed, float* __restrict__ scale,
                                                      const int* __restrict__ gate) {
@@ -96,7 +104,7 @@ __global__ void __launch_bounds__(128) pack_w_kernel(const float2* __restrict__ 
     int e = 0;
     if (mx > 0.f) (void)frexpf(mx, &e);  // mx = f * 2^e, f in [0.5, 1)
     if (tid == 0) scale[j] = (mx > 0.f && j < M) ? ldexpf(1.f, e - 27) : 0.f;
-    const int nt = j / TM_JT, jl = j % TM_JT;
+    const int nt = j / TH_JT, jl = j % TH_JT;
     for (int item = tid; item < 2 * K16; item += 128) {
         const int part = item & 1, k16 = item >> 1;
         unsigned d[4][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
@@ -116,7 +124,7 @@ __global__ void __launch_bounds__(128) pack_w_kernel(const float2* __restrict__ 
                 }
             }
         }
-        uint4* dst = B_packed + ((long long)nt * K16 + k16) * TM_N + jl * 8 + part * 4;
+        uint4* dst = B_packed + ((long long)nt * K16 + k16) * TH_N + jl * 8 + part * 4;
 #pragma unroll
         for (int l = 0; l < 4; ++l) dst[l] = make_uint4(d[l][0], d[l][1], d[l][2], d[l][3]);
     }
@@ -159,6 +167,7 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes
 }
 constexpr uint32_t TM_IDESC = (2u << 4) /* D = S32 */ | (1u << 7) /* A = INT8 */ | (1u << 10) /* B = INT8 */ |
                               ((uint32_t)(TM_N >> 3) << 17) | ((uint32_t)(TM_M >> 4) << 24);
+constexpr uint32_t TH_IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TH_N >> 3) << 17) | ((uint32_t)(TM_M >> 4) << 24);
 
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, int (&v)[32]) {
     asm volatile(
@@ -227,13 +236,13 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
     const int K16 = p.K16;
     unsigned char* const sA = tm_smem;
     unsigned char* const sB = tm_smem + (size_t)K16 * TM_A_K16_BYTES;
-    uint64_t* const bars = reinterpret_cast<uint64_t*>(sB + (size_t)TM_STAGES * TM_B_STAGE_BYTES);
+    uint64_t* const bars = reinterpret_cast<uint64_t*>(sB + (size_t)TH_STAGES * TH_B_STAGE_BYTES);
     uint64_t* const a_full = bars;
     uint64_t* const b_full = bars + 1;
-    uint64_t* const b_empty = bars + 1 + TM_STAGES;
-    uint64_t* const t_full = bars + 1 + 2 * TM_STAGES;
-    uint64_t* const t_empty = bars + 2 + 2 * TM_STAGES;
-    uint32_t* const tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 + 2 * TM_STAGES);
+    uint64_t* const b_empty = bars + 1 + TH_STAGES;
+    uint64_t* const t_full = bars + 1 + 2 * TH_STAGES;   // [2]: one per accumulator set
+    uint64_t* const t_empty = bars + 3 + 2 * TH_STAGES;  // [2]
+    uint32_t* const tmem_slot = reinterpret_cast<uint32_t*>(bars + 5 + 2 * TH_STAGES);
     double* const lp_x = reinterpret_cast<double*>(sB);           // reused after the main loop: [128][2]
     float* const nrm_x = reinterpret_cast<float*>(lp_x + 2 * TM_M);  // [128][5]
 
@@ -243,15 +252,17 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
 
     if (tid == 0) {
         mbar_init(a_full, 1);
-        for (int s = 0; s < TM_STAGES; ++s) {
+        for (int s = 0; s < TH_STAGES; ++s) {
             mbar_init(&b_full[s], 1);
             mbar_init(&b_empty[s], 1);
         }
-        mbar_init(t_full, 1);
-        mbar_init(t_empty, 8);
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&t_full[s], 1);
+            mbar_init(&t_empty[s], 8);
+        }
         fence_mbar_init();
     }
-    if (warp == 1) tmem_alloc(tmem_slot, TM_N);
+    if (warp == 1) tmem_alloc(tmem_slot, 2 * TH_N);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -265,11 +276,11 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
             int it = 0;
             for (int nt = 0; nt < p.nNT; ++nt)
                 for (int kc = 0; kc < nKC; ++kc, ++it) {
-                    const int s = it % TM_STAGES;
-                    mbar_wait(&b_empty[s], ((it / TM_STAGES) & 1) ^ 1);
-                    mbar_expect_tx(&b_full[s], TM_B_STAGE_BYTES);
-                    bulk_g2s(sB + (size_t)s * TM_B_STAGE_BYTES,
-                             p.B_packed + ((long long)nt * K16 + kc * (TM_KC / 16)) * TM_N, TM_B_STAGE_BYTES,
+                    const int s = it % TH_STAGES;
+                    mbar_wait(&b_empty[s], ((it / TH_STAGES) & 1) ^ 1);
+                    mbar_expect_tx(&b_full[s], TH_B_STAGE_BYTES);
+                    bulk_g2s(sB + (size_t)s * TH_B_STAGE_BYTES,
+                             p.B_packed + ((long long)nt * K16 + kc * (TM_KC / 16)) * TH_N, TH_B_STAGE_BYTES,
                              &b_full[s]);
                 }
         }
@@ -279,27 +290,28 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
             const uint32_t sA_u = smem_u32(sA), sB_u = smem_u32(sB);
             int it = 0;
             for (int nt = 0; nt < p.nNT; ++nt) {
-                mbar_wait(t_empty, (nt & 1) ^ 1);
+                const int set = nt & 1;
+                mbar_wait(&t_empty[set], ((nt >> 1) & 1) ^ 1);
                 tc_fence_after();
                 for (int kc = 0; kc < nKC; ++kc, ++it) {
-                    const int s = it % TM_STAGES;
-                    mbar_wait(&b_full[s], (it / TM_STAGES) & 1);
+                    const int s = it % TH_STAGES;
+                    mbar_wait(&b_full[s], (it / TH_STAGES) & 1);
                     tc_fence_after();
 #pragma unroll
                     for (int ks = 0; ks < TM_KC / 32; ++ks) {
                         const uint64_t ad = umma_desc(sA_u + (uint32_t)(kc * (TM_KC / 16) + ks * 2) * TM_A_K16_BYTES,
                                                       TM_A_K16_BYTES, 128);
-                        const uint64_t bd = umma_desc(sB_u + (uint32_t)s * TM_B_STAGE_BYTES + (uint32_t)(ks * 2) * TM_B_K16_BYTES,
-                                                      TM_B_K16_BYTES, 128);
-                        umma_i8(tmem_base, ad, bd, TM_IDESC, (kc | ks) ? 1u : 0u);
+                        const uint64_t bd = umma_desc(sB_u + (uint32_t)s * TH_B_STAGE_BYTES + (uint32_t)(ks * 2) * TH_B_K16_BYTES,
+                                                      TH_B_K16_BYTES, 128);
+                        umma_i8(tmem_base + (uint32_t)set * TH_N, ad, bd, TH_IDESC, (kc | ks) ? 1u : 0u);
                     }
                     tc_commit(&b_empty[s]);  // frees the stage once these MMAs have read it
                 }
-                tc_commit(t_full);
+                tc_commit(&t_full[set]);
             }
         }
     } else {
-        // ---------------- epilogue: 8 warps; TMEM lanes 32*(warp%4).., column half (warp-2)/4 = 16 hidden units
+        // ---------------- epilogue: 8 warps; TMEM lanes 32*(warp%4).., column half (warp-2)/4 = 8 hidden units
         const int ew = warp - 2;
         const int lane_grp = warp & 3, half = ew >> 2;
         const int row = lane_grp * 32 + lane;
@@ -311,21 +323,24 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
         float2 n2 = make_float2(0.f, 0.f), n4 = n2, n6 = n2, n8 = n2;  // the two halves of a unit pair accumulate apart
         float tmx = 0.f;
         for (int nt = 0; nt < p.nNT; ++nt) {
-            // scale and bias of this warp's 16 hidden units: lane u (and u + 16) holds unit u, fetched before the
+            // scale and bias of this warp's 8 hidden units: lane u (mod 8) holds unit u, fetched before the
             // accumulator wait and handed round by shuffles
-            const int jmine = nt * TM_JT + half * 16 + (lane & 15);
+            const int set = nt & 1;
+            const int jmine = nt * TH_JT + half * 8 + (lane & 7);
             const float my_sc = p.scale[jmine];
             const float2 my_b = jmine < p.M ? p.bvec[jmine] : make_float2(0.f, 0.f);
-            mbar_wait(t_full, nt & 1);
+            mbar_wait(&t_full[set], (nt >> 1) & 1);
             tc_fence_after();
-#pragma unroll 1
-            for (int sb = 0; sb < 2; ++sb) {  // 8 hidden units per pass = one 16-byte slab of every series plane
+            {   // 8 hidden units per warp and tile = one 16-byte slab of every series plane
                 int v0[32], v1[32];
-                const uint32_t col = (uint32_t)(half * 128 + sb * 64);
+                const uint32_t col = (uint32_t)(set * TH_N + half * 64);
                 tmem_ld32_nowait(tmem_base + ((uint32_t)(lane_grp * 32) << 16) + col, v0);
                 tmem_ld32_nowait(tmem_base + ((uint32_t)(lane_grp * 32) << 16) + col + 32, v1);
                 tmem_ld_wait();
-                const int jbase = nt * TM_JT + half * 16 + sb * 8;
+                tc_fence_before();  // the accumulators are in registers: hand the set back to the MMA issuer
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&t_empty[set]);
+                const int jbase = nt * TH_JT + half * 8;
                 float2 tr[4], ti[4];
                 float lsr = 0.f, lsi = 0.f;
 #pragma unroll
@@ -337,7 +352,7 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
                         const int u = 2 * pq + h;
                         const int j = jbase + u;
                         live[h] = j < p.M;
-                        const int src = sb * 8 + u;
+                        const int src = u;
                         const float sc = __shfl_sync(0xffffffffu, my_sc, src);
                         const float2 bj = make_float2(__shfl_sync(0xffffffffu, my_b.x, src), __shfl_sync(0xffffffffu, my_b.y, src));
                         const int* w = (u < 4) ? &v0[u * 8] : &v1[(u - 4) * 8];
@@ -403,9 +418,6 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
                     for (int pl = 0; pl < 8; ++pl) dst[pl * 2 * TM_M] = make_uint4(wd[pl][0], wd[pl][1], wd[pl][2], wd[pl][3]);
                 }
             }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(t_empty);
         }
         // visible bias, split between the two column halves of a row
         if (b < p.B && p.logpsi) {
@@ -446,7 +458,7 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
     __syncthreads();
     if (warp == 1) {
         tc_fence_after();
-        tmem_dealloc(tmem_base, TM_N);
+        tmem_dealloc(tmem_base, 2 * TH_N);
     }
 }
 
