@@ -92,6 +92,7 @@ struct DeviceState {
     cudaMemPool_t pool = nullptr;
     int* status = nullptr;  // [4]: guard flag, failed samples, path tag of the last call (1 series, 2 product), -
     int* tags = nullptr;    // [4] constant {0, 1, 2, 3}: device-side source of the path tag
+    std::atomic<int> last_tag{0};  // path tag the most recent call enqueued
     std::map<const void*, size_t> smem_optin;
 };
 static DeviceState g_dev[MAX_DEVICES];
@@ -777,6 +778,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     }
     NQS_PROF(5, st);
     const int* gate = (use_series && use_product) ? status : nullptr;
+    const bool fused_finalize = use_product && !use_series && nTiles == 1;  // eloc_kernel writes E_loc itself
     if (use_product && !tp_now) {  // fallback pass: tanh(theta) for the product form, only if the guard failed
         ThetaOut o;
         o.tp = tp;
@@ -797,20 +799,25 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         p.H = h->dev;
         p.partial = partial;
         p.status = gate;
+        p.eloc_out = fused_finalize ? (float2*)d_eloc : nullptr;
         NQS_TRY(launch_eloc(D, h, p, B_pad, st));
     }
     NQS_PROF(6, st);
-    if (use_product || !use_series) {
+    if ((use_product || !use_series) && !fused_finalize) {
         finalize_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(d_spins, (long long)B, N, h->dev, partial,
                                                                      have_cols ? nTiles : 0, (float2*)d_eloc, gate);
         NQS_LAUNCHED();
     }
-    // debug record of the decision (nqs_debug_last_a5): {guard flag, failed samples} of this call, path tag
-    if (use_series)
+    // debug record of the decision (nqs_debug_last_a5): {guard flag, failed samples} of this call, path tag.
+    // Product-only calls rewrite it only when the previous call on this device was not one of them.
+    if (use_series) {
         NQS_CUDA(cudaMemcpyAsync(D->status, status, 2 * sizeof(int), cudaMemcpyDeviceToDevice, st));
-    else
+        NQS_CUDA(cudaMemcpyAsync(D->status + 2, D->tags + 1, sizeof(int), cudaMemcpyDeviceToDevice, st));
+        D->last_tag.store(1);
+    } else if (D->last_tag.exchange(2) != 2) {
         NQS_CUDA(cudaMemsetAsync(D->status, 0, 2 * sizeof(int), st));
-    NQS_CUDA(cudaMemcpyAsync(D->status + 2, D->tags + (use_series ? 1 : 2), sizeof(int), cudaMemcpyDeviceToDevice, st));
+        NQS_CUDA(cudaMemcpyAsync(D->status + 2, D->tags + 2, sizeof(int), cudaMemcpyDeviceToDevice, st));
+    }
     NQS_PROF(7, st);
     g_prof_valid = g_prof_on;
     mark_use(h, st);

@@ -218,6 +218,7 @@ struct ElocParams {
     DevHam H;
     float2* partial;        // [B][nTiles]
     const int* status;      // nullptr, or the guard word of the series path: run only if (status[0] & 1)
+    float2* eloc_out;       // [B] or nullptr: with a single column tile the kernel also adds the diagonal and writes E_loc
 };
 
 template <int WC, int WS, int KJ>
@@ -375,31 +376,45 @@ __global__ void __launch_bounds__(WC * WS * 32, (WC * WS <= 10) ? 2 : 1) eloc_ke
         __syncthreads();
     }
 
-    // a4 (part 2) + a6: matrix elements, rho, reduction over the block's columns
+    // a4 (part 2) + a6: matrix elements, rho, reduction over the block's columns.  Everything that depends on the
+    // column only is fetched once; the per-sample part is branch-free (inline terms) so that the loads of the 16
+    // samples a thread owns are in flight together -- on small problems this epilogue is the critical path.
     float2* const accs = reinterpret_cast<float2*>(smem_raw);  // [TB][WC], stages are dead now
     const int g = p.H.col_group[c];
     const float4 rho = p.rho[c];
+    const int ck = p.H.col_k[c], cs2 = p.H.col_s2[c], cs3 = p.H.col_s3[c];
+    const int pk = p.H.col_p[c], p2 = p.H.col_p2[c], p3 = p.H.col_p3[c];
+    const int first = g >= 0 ? p.H.grp_first[g] : 0, count = g >= 0 ? p.H.grp_count[g] : 0;
+    bool generic = count > 2;  // inline: at most two terms, none with more than two z factors
+    if (p.H.has_zx)
+        for (int u = 0; u < count; ++u) generic |= p.H.gt_zx_off[first + u + 1] > p.H.gt_zx_off[first + u];
+    int z0a = -1, z1a = -1, z0b = -1, z1b = -1;
+    float2 ca = make_float2(0.f, 0.f), cb = ca;
+    if (!generic && count >= 1) z0a = p.H.gt_z0[first], z1a = p.H.gt_z1[first], ca = p.H.gt_c[first];
+    if (!generic && count >= 2) z0b = p.H.gt_z0[first + 1], z1b = p.H.gt_z1[first + 1], cb = p.H.gt_c[first + 1];
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
         const int pl = ws * 16 + 2 * r + ls;
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const long long b = 2 * (pair0 + pl) + h;
+            const bool live_b = g >= 0 && b < p.B;
+            const int8_t* srow = p.spins + (b < p.B ? b : p.B - 1) * p.N;
+            auto spin_or = [&](int z, int dflt) { return z >= 0 ? (int)srow[z] : dflt; };
+            const int si = srow[site];
+            const bool active = live_b && spin_or(ck, si * pk) * si == pk && spin_or(cs2, si * p2) * si == p2 &&
+                                spin_or(cs3, si * p3) * si == p3;
+            const float fa = (float)(spin_or(z0a, 1) * spin_or(z1a, 1)), fb = (float)(spin_or(z0b, 1) * spin_or(z1b, 1));
+            float2 m = make_float2(fmaf(ca.x, fa, cb.x * fb), fmaf(ca.y, fa, cb.y * fb));
+            if (generic && active) m = group_element(p.H, srow, g);
             float cr = 0.f, ci = 0.f;
-            if (g >= 0 && b < p.B) {
-                const int8_t* srow = p.spins + b * p.N;
-                const int si = srow[site];
-                if (column_active(p.H, srow, c, si)) {
-                    const float2 m = group_element(p.H, srow, g);
-                    if (m.x != 0.f || m.y != 0.f) {
-                        const float rr = si > 0 ? rho.x : rho.z, ri = si > 0 ? rho.y : rho.w;
-                        const float vr = m.x * rr - m.y * ri, vi = m.x * ri + m.y * rr;
-                        const float pr = h ? Pr[r].y : Pr[r].x, pi = h ? Pi[r].y : Pi[r].x;
-                        const int ex = h ? exB[r] : exA[r];
-                        cr = ldexpf(vr * pr - vi * pi, ex);
-                        ci = ldexpf(vr * pi + vi * pr, ex);
-                    }
-                }
+            if (active && (m.x != 0.f || m.y != 0.f)) {
+                const float rr = si > 0 ? rho.x : rho.z, ri = si > 0 ? rho.y : rho.w;
+                const float vr = m.x * rr - m.y * ri, vi = m.x * ri + m.y * rr;
+                const float pr = h ? Pr[r].y : Pr[r].x, pi = h ? Pi[r].y : Pi[r].x;
+                const int ex = h ? exB[r] : exA[r];
+                cr = ldexpf(vr * pr - vi * pi, ex);
+                ci = ldexpf(vr * pi + vi * pr, ex);
             }
 #pragma unroll
             for (int o = 1; o < 16; o <<= 1) {
@@ -419,7 +434,12 @@ __global__ void __launch_bounds__(WC * WS * 32, (WC * WS <= 10) ? 2 : 1) eloc_ke
                 sr += accs[sl * WC + w].x;
                 si += accs[sl * WC + w].y;
             }
-            p.partial[b * p.nTiles + tile] = make_float2(sr, si);
+            if (p.eloc_out) {  // single column tile: a6 finishes here (diagonal + off-diagonal sum), no finalize launch
+                const float2 d = diagonal_element(p.H, p.spins + b * p.N);
+                p.eloc_out[b] = make_float2(d.x + sr, d.y + si);
+            } else {
+                p.partial[b * p.nTiles + tile] = make_float2(sr, si);
+            }
         }
     }
 }
