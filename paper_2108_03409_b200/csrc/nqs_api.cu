@@ -71,7 +71,8 @@ static std::atomic<int> g_opt[NQS_OPT_COUNT] = {};
 
 extern "C" int nqs_set_option(int32_t key, int32_t value) {
     if (key < 0 || key >= NQS_OPT_COUNT) return fail(NQS_ERR_INVALID_ARG, "nqs_set_option: unknown key");
-    const int hi = key == NQS_OPT_A5_PATH ? 3 : 1;
+    const int hi = key == NQS_OPT_A5_PATH ? 3 : key == NQS_OPT_SERIES_CLUSTER ? 4 : 1;
+    if (key == NQS_OPT_SERIES_CLUSTER && value == 3) return fail(NQS_ERR_INVALID_ARG, "cluster size must be 0, 1, 2 or 4");
     if (value < 0 || value > hi) return fail(NQS_ERR_INVALID_ARG, "nqs_set_option: value out of range");
     g_opt[key].store(value);
     return NQS_OK;
@@ -767,7 +768,25 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         gp.partial = spartial;
         const long long blocks = (B_pad / SR_M) * nNT;
         if (blocks > 0x7fffffffll) return fail(NQS_ERR_UNSUPPORTED, "B x column tiles exceeds the grid limit");
-        series_gemm_kernel<<<(unsigned)blocks, SR_THREADS, smem, st>>>(gp);
+        // optionally the column tiles of a sample tile form a cluster and share the A planes by multicast (measured:
+        // no gain -- the kernel is bound by shared-memory bandwidth, not by the L2 fill)
+        int cs = g_opt[NQS_OPT_SERIES_CLUSTER].load();
+        if (cs == 0) cs = 1;
+        while (cs > 1 && nNT % cs != 0) cs >>= 1;
+        gp.CS = cs;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)blocks);
+        cfg.blockDim = dim3(SR_THREADS);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)cs;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        NQS_CUDA(cudaLaunchKernelEx(&cfg, series_gemm_kernel, gp));
         NQS_LAUNCHED();
     }
     NQS_PROF(4, st);

@@ -292,6 +292,27 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
 #pragma unroll
     for (int k = 0; k < 16; ++k) v[k] = __uint_as_float(r[k]);
 }
+// cluster helpers: the column-tile CTAs of one sample tile form a cluster and share the A planes by multicast
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_g2s_multicast(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar,
+                                                   uint16_t mask) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(smem_dst)),
+        "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "h"(mask)
+        : "memory");
+}
+__device__ __forceinline__ void tc_commit_multicast(uint64_t* bar, uint16_t mask) {
+    asm volatile(
+        "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
+            smem_u32(bar)),
+        "h"(mask)
+        : "memory");
+}
+
 // D = F32, A = B = F16, K-major both, N >> 3 at bit 17, M >> 4 at bit 24; bit 13 negates A
 __host__ __device__ inline uint32_t series_idesc(int NB) {
     return (1u << 4) | ((uint32_t)(NB >> 3) << 17) | ((uint32_t)(SR_M >> 4) << 24);
@@ -313,6 +334,7 @@ struct SeriesGemmParams {
     const int8_t* spins;     // [B][N]
     long long B;
     int N, nJC, NB, nNT;
+    int CS;                  // cluster size (1, 2 or 4 consecutive column tiles of a sample tile; divides nNT)
     DevHam H;
     float4* partial;         // [B][nNT]: (Re, Im of sum_c m R [+ diagonal in tile 0], guard eps, 0)
 };
@@ -336,11 +358,13 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
     const int nt = blockIdx.x % p.nNT;
     const long long mt = blockIdx.x / p.nNT;
     const int nJC = p.nJC;
+    const int CS = p.CS, rank = nt % CS;  // cluster = CS consecutive column tiles of this sample tile
+    const uint16_t cmask = (uint16_t)((1u << CS) - 1u);
 
     if (tid == 0) {
         for (int s = 0; s < SR_STAGES; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], 1);
+            mbar_init(&empty[s], (uint32_t)CS);  // a stage is free when every CTA of the cluster has consumed it
         }
         mbar_init(t_full, 1);
         fence_mbar_init();
@@ -348,6 +372,7 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
     if (warp == 1) tmem_alloc(tmem_slot, 512);
     tc_fence_before();
     __syncthreads();
+    if (CS > 1) cluster_sync_all();  // every CTA's barriers exist before a peer's copy or commit can reach them
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
@@ -360,7 +385,13 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 mbar_wait(&empty[s], ((kc / SR_STAGES) & 1) ^ 1);
                 unsigned char* const st = sr_smem + (size_t)s * stage_bytes;
                 mbar_expect_tx(&full[s], stage_bytes);
-                bulk_g2s(st, gA + (long long)kc * SR_PLANES * SR_A_PLANE_U4, SR_A_STAGE_BYTES, &full[s]);
+                const unsigned char* srcA = reinterpret_cast<const unsigned char*>(gA + (long long)kc * SR_PLANES * SR_A_PLANE_U4);
+                if (CS == 1) {
+                    bulk_g2s(st, srcA, SR_A_STAGE_BYTES, &full[s]);
+                } else {  // this CTA fetches its 1/CS of the A planes and multicasts it to the whole cluster
+                    const uint32_t slice = SR_A_STAGE_BYTES / (uint32_t)CS;
+                    bulk_g2s_multicast(st + (size_t)rank * slice, srcA + (size_t)rank * slice, slice, &full[s], cmask);
+                }
                 bulk_g2s(st + SR_A_STAGE_BYTES, gB + (long long)kc * SR_PLANES * (2 * NB), b_stage_bytes, &full[s]);
             }
         }
@@ -391,7 +422,8 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 cprod(2, 0, d_or, d_oi, 1u);      // t.lo T.hi
                 cprod(6, 6, d_or, d_oi, 1u);      // t^3 T^3 / 3
                 cprod(4, 4, d_er, d_ei, first);   // t^2 T^2 / 2
-                tc_commit(&empty[s]);
+                if (CS == 1) tc_commit(&empty[s]);
+                else tc_commit_multicast(&empty[s], cmask);
             }
             tc_commit(t_full);
         }
@@ -528,6 +560,7 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
     }
     tc_fence_before();
     __syncthreads();
+    if (CS > 1) cluster_sync_all();  // no CTA leaves while a peer's commit may still arrive on its barriers
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc(tmem_base, 512);

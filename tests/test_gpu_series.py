@@ -144,3 +144,18 @@ def test_auto_threshold(nqs):
     w = wl.make_config(3, B=8192)  # 8192 * 100 * 400 = 3.3e8 >= 2^28
     _, _, took = run(nqs, w, "auto")
     assert took["path"] == "series" and not took["guard_failed"]
+
+
+def test_cluster_multicast_is_bit_identical(nqs):
+    """NQS_OPT_SERIES_CLUSTER: the column tiles of a sample tile as a thread-block cluster sharing the t^k planes by
+    multicast (2 and 4 CTAs) give the same bits as independent CTAs."""
+    w = wl.make_config(5, B=1000)  # 4 column tiles
+    out = {}
+    for cs in (1, 2, 4):
+        nqs.set_option("series_cluster", cs)
+        try:
+            out[cs], _, took = run(nqs, w, "series_only")
+        finally:
+            nqs.set_option("series_cluster", 0)
+        assert took["path"] == "series" and not took["guard_failed"]
+    assert np.array_equal(out[1], out[2]) and np.array_equal(out[1], out[4])
