@@ -268,7 +268,10 @@ int nqs_vmc_step_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t B, i
  * a deterministic function of its inputs.  The acceptance test is evaluated in float32 (a decision
  * closer to a tie than ~1e-4 in log |ratio|^2 may differ from exact arithmetic).  The chain state is
  * exp(2 theta), recomputed from the spins every two sweeps (2 N steps) and updated in place by one
- * complex multiplication per hidden unit on each accepted move.  Valid for |Re theta| < 22.  Sites outside [0,N) are undefined behaviour.  S = 0 is a no-op.  Asynchronous.
+ * complex multiplication per hidden unit on each accepted move.  Valid for |Re theta| < 22: beyond that
+ * |exp(2 theta) + 1|^2 leaves the float32 range, the log-ratio becomes NaN and the chain stops accepting; such a
+ * chain is REPORTED, not silently frozen: d_accepted[c] = -1 (its spins are then meaningless).  Sites outside
+ * [0,N) are undefined behaviour.  S = 0 is a no-op.  Asynchronous.
  * NQS_ERR_UNSUPPORTED if one chain's state (8 M + N bytes) does not fit shared memory twice.
  * ------------------------------------------------------------------------------------- */
 int nqs_metropolis(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64 *d_a,

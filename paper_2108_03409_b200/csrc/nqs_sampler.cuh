@@ -133,6 +133,7 @@ __global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroPara
     const int nFull = MP / (32 * MT_UNROLL);  // groups of 32 x MT_UNROLL pairs with no ragged lane
     const float4 one4 = make_float4(1.f, 1.f, 0.f, 0.f);
     int acc = 0;
+    bool bad = false;
     for (int step = 0; step < p.S; ++step) {
         int site = 0;
         float ul = 0.f;
@@ -175,6 +176,7 @@ __global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroPara
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) lg += __shfl_xor_sync(0xffffffffu, lg, o);
         const float lk = p.lk2[site];
+        bad |= !(fabsf(lg) <= 3.0e38f);  // NaN / inf: a hidden unit left the float32 range of exp(2 theta)
         const bool accept = log2f(ul) < (sgi > 0 ? lk : -lk) + lg;  // u == 0: -inf, always accepted
         if (lane == 0 && p.decisions) p.decisions[(long long)step * p.C + c] = accept ? 1 : 0;
         if (accept) {
@@ -206,7 +208,10 @@ __global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroPara
         __syncwarp();
     }
     for (int i = lane; i < p.N; i += 32) p.spins[c * p.N + i] = s_s[i];
-    if (lane == 0 && p.accepted) p.accepted[c] = p.accumulate ? p.accepted[c] + acc : acc;
+    if (lane == 0 && p.accepted) {
+        const int prev = p.accumulate ? p.accepted[c] : 0;
+        p.accepted[c] = (bad || prev < 0) ? -1 : prev + acc;  // -1: the chain's state overflowed (|Re theta| >~ 22)
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -299,6 +304,7 @@ __global__ void __launch_bounds__(MetroSharedCfg<PPL>::NT, 1) metropolis_shared_
         for (int t = 0; t < MS_BUFS - 1 && t < p.S; ++t) stage(t);
 
     int acc = 0;
+    bool bad = false;
     float u_next = (live_chain && p.S > 0) ? p.u[c] : 2.f;  // the uniform of a step is fetched one step ahead
     for (int step = 0; step < p.S; ++step) {
         __syncthreads();  // every warp has finished step - 1: its row buffer may be overwritten
@@ -335,6 +341,7 @@ __global__ void __launch_bounds__(MetroSharedCfg<PPL>::NT, 1) metropolis_shared_
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) lg += __shfl_xor_sync(0xffffffffu, lg, o);
         const float lk = lk_s[site];
+        bad |= !(fabsf(lg) <= 3.0e38f);  // NaN / inf: a hidden unit left the float32 range of exp(2 theta)
         const bool accept = live_chain && (log2f(ul) < (sgi > 0 ? lk : -lk) + lg);  // u == 0: -inf, always accepted
         if (lane == 0 && live_chain && p.decisions) p.decisions[(long long)step * p.C + c] = accept ? 1 : 0;
         if (accept) {
@@ -356,7 +363,10 @@ __global__ void __launch_bounds__(MetroSharedCfg<PPL>::NT, 1) metropolis_shared_
     }
     if (live_chain) {
         for (int i = lane; i < p.N; i += 32) p.spins[c * p.N + i] = s_s[i];
-        if (lane == 0 && p.accepted) p.accepted[c] = p.accumulate ? p.accepted[c] + acc : acc;
+        if (lane == 0 && p.accepted) {
+            const int prev = p.accumulate ? p.accepted[c] : 0;
+            p.accepted[c] = (bad || prev < 0) ? -1 : prev + acc;  // -1: the chain's state overflowed
+        }
     }
 }
 

@@ -235,3 +235,35 @@ def test_metropolis_samples_the_born_distribution(nqs):
     idx = ((1 - final.astype(np.int64)) // 2) @ (1 << np.arange(N - 1, -1, -1))
     freq = np.bincount(idx, minlength=1 << N) / C
     assert np.all(np.abs(freq - p) < 4.5 * np.sqrt(p * (1 - p) / C)), np.abs(freq - p).max()
+
+
+def test_saturated_chain_is_reported_not_frozen(nqs):
+    """ADVICE (round 1): with the state exp(2 theta), |Re theta| >~ 22 overflows float32 and the chain would stop
+    accepting silently.  It must be reported instead: accepted = -1 for such a chain, for both sampler kernels; chains
+    of the same call that stay in range are unaffected."""
+    import torch
+
+    N, M, C, S = 16, 12, 40, 30
+    w = wl.make_random(N, M, C, 4, 0.05, 123)
+    W = w.W.copy()
+    W[3, :] = 2.0  # hidden unit 3: theta = b_3 + 2 sum_i s_i, i.e. |Re theta| = 32 for the aligned configurations
+    spins = w.spins.copy()
+    spins[0, :] = 1     # chain 0: Re theta_3 = +32 -> exp(64) overflows
+    spins[1, :] = -1    # chain 1: Re theta_3 = -32 -> exp(-64) underflows to 0: |E + 1|^2 = 1, stays finite
+    spins[2, : N // 2] = 1
+    spins[2, N // 2:] = -1  # chain 2: Re theta_3 ~ 0
+    rng = np.random.default_rng(124)
+    sites1 = rng.integers(0, N, S).astype(np.int32)
+    u = rng.random((S, C), dtype=np.float32)
+    d = torch.device("cuda:0")
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x)).to(d)  # noqa: E731
+    sites = np.ascontiguousarray(np.broadcast_to(sites1[:, None], (S, C)))
+    acc_a = nqs.metropolis(t(spins), t(w.a), t(w.b), t(W), t(sites), t(u)).cpu().numpy()
+    acc_b = nqs.metropolis_shared(t(spins), t(w.a), t(w.b), t(W), t(sites1), t(u)).cpu().numpy()
+    for acc in (acc_a, acc_b):
+        assert acc[0] == -1, "the overflowing chain must be flagged"
+    assert np.array_equal(acc_a, acc_b)
+    # (the strong unit pulls other chains towards alignment too; whichever saturate are flagged the same way by both
+    # kernels.)  With the original small parameters nothing is flagged:
+    acc_ok = nqs.metropolis_shared(t(spins), t(w.a), t(w.b), t(w.W), t(sites1), t(u)).cpu().numpy()
+    assert np.all(acc_ok >= 0)

@@ -159,3 +159,28 @@ def test_cluster_multicast_is_bit_identical(nqs):
             nqs.set_option("series_cluster", 0)
         assert took["path"] == "series" and not took["guard_failed"]
     assert np.array_equal(out[1], out[2]) and np.array_equal(out[1], out[4])
+
+
+def test_series_with_the_simt_theta_kernel(nqs, oracle):
+    """N > 512 is outside the tensor-core theta kernel: theta_kernel (FP32 SIMT) writes tanh(theta) and
+    series_pack_kernel builds the FP16 planes and the row norms from it; also through the NQS_OPT_THETA_PATH switch
+    at a size both theta kernels cover (the two ways to the planes must agree within the tolerance)."""
+    N, M, B = 530, 48, 300
+    a, b, W = wl.rbm_parameters(N, M, 0.004, [92, 0])
+    ham = wl.tfim(wl.chain_bonds(N), N, 1.0, 0.8)
+    w = wl.Workload("chain_N530", N, M, B, wl.iid_spins(B, N, [92, 1]), a, b, W, ham)
+    e, l, took = run(nqs, w, "series_only")
+    assert took["path"] == "series" and not took["guard_failed"], took
+    e_ref, l_ref = oracle_on(oracle, w, slice(None), "fast")
+    check_eloc(e, e_ref, "series, N=530")
+    check_logpsi(l, l_ref, "series, N=530")
+    w3 = wl.make_config(3, B=700)
+    e_ref, l_ref = oracle_on(oracle, w3, slice(None), "fast")
+    nqs.set_option("theta_path", 1)
+    try:
+        e1, l1, took = run(nqs, w3, "series_only")
+    finally:
+        nqs.set_option("theta_path", 0)
+    assert took["path"] == "series" and not took["guard_failed"], took
+    check_eloc(e1, e_ref, "series, SIMT theta, config 3")
+    check_logpsi(l1, l_ref, "series, SIMT theta, config 3")
