@@ -382,3 +382,47 @@ def test_large_N_takes_the_simt_theta_kernel(nqs, oracle):
     l2 = nqs.log_psi(sp, ad, bd, Wd)
     torch.cuda.synchronize()
     check_logpsi(l2.cpu().numpy(), l_ref, "N=530 nqs_log_psi")
+
+
+def test_nqs_validate_rejects_bad_spin_values(nqs, monkeypatch):
+    """spin values other than +1/-1 are undefined behaviour in release and checked when NQS_VALIDATE=1
+    (read at every call): every device entry point that takes spins then returns NQS_ERR_INVALID_ARG."""
+    import torch
+
+    w = wl.make_config(2, B=300)
+    spins, a, b, W = to_dev(w)
+    bad = spins.clone()
+    bad[17, 5] = 0
+    bad[200, 39] = 3
+    monkeypatch.setenv("NQS_VALIDATE", "1")
+    e, l = nqs.local_energy(spins, a, b, W, w.ham.sites, w.ham.paulis, w.ham.coeffs)  # valid spins pass
+    torch.cuda.synchronize()
+    for call in (lambda: nqs.local_energy(bad, a, b, W, w.ham.sites, w.ham.paulis, w.ham.coeffs),
+                 lambda: nqs.log_psi(bad, a, b, W),
+                 lambda: nqs.metropolis(bad.clone(), a, b, W, torch.zeros((1, w.B), dtype=torch.int32, device=bad.device),
+                                        torch.zeros((1, w.B), dtype=torch.float32, device=bad.device))):
+        with pytest.raises(nqs.NqsError) as ei:
+            call()
+        assert ei.value.code == -1 and "2 spin values" in str(ei.value)
+    monkeypatch.delenv("NQS_VALIDATE")
+    nqs.log_psi(bad, a, b, W)  # release mode: not checked (undefined values, no error)
+    torch.cuda.synchronize()
+
+
+def test_two_devices_in_one_process(nqs, oracle):
+    """ADVICE (round 1): kernel attributes and the scratch pool are per device.  Needs two GPUs; skipped otherwise."""
+    import torch
+
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices in one process")
+    w = wl.make_config(3, B=4096)
+    e_ref, _ = oracle_on(oracle, w, np.arange(0, w.B, 64), "fast")
+    for dev in (0, 1):
+        d = torch.device("cuda", dev)
+        with torch.cuda.device(d):
+            args = [torch.from_numpy(x).to(d) for x in (w.spins, w.a, w.b, w.W)]
+            e, _ = nqs.local_energy(*args, w.ham.sites, w.ham.paulis, w.ham.coeffs)
+            F = nqs.forces(*args, e)
+            torch.cuda.synchronize(d)
+            check_eloc(e.cpu().numpy()[::64], e_ref, f"device {dev}")
+            assert torch.isfinite(torch.view_as_real(F)).all()
