@@ -161,14 +161,11 @@ int nqs_local_energy_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t 
  *                       2 = series + guard + fallback at ANY size
  *                       3 = series only: the guard is evaluated and recorded but nothing is recomputed
  *   NQS_OPT_THETA_PATH  0 = automatic (int8 tcgen05 kernel for N <= 512, else FP32 SIMT)   1 = FP32 SIMT only
- *   NQS_OPT_SERIES_CLUSTER  thread-block cluster size of the series GEMM (the column tiles of a sample tile share
- *                       its operand planes by multicast): 0 = automatic (1: measured no gain), 1 = no cluster, 2, 4; reduced until
- *                       it divides the number of column tiles
  * nqs_debug_last_a5 (synchronises `stream`; tests only; not meaningful while calls run concurrently on other
  * streams): out[0] = 1 if the most recent nqs_local_energy* call on this device attempted the series path, 2 if
  * it used the product form only; out[1] = 1 if the guard failed; out[2] = samples over the guard threshold.
  * ------------------------------------------------------------------------------------- */
-enum { NQS_OPT_A5_PATH = 0, NQS_OPT_THETA_PATH = 1, NQS_OPT_SERIES_CLUSTER = 2, NQS_OPT_COUNT = 3 };
+enum { NQS_OPT_A5_PATH = 0, NQS_OPT_THETA_PATH = 1, NQS_OPT_COUNT = 2 };
 int nqs_set_option(int32_t key, int32_t value);
 int nqs_get_option(int32_t key, int32_t *value);
 int nqs_debug_last_a5(int32_t out[3], void *stream);

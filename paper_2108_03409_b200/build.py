@@ -29,6 +29,7 @@ def nvcc_command(out: str, verbose: bool = False) -> list[str]:
     ]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("NQS_NVCC_FLAGS", "").split()  # development switches, e.g. -DNQS_SERIES_TIMELINE
     cmd += [os.path.join(CSRC, s) for s in SOURCES]
     return cmd
 

@@ -68,11 +68,13 @@ extern "C" const char* nqs_version(void) { return "0.2.0 sm_100a"; }
 // options (include/nqs.h: nqs_set_option)
 // ----------------------------------------------------------------------------------------
 static std::atomic<int> g_opt[NQS_OPT_COUNT] = {};
+#ifdef NQS_SERIES_TIMELINE
+static long long* g_series_timeline = nullptr;
+#endif
 
 extern "C" int nqs_set_option(int32_t key, int32_t value) {
     if (key < 0 || key >= NQS_OPT_COUNT) return fail(NQS_ERR_INVALID_ARG, "nqs_set_option: unknown key");
-    const int hi = key == NQS_OPT_A5_PATH ? 3 : key == NQS_OPT_SERIES_CLUSTER ? 4 : 1;
-    if (key == NQS_OPT_SERIES_CLUSTER && value == 3) return fail(NQS_ERR_INVALID_ARG, "cluster size must be 0, 1, 2 or 4");
+    const int hi = key == NQS_OPT_A5_PATH ? 3 : 1;
     if (value < 0 || value > hi) return fail(NQS_ERR_INVALID_ARG, "nqs_set_option: value out of range");
     g_opt[key].store(value);
     return NQS_OK;
@@ -766,27 +768,12 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         gp.nNT = nNT;
         gp.H = h->dev;
         gp.partial = spartial;
+#ifdef NQS_SERIES_TIMELINE
+        gp.timeline = g_series_timeline;
+#endif
         const long long blocks = (B_pad / SR_M) * nNT;
         if (blocks > 0x7fffffffll) return fail(NQS_ERR_UNSUPPORTED, "B x column tiles exceeds the grid limit");
-        // optionally the column tiles of a sample tile form a cluster and share the A planes by multicast (measured:
-        // no gain -- the kernel is bound by shared-memory bandwidth, not by the L2 fill)
-        int cs = g_opt[NQS_OPT_SERIES_CLUSTER].load();
-        if (cs == 0) cs = 1;
-        while (cs > 1 && nNT % cs != 0) cs >>= 1;
-        gp.CS = cs;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)blocks);
-        cfg.blockDim = dim3(SR_THREADS);
-        cfg.dynamicSmemBytes = smem;
-        cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = (unsigned)cs;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        NQS_CUDA(cudaLaunchKernelEx(&cfg, series_gemm_kernel, gp));
+        series_gemm_kernel<<<(unsigned)blocks, SR_THREADS, smem, st>>>(gp);
         NQS_LAUNCHED();
     }
     NQS_PROF(4, st);
@@ -847,6 +834,16 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     }
     return NQS_OK;
 }
+
+#ifdef NQS_SERIES_TIMELINE
+// development builds only (NQS_NVCC_FLAGS=-DNQS_SERIES_TIMELINE): a device buffer of [blocks][8] int64 that receives
+// the clock64 stamps of every series_gemm_kernel block (start, after set-up, after the prologue, accumulators ready,
+// epilogue done, end)
+extern "C" int nqs_debug_series_timeline(void* d_buf) {
+    g_series_timeline = (long long*)d_buf;
+    return NQS_OK;
+}
+#endif
 
 extern "C" int nqs_debug_last_a5(int32_t out[3], void* stream) {
     if (!out) return fail(NQS_ERR_INVALID_ARG, "out is NULL");

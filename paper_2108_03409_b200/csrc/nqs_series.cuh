@@ -39,7 +39,10 @@ constexpr int SR_PLANES = 8;              // hi.re hi.im lo.re lo.im sq.re sq.im
 constexpr int SR_A_PLANE_U4 = 2 * SR_M;   // uint4 per A plane: [slab 2][row 128][16 bytes]
 constexpr int SR_A_STAGE_BYTES = SR_PLANES * SR_A_PLANE_U4 * 16;  // 32 KB
 constexpr int SR_STAGES = 3;
-constexpr int SR_EPI_WARPS = 8;           // two per TMEM lane group: each takes half of the tile's columns
+constexpr int SR_EPI_PARTS = 4;           // epilogue warps per TMEM lane group: each takes a quarter of the tile's columns
+constexpr int SR_EPI_WARPS = 4 * SR_EPI_PARTS;
+constexpr int SR_EPI_THREADS = 32 * SR_EPI_WARPS;
+constexpr int SR_EPI_COLS = 8;            // columns per TMEM load batch
 constexpr int SR_THREADS = 64 + 32 * SR_EPI_WARPS;  // producer, MMA issuer, epilogue warps
 constexpr int SR_MAX_N = 2048;            // sites (bit-packed spins of the tile live in shared memory)
 // power-of-two operand scales (keep the FP16 parts normal; removed exactly in the epilogue)
@@ -76,7 +79,7 @@ static_assert(sizeof(SeriesTerms) == 32, "SeriesTerms layout");
 __host__ __device__ inline int series_bits_stride(int N) { return (N + 31) / 32 | 1; }  // odd: conflict-free rows
 __host__ __device__ inline size_t series_gemm_smem_bytes(int NB, int N) {
     return (size_t)SR_STAGES * (SR_A_STAGE_BYTES + 256 * NB) + (size_t)NB * (sizeof(SeriesCol) + sizeof(SeriesTerms)) +
-           (size_t)SR_M * series_bits_stride(N) * 4 + (size_t)SR_M * 16 + 256;
+           (size_t)SR_M * series_bits_stride(N) * 4 + (size_t)(SR_EPI_PARTS - 1) * SR_M * 16 + 256;
 }
 
 __device__ __forceinline__ unsigned pack_h2(float a, float b) {
@@ -279,6 +282,13 @@ __device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64
         "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
         : "memory");
 }
+// no register of v may be touched before tcgen05.wait::ld (the load is asynchronous)
+__device__ __forceinline__ void tmem_ld8_nowait(uint32_t taddr, float (&v)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+                 : "r"(taddr)
+                 : "memory");
+}
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
     uint32_t r[16];
     asm volatile(
@@ -292,27 +302,6 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
 #pragma unroll
     for (int k = 0; k < 16; ++k) v[k] = __uint_as_float(r[k]);
 }
-// cluster helpers: the column-tile CTAs of one sample tile form a cluster and share the A planes by multicast
-__device__ __forceinline__ void cluster_sync_all() {
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void bulk_g2s_multicast(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar,
-                                                   uint16_t mask) {
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1], %2, [%3], %4;" ::"r"(
-            smem_u32(smem_dst)),
-        "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "h"(mask)
-        : "memory");
-}
-__device__ __forceinline__ void tc_commit_multicast(uint64_t* bar, uint16_t mask) {
-    asm volatile(
-        "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
-            smem_u32(bar)),
-        "h"(mask)
-        : "memory");
-}
-
 // D = F32, A = B = F16, K-major both, N >> 3 at bit 17, M >> 4 at bit 24; bit 13 negates A
 __host__ __device__ inline uint32_t series_idesc(int NB) {
     return (1u << 4) | ((uint32_t)(NB >> 3) << 17) | ((uint32_t)(SR_M >> 4) << 24);
@@ -334,10 +323,17 @@ struct SeriesGemmParams {
     const int8_t* spins;     // [B][N]
     long long B;
     int N, nJC, NB, nNT;
-    int CS;                  // cluster size (1, 2 or 4 consecutive column tiles of a sample tile; divides nNT)
     DevHam H;
     float4* partial;         // [B][nNT]: (Re, Im of sum_c m R [+ diagonal in tile 0], guard eps, 0)
+#ifdef NQS_SERIES_TIMELINE
+    long long* timeline;     // [blocks][8] clock64 stamps of the first epilogue thread (development builds only)
+#endif
 };
+#ifdef NQS_SERIES_TIMELINE
+#define NQS_STAMP(k) stamp[k] = clock64()
+#else
+#define NQS_STAMP(k)
+#endif
 
 __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const SeriesGemmParams p) {
     extern __shared__ __align__(128) unsigned char sr_smem[];
@@ -345,8 +341,8 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
     const uint32_t b_stage_bytes = 256u * NB, stage_bytes = SR_A_STAGE_BYTES + b_stage_bytes;
     SeriesCol* const scol = reinterpret_cast<SeriesCol*>(sr_smem + (size_t)SR_STAGES * stage_bytes);
     SeriesTerms* const sterm = reinterpret_cast<SeriesTerms*>(scol + NB);
-    float4* const sred = reinterpret_cast<float4*>(sterm + NB);  // [128]: partial sums of the second column half
-    uint32_t* const sbits = reinterpret_cast<uint32_t*>(sred + SR_M);
+    float4* const sred = reinterpret_cast<float4*>(sterm + NB);  // [parts - 1][128]: partial sums of the other column parts
+    uint32_t* const sbits = reinterpret_cast<uint32_t*>(sred + (SR_EPI_PARTS - 1) * SR_M);
     const int bstride = series_bits_stride(p.N);
     uint64_t* const bars = reinterpret_cast<uint64_t*>(sbits + (size_t)SR_M * bstride + (((size_t)SR_M * bstride) & 1));
     uint64_t* const full = bars;
@@ -355,16 +351,18 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
     uint32_t* const tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * SR_STAGES + 1);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+#ifdef NQS_SERIES_TIMELINE
+    long long stamp[6] = {0, 0, 0, 0, 0, 0};
+#endif
+    NQS_STAMP(0);
     const int nt = blockIdx.x % p.nNT;
     const long long mt = blockIdx.x / p.nNT;
     const int nJC = p.nJC;
-    const int CS = p.CS, rank = nt % CS;  // cluster = CS consecutive column tiles of this sample tile
-    const uint16_t cmask = (uint16_t)((1u << CS) - 1u);
 
     if (tid == 0) {
         for (int s = 0; s < SR_STAGES; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], (uint32_t)CS);  // a stage is free when every CTA of the cluster has consumed it
+            mbar_init(&empty[s], 1);
         }
         mbar_init(t_full, 1);
         fence_mbar_init();
@@ -372,9 +370,9 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
     if (warp == 1) tmem_alloc(tmem_slot, 512);
     tc_fence_before();
     __syncthreads();
-    if (CS > 1) cluster_sync_all();  // every CTA's barriers exist before a peer's copy or commit can reach them
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    NQS_STAMP(1);
 
     if (warp == 0) {
         if (lane == 0) {
@@ -385,13 +383,7 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 mbar_wait(&empty[s], ((kc / SR_STAGES) & 1) ^ 1);
                 unsigned char* const st = sr_smem + (size_t)s * stage_bytes;
                 mbar_expect_tx(&full[s], stage_bytes);
-                const unsigned char* srcA = reinterpret_cast<const unsigned char*>(gA + (long long)kc * SR_PLANES * SR_A_PLANE_U4);
-                if (CS == 1) {
-                    bulk_g2s(st, srcA, SR_A_STAGE_BYTES, &full[s]);
-                } else {  // this CTA fetches its 1/CS of the A planes and multicasts it to the whole cluster
-                    const uint32_t slice = SR_A_STAGE_BYTES / (uint32_t)CS;
-                    bulk_g2s_multicast(st + (size_t)rank * slice, srcA + (size_t)rank * slice, slice, &full[s], cmask);
-                }
+                bulk_g2s(st, gA + (long long)kc * SR_PLANES * SR_A_PLANE_U4, SR_A_STAGE_BYTES, &full[s]);
                 bulk_g2s(st + SR_A_STAGE_BYTES, gB + (long long)kc * SR_PLANES * (2 * NB), b_stage_bytes, &full[s]);
             }
         }
@@ -422,24 +414,23 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 cprod(2, 0, d_or, d_oi, 1u);      // t.lo T.hi
                 cprod(6, 6, d_or, d_oi, 1u);      // t^3 T^3 / 3
                 cprod(4, 4, d_er, d_ei, first);   // t^2 T^2 / 2
-                if (CS == 1) tc_commit(&empty[s]);
-                else tc_commit_multicast(&empty[s], cmask);
+                tc_commit(&empty[s]);
             }
             tc_commit(t_full);
         }
     } else {
-        // ---------------- epilogue warps: TMEM lane group = warp % 4, column half = (warp - 2) / 4
-        const int lane_grp = warp & 3, half = (warp - 2) >> 2;
+        // ---------------- epilogue warps: TMEM lane group = warp % 4, column part = (warp - 2) / 4
+        const int lane_grp = warp & 3, part = (warp - 2) >> 2;
         const int row = lane_grp * 32 + lane;
         const long long b = mt * SR_M + row;
-        // while the MMAs run: column records -> smem (second half), bit-packed spins of the own row (first half)
-        if (half == 1) {
+        // while the MMAs run: column records -> smem (part 1), bit-packed spins of the own row (part 0)
+        if (part == 1) {
             const int et = tid - 64 - 128;
             for (int idx = et; idx < NB * 4; idx += 128)
                 reinterpret_cast<uint4*>(scol)[idx] = reinterpret_cast<const uint4*>(p.cols + (long long)nt * NB)[idx];
             for (int idx = et; idx < NB * 2; idx += 128)
                 reinterpret_cast<uint4*>(sterm)[idx] = reinterpret_cast<const uint4*>(p.terms + (long long)nt * NB)[idx];
-        } else {
+        } else if (part == 0) {
             uint32_t* const wbits = sbits + (size_t)row * bstride;
             const int nW = (p.N + 31) / 32;
             if (b >= p.B) {
@@ -470,13 +461,13 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 }
             }
         }
-        asm volatile("bar.sync 1, 256;" ::: "memory");  // records and bits visible to the eight epilogue warps
+        asm volatile("bar.sync 1, %0;" ::"n"(SR_EPI_THREADS) : "memory");  // records and bits visible to the epilogue warps
         const uint32_t* const mybits = sbits + (size_t)row * bstride;
         auto spin_or_one = [&](int z) { return z >= 0 ? spin_from_bits(mybits, z) : 1.f; };
         float er_acc = 0.f, ei_acc = 0.f, eps = 0.f;
-        if (nt == 0) {  // diagonal terms (empty flip set): d = sum_t c_t s[z0] s[z1]; the halves split the list
+        if (nt == 0) {  // diagonal terms (empty flip set): d = sum_t c_t s[z0] s[z1]; the parts split the list
 #pragma unroll 4
-            for (int t = half; t < p.H.Td; t += 2) {
+            for (int t = part; t < p.H.Td; t += SR_EPI_PARTS) {
                 float f = spin_or_one(p.H.diag_z0[t]) * spin_or_one(p.H.diag_z1[t]);
                 if (p.H.has_zx)
                     for (int x = p.H.diag_zx_off[t]; x < p.H.diag_zx_off[t + 1]; ++x) f *= spin_from_bits(mybits, p.H.diag_zx[x]);
@@ -485,23 +476,27 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 ei_acc = fmaf(cc.y, f, ei_acc);
             }
         }
+        NQS_STAMP(2);
         const float4 rn = p.rown[b];
         const float rmax = p.rowmax[b];
-        const int nBatch = NB / 16, b_lo = half ? (nBatch + 1) / 2 : 0, b_hi = half ? nBatch : (nBatch + 1) / 2;
-        mbar_wait(t_full, 0);
+        const int nBatch = NB / SR_EPI_COLS;
+        const int b_lo = nBatch * part / SR_EPI_PARTS, b_hi = nBatch * (part + 1) / SR_EPI_PARTS;
+        mbar_wait_sleep(t_full, 0, 256);
+        NQS_STAMP(3);
         tc_fence_after();
         const uint32_t tbase = tmem_base + ((uint32_t)(lane_grp * 32) << 16);
 #pragma unroll 1
         for (int bt = b_lo; bt < b_hi; ++bt) {
-            const int c0 = bt * 16;
-            float vor[16], voi[16], ver[16], vei[16];
-            tmem_ld16(tbase + (uint32_t)c0, vor);
-            tmem_ld16(tbase + (uint32_t)(NB + c0), voi);
-            tmem_ld16(tbase + (uint32_t)(2 * NB + c0), ver);
-            tmem_ld16(tbase + (uint32_t)(3 * NB + c0), vei);
-            // branch-free per column, so that the 16 columns of a batch overlap in the pipeline
+            const int c0 = bt * SR_EPI_COLS;
+            float vor[SR_EPI_COLS], voi[SR_EPI_COLS], ver[SR_EPI_COLS], vei[SR_EPI_COLS];
+            tmem_ld8_nowait(tbase + (uint32_t)c0, vor);
+            tmem_ld8_nowait(tbase + (uint32_t)(NB + c0), voi);
+            tmem_ld8_nowait(tbase + (uint32_t)(2 * NB + c0), ver);
+            tmem_ld8_nowait(tbase + (uint32_t)(3 * NB + c0), vei);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            // branch-free per column, so that the columns of a batch overlap in the pipeline
 #pragma unroll
-            for (int q = 0; q < 16; ++q) {
+            for (int q = 0; q < SR_EPI_COLS; ++q) {
                 const SeriesCol cr = scol[c0 + q];
                 const SeriesTerms tm = sterm[c0 + q];
                 const float si = spin_from_bits(mybits, cr.site);
@@ -550,17 +545,27 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 eps += live ? bound : 0.f;
             }
         }
-        // the second column half hands its sums to the first, which owns the row's output
-        if (half == 1) sred[row] = make_float4(er_acc, ei_acc, eps, 0.f);
-        asm volatile("bar.sync 1, 256;" ::: "memory");
-        if (half == 0 && b < p.B) {
-            const float4 o = sred[row];
-            p.partial[b * p.nNT + nt] = make_float4(er_acc + o.x, ei_acc + o.y, eps + o.z, 0.f);
+        NQS_STAMP(4);
+        // the other column parts hand their sums to part 0, which owns the row's output (fixed order: deterministic)
+        if (part > 0) sred[(part - 1) * SR_M + row] = make_float4(er_acc, ei_acc, eps, 0.f);
+        asm volatile("bar.sync 1, %0;" ::"n"(SR_EPI_THREADS) : "memory");
+        if (part == 0 && b < p.B) {
+#pragma unroll
+            for (int q = 0; q < SR_EPI_PARTS - 1; ++q) {
+                const float4 o = sred[q * SR_M + row];
+                er_acc += o.x, ei_acc += o.y, eps += o.z;
+            }
+            p.partial[b * p.nNT + nt] = make_float4(er_acc, ei_acc, eps, 0.f);
         }
     }
+#ifdef NQS_SERIES_TIMELINE
+    if (p.timeline && tid == 64) {
+        NQS_STAMP(5);
+        for (int k = 0; k < 6; ++k) p.timeline[(long long)blockIdx.x * 8 + k] = stamp[k];
+    }
+#endif
     tc_fence_before();
     __syncthreads();
-    if (CS > 1) cluster_sync_all();  // no CTA leaves while a peer's commit may still arrive on its barriers
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc(tmem_base, 512);

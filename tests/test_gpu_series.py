@@ -146,21 +146,6 @@ def test_auto_threshold(nqs):
     assert took["path"] == "series" and not took["guard_failed"]
 
 
-def test_cluster_multicast_is_bit_identical(nqs):
-    """NQS_OPT_SERIES_CLUSTER: the column tiles of a sample tile as a thread-block cluster sharing the t^k planes by
-    multicast (2 and 4 CTAs) give the same bits as independent CTAs."""
-    w = wl.make_config(5, B=1000)  # 4 column tiles
-    out = {}
-    for cs in (1, 2, 4):
-        nqs.set_option("series_cluster", cs)
-        try:
-            out[cs], _, took = run(nqs, w, "series_only")
-        finally:
-            nqs.set_option("series_cluster", 0)
-        assert took["path"] == "series" and not took["guard_failed"]
-    assert np.array_equal(out[1], out[2]) and np.array_equal(out[1], out[4])
-
-
 def test_series_with_the_simt_theta_kernel(nqs, oracle):
     """N > 512 is outside the tensor-core theta kernel: theta_kernel (FP32 SIMT) writes tanh(theta) and
     series_pack_kernel builds the FP16 planes and the row norms from it; also through the NQS_OPT_THETA_PATH switch
