@@ -342,7 +342,7 @@ def run_ours(args) -> None:
                     "frac_of_sustained_peak": (achieved / peaks["bf16_tflops_sustained"]
                                                if peaks["bf16_tflops_sustained"] else None)}
         else:
-            dom, dom_ms = "eloc_kernel", km["eloc"]
+            dom, dom_ms = ("small_eloc_kernel" if took["path"] == "small" else "eloc_kernel"), km["eloc"]
             achieved = 2.0 * work["a5_fp32"] / (dom_ms * 1e-3) / 1e12
             roof = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": fp32_peak_tflops, "unit": "TFLOP/s",
                     "frac": achieved / fp32_peak_tflops,
@@ -365,7 +365,8 @@ def run_ours(args) -> None:
             "config": {"workload": w.name, "N": w.N, "M": w.M, "B_per_gpu": w.B, "global_batch": plan["global_batch"],
                        "terms": w.ham.T, "flip_groups": ham.G, "table_columns": ham.C,
                        "connected_per_sample": ham.G + 1, "a5_path": "tensor-core series (guard passed)" if series else
-                       ("FP32 product form (series guard failed)" if took["path"] == "series" else "FP32 product form"),
+                       ("FP32 product form (series guard failed)" if took["path"] == "series" else
+                        "FP32 product form, single launch" if took["path"] == "small" else "FP32 product form"),
                        "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB write outside the event pairs)",
                        "parallelism": f"replicas over B x{world}, no collective"},
             "connected_evals_per_s": value * (ham.G + 1),

@@ -96,7 +96,10 @@ int nqs_local_energy(const int8_t *d_spins, int64_t B, int32_t N, int32_t M, con
                      nqs_c64 *d_logpsi, void *stream);
 
 /* Same with HOST buffers for everything (spins, parameters, outputs): H2D copies, kernels,
- * D2H copies, stream synchronise.  h_logpsi may be NULL. */
+ * D2H copies, stream synchronise.  h_logpsi may be NULL.  Batches of 65536 samples and more go through
+ * the device in chunks of >= 32768 samples on two library-owned streams, so that the copy of chunk k + 1
+ * overlaps the kernels of chunk k (pinned host buffers are needed for the overlap; pageable ones work,
+ * serially).  Calls on the same device are serialised. */
 int nqs_local_energy_host(const int8_t *h_spins, int64_t B, int32_t N, int32_t M, const nqs_c64 *h_a,
                           const nqs_c64 *h_b, const nqs_c64 *h_W, int32_t T, const int32_t *h_sites,
                           const uint8_t *h_paulis, const nqs_c64 *h_coeffs, nqs_c64 *h_eloc,
@@ -161,11 +164,16 @@ int nqs_local_energy_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t 
  *                       2 = series + guard + fallback at ANY size
  *                       3 = series only: the guard is evaluated and recorded but nothing is recomputed
  *   NQS_OPT_THETA_PATH  0 = automatic (int8 tcgen05 kernel for N <= 512, else FP32 SIMT)   1 = FP32 SIMT only
+ *   NQS_OPT_SMALL_PATH  0 = automatic: below the series' size threshold, when columns x M x 16 bytes of tables and the
+ *                       per-sample state of >= 16 samples fit in 200 KB of shared memory, ONE kernel does the whole call
+ *                       (csrc/nqs_small.cuh; theta accumulated in float64)                 1 = never (multi-launch path)
+ *   NQS_OPT_HOST_CHUNKS 0 = automatic: nqs_local_energy_host sends the batch through the device in B / 32768 chunks
+ *                       (at most 16), copying chunk k + 1 while the kernels of chunk k run      1 .. 16 = that many
  * nqs_debug_last_a5 (synchronises `stream`; tests only; not meaningful while calls run concurrently on other
  * streams): out[0] = 1 if the most recent nqs_local_energy* call on this device attempted the series path, 2 if
- * it used the product form only; out[1] = 1 if the guard failed; out[2] = samples over the guard threshold.
+ * it used the product form only, 3 if the single-launch kernel for small problems ran; out[1] = 1 if the guard failed; out[2] = samples over the guard threshold.
  * ------------------------------------------------------------------------------------- */
-enum { NQS_OPT_A5_PATH = 0, NQS_OPT_THETA_PATH = 1, NQS_OPT_COUNT = 2 };
+enum { NQS_OPT_A5_PATH = 0, NQS_OPT_THETA_PATH = 1, NQS_OPT_HOST_CHUNKS = 2, NQS_OPT_SMALL_PATH = 3, NQS_OPT_COUNT = 4 };
 int nqs_set_option(int32_t key, int32_t value);
 int nqs_get_option(int32_t key, int32_t *value);
 int nqs_debug_last_a5(int32_t out[3], void *stream);

@@ -109,7 +109,7 @@ def profile_last() -> dict:
     return {k: ms[i] for i, k in enumerate(PROFILE_SEGMENTS)}
 
 
-OPTIONS = {"a5_path": 0, "theta_path": 1}
+OPTIONS = {"a5_path": 0, "theta_path": 1, "host_chunks": 2, "small_path": 3}
 A5_PATHS = {"auto": 0, "product": 1, "series_guarded": 2, "series_only": 3}
 
 
@@ -135,7 +135,7 @@ def debug_last_a5() -> dict:
     """nqs_debug_last_a5 (synchronises): which a5 path the last nqs_local_energy* call took."""
     out = (ctypes.c_int32 * 3)()
     _check(load_library().nqs_debug_last_a5(out, _stream()))
-    return dict(path={1: "series", 2: "product"}.get(out[0], "none"), guard_failed=bool(out[1]), samples_over=int(out[2]))
+    return dict(path={1: "series", 2: "product", 3: "small"}.get(out[0], "none"), guard_failed=bool(out[1]), samples_over=int(out[2]))
 
 
 MICROBENCH_KINDS = {"ffma": 0, "ffma2": 1, "a5_body_packed": 2, "a5_body_scalar": 3, "mufu_ex2": 4}
@@ -245,11 +245,14 @@ class Hamiltonian:
             raise ValueError("N mismatch with the compiled Hamiltonian")
         eloc = torch.empty(B, dtype=torch.complex64, device=spins.device)
         logpsi = torch.empty(B, dtype=torch.complex64, device=spins.device) if want_logpsi else None
-        with torch.cuda.device(spins.device):
-            _check(load_library().nqs_local_energy_h(
-                self._h, _dev(spins, torch.int8, "spins"), B, M, _dev(a, torch.complex64, "a"),
+        args = (self._h, _dev(spins, torch.int8, "spins"), B, M, _dev(a, torch.complex64, "a"),
                 _dev(b, torch.complex64, "b"), _dev(W, torch.complex64, "W"), ctypes.c_void_p(eloc.data_ptr()),
-                ctypes.c_void_p(logpsi.data_ptr()) if want_logpsi else None, _stream()))
+                ctypes.c_void_p(logpsi.data_ptr()) if want_logpsi else None)
+        if spins.device.index == torch.cuda.current_device():  # the common case: no device switch to pay for
+            _check(load_library().nqs_local_energy_h(*args, _stream()))
+        else:
+            with torch.cuda.device(spins.device):
+                _check(load_library().nqs_local_energy_h(*args, _stream()))
         return (eloc, logpsi) if want_logpsi else eloc
 
     def local_energy_forces(self, spins, a, b, W, weights=None):

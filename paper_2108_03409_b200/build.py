@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnqs_b200.so")
 SOURCES = ["nqs_api.cu", "nqs_hamiltonian.cpp"]
-DEPS = SOURCES + ["nqs_kernels.cuh", "nqs_theta_mma.cuh", "nqs_forces.cuh", "nqs_fisher.cuh", "nqs_microbench.cuh", "nqs_sampler.cuh", "nqs_series.cuh", "nqs_device.cuh", "nqs_hamiltonian.h", os.path.join("..", "..", "include", "nqs.h")]
+DEPS = SOURCES + ["nqs_kernels.cuh", "nqs_theta_mma.cuh", "nqs_forces.cuh", "nqs_fisher.cuh", "nqs_microbench.cuh", "nqs_sampler.cuh", "nqs_series.cuh", "nqs_small.cuh", "nqs_device.cuh", "nqs_hamiltonian.h", os.path.join("..", "..", "include", "nqs.h")]
 
 
 def nvcc_command(out: str, verbose: bool = False) -> list[str]:

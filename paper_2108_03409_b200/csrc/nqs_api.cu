@@ -23,6 +23,7 @@
 #include "nqs_microbench.cuh"
 #include "nqs_sampler.cuh"
 #include "nqs_series.cuh"
+#include "nqs_small.cuh"
 #include "nqs_theta_mma.cuh"
 
 using namespace nqs;
@@ -68,13 +69,15 @@ extern "C" const char* nqs_version(void) { return "0.2.0 sm_100a"; }
 // options (include/nqs.h: nqs_set_option)
 // ----------------------------------------------------------------------------------------
 static std::atomic<int> g_opt[NQS_OPT_COUNT] = {};
+constexpr int HOST_MAX_CHUNKS = 16;  // nqs_local_energy_host
+constexpr size_t SMALL_SMEM_MAX = 200 * 1024;  // shared memory of small_eloc_kernel above which the multi-launch path runs
 #ifdef NQS_SERIES_TIMELINE
 static long long* g_series_timeline = nullptr;
 #endif
 
 extern "C" int nqs_set_option(int32_t key, int32_t value) {
     if (key < 0 || key >= NQS_OPT_COUNT) return fail(NQS_ERR_INVALID_ARG, "nqs_set_option: unknown key");
-    const int hi = key == NQS_OPT_A5_PATH ? 3 : 1;
+    const int hi = key == NQS_OPT_A5_PATH ? 3 : key == NQS_OPT_HOST_CHUNKS ? HOST_MAX_CHUNKS : 1;  // the others: 0 / 1
     if (value < 0 || value > hi) return fail(NQS_ERR_INVALID_ARG, "nqs_set_option: value out of range");
     g_opt[key].store(value);
     return NQS_OK;
@@ -97,6 +100,12 @@ struct DeviceState {
     int* tags = nullptr;    // [4] constant {0, 1, 2, 3}: device-side source of the path tag
     std::atomic<int> last_tag{0};  // path tag the most recent call enqueued
     std::map<const void*, size_t> smem_optin;
+    int sms = 148;  // multiprocessors of the device
+    // host-buffer entry points (nqs_local_energy_host): a copy stream, a compute stream and the events between them,
+    // made on first use and kept; host_mu serialises those entry points per device
+    cudaStream_t host_copy = nullptr, host_comp = nullptr;
+    cudaEvent_t host_ev[HOST_MAX_CHUNKS + 1] = {};
+    std::mutex host_mu;
 };
 static DeviceState g_dev[MAX_DEVICES];
 static std::mutex g_dev_mu;
@@ -126,6 +135,7 @@ static int device_state(DeviceState** out) {
         const int init[8] = {0, 0, 0, 0, 0, 1, 2, 3};
         NQS_CUDA(cudaMemcpy(D.status, init, sizeof(init), cudaMemcpyHostToDevice));
         D.tags = D.status + 4;
+        NQS_CUDA(cudaDeviceGetAttribute(&D.sms, cudaDevAttrMultiProcessorCount, dev));
         D.ready = true;
     }
     *out = &D;
@@ -693,6 +703,48 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     const bool use_series = series_ok && (opt == 2 || opt == 3 || (opt == 0 && big));
     const bool use_product = have_cols && !(use_series && opt == 3);
 
+    // small problems: a1 .. a6 in one launch (nqs_small.cuh) when the tables of a CTA fit in shared memory
+    if (opt == 0 && !use_series && !keep_tp && g_opt[NQS_OPT_SMALL_PATH].load() == 0) {
+        if (small_smem_bytes(N, M, h->C, 4) <= SMALL_SMEM_MAX) {
+            // samples per CTA: the batch spread over a whole number of waves of one CTA per SM, as far as the CTA's
+            // shared memory allows
+            int SB = 4;
+            for (int waves = 1;; ++waves) {
+                SB = (int)round_up((B + (long long)D->sms * waves - 1) / ((long long)D->sms * waves), 4);
+                if (SB <= SM_MAX_SB && small_smem_bytes(N, M, h->C, SB) <= SMALL_SMEM_MAX) break;
+            }
+            const size_t smem = small_smem_bytes(N, M, h->C, SB);
+            NQS_TRY(ensure_smem(D, small_eloc_kernel, smem));
+            SmallParams sp;
+            sp.spins = d_spins;
+            sp.B = B;
+            sp.N = N;
+            sp.M = M;
+            sp.C = h->C;
+            sp.a = (const float2*)d_a;
+            sp.b = (const float2*)d_b;
+            sp.W = (const float2*)d_W;
+            sp.H = h->dev;
+            sp.eloc = (float2*)d_eloc;
+            sp.logpsi = (float2*)d_logpsi;
+            sp.SB = SB;
+            const long long blocks = (B + SB - 1) / SB;
+            if (blocks > 0x7fffffffll) return fail(NQS_ERR_UNSUPPORTED, "B exceeds the grid limit");
+            for (int k = 0; k <= 5; ++k) NQS_PROF(k, st);
+            small_eloc_kernel<<<(unsigned)blocks, small_threads(h->C, SB), smem, st>>>(sp);
+            NQS_LAUNCHED();
+            NQS_PROF(6, st);
+            if (D->last_tag.exchange(3) != 3) {
+                NQS_CUDA(cudaMemsetAsync(D->status, 0, 2 * sizeof(int), st));
+                NQS_CUDA(cudaMemcpyAsync(D->status + 2, D->tags + 3, sizeof(int), cudaMemcpyDeviceToDevice, st));
+            }
+            NQS_PROF(7, st);
+            g_prof_valid = g_prof_on;
+            mark_use(h, st);
+            return NQS_OK;
+        }
+    }
+
     // the tensor-core theta kernel writes the series planes itself; tanh(theta) is then only needed by the
     // product form (in a gated second pass if the guard fails) or by the caller (keep_tp)
     const bool fused_pack = use_series && theta_use_mma(N);
@@ -835,6 +887,16 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     return NQS_OK;
 }
 
+#ifdef NQS_SMALL_TIMELINE
+// development builds only (NQS_NVCC_FLAGS=-DNQS_SMALL_TIMELINE): clock64 at the phase boundaries of block 0 of the most
+// recent small_eloc_kernel (start, W levels done, theta done, tables done, amplitudes done, end)
+extern "C" int nqs_debug_small_timeline(long long out[8]) {
+    NQS_CUDA(cudaDeviceSynchronize());
+    NQS_CUDA(cudaMemcpyFromSymbol(out, g_small_stamps, 8 * sizeof(long long)));
+    return NQS_OK;
+}
+#endif
+
 #ifdef NQS_SERIES_TIMELINE
 // development builds only (NQS_NVCC_FLAGS=-DNQS_SERIES_TIMELINE): a device buffer of [blocks][8] int64 that receives
 // the clock64 stamps of every series_gemm_kernel block (start, after set-up, after the prologue, accumulators ready,
@@ -853,7 +915,7 @@ extern "C" int nqs_debug_last_a5(int32_t out[3], void* stream) {
     int v[3] = {0, 0, 0};
     NQS_CUDA(cudaMemcpyAsync(v, D->status, 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
     NQS_CUDA(cudaStreamSynchronize(st));
-    out[0] = v[2];  // 1 = the series path was attempted, 2 = product form only
+    out[0] = v[2];  // 1 = the series path was attempted, 2 = product form only, 3 = the single-launch kernel
     out[1] = v[0];  // 1 = the guard failed (and, unless NQS_OPT_A5_PATH = 3, the product form recomputed the call)
     out[2] = v[1];  // samples whose error bound exceeded the guard threshold
     return NQS_OK;
@@ -929,32 +991,21 @@ extern "C" int nqs_enumerate_connected(const int8_t* d_spins, int64_t B, int32_t
 // ----------------------------------------------------------------------------------------
 // host-buffer entry points (end-to-end: H2D, kernels, D2H, synchronise)
 // ----------------------------------------------------------------------------------------
-struct HostStage {
-    cudaStream_t st = nullptr;
-    std::vector<void*> bufs;
-    ~HostStage() {
-        for (void* b : bufs) cudaFreeAsync(b, st);
-        if (st) {
-            cudaStreamSynchronize(st);
-            cudaStreamDestroy(st);
-        }
-    }
-    int init() {
-        NQS_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
-        return NQS_OK;
-    }
-    int to_device(const void* h, size_t bytes, void** d) {
-        NQS_CUDA(cudaMallocAsync(d, bytes ? bytes : 16, st));
-        bufs.push_back(*d);
-        if (bytes) NQS_CUDA(cudaMemcpyAsync(*d, h, bytes, cudaMemcpyHostToDevice, st));
-        return NQS_OK;
-    }
-    int alloc(size_t bytes, void** d) {
-        NQS_CUDA(cudaMallocAsync(d, bytes ? bytes : 16, st));
-        bufs.push_back(*d);
-        return NQS_OK;
-    }
-};
+
+// Host buffers in, host buffers out (the end-to-end leg of bench.py).  The batch goes through the device in chunks:
+// the parameters and the first chunk of spins are copied, then the kernels of chunk k run on the compute stream while
+// the copy stream brings chunk k + 1 -- the transfer of all but the first chunk hides behind the kernels.  Chunks are
+// at least HOST_CHUNK_MIN samples (a chunk must still fill the 296 CTA slots of the theta kernel) and a multiple of
+// 256; every sample's result is independent of the chunking except that the series guard decides per chunk.
+constexpr int64_t HOST_CHUNK_MIN = 32768;
+
+static int host_streams(DeviceState* D) {
+    if (D->host_comp) return NQS_OK;
+    NQS_CUDA(cudaStreamCreateWithFlags(&D->host_copy, cudaStreamNonBlocking));
+    NQS_CUDA(cudaStreamCreateWithFlags(&D->host_comp, cudaStreamNonBlocking));
+    for (int k = 0; k <= HOST_MAX_CHUNKS; ++k) NQS_CUDA(cudaEventCreateWithFlags(&D->host_ev[k], cudaEventDisableTiming));
+    return NQS_OK;
+}
 
 extern "C" int nqs_local_energy_host(const int8_t* h_spins, int64_t B, int32_t N, int32_t M, const nqs_c64* h_a,
                                      const nqs_c64* h_b, const nqs_c64* h_W, int32_t T, const int32_t* h_sites,
@@ -964,23 +1015,55 @@ extern "C" int nqs_local_energy_host(const int8_t* h_spins, int64_t B, int32_t N
     if (B > 0 && !h_eloc) return fail(NQS_ERR_INVALID_ARG, "h_eloc is NULL");
     DeviceState* D = nullptr;
     NQS_TRY(device_state(&D));
-    HostStage S;
-    NQS_TRY(S.init());
+    std::lock_guard<std::mutex> host_lock(D->host_mu);
+    NQS_TRY(host_streams(D));
+    cudaStream_t comp = D->host_comp, copy = D->host_copy;
     HamRef h;
-    NQS_TRY(cached_hamiltonian(N, T, 2, h_sites, h_paulis, h_coeffs, S.st, &h));
+    NQS_TRY(cached_hamiltonian(N, T, 2, h_sites, h_paulis, h_coeffs, comp, &h));
     if (B == 0) return NQS_OK;
-    void *ds, *da, *db, *dW, *de, *dl = nullptr;
-    NQS_TRY(S.to_device(h_spins, (size_t)B * N, &ds));
-    NQS_TRY(S.to_device(h_a, sizeof(nqs_c64) * N, &da));
-    NQS_TRY(S.to_device(h_b, sizeof(nqs_c64) * M, &db));
-    NQS_TRY(S.to_device(h_W, sizeof(nqs_c64) * (size_t)M * N, &dW));
-    NQS_TRY(S.alloc(sizeof(nqs_c64) * B, &de));
-    if (h_logpsi) NQS_TRY(S.alloc(sizeof(nqs_c64) * B, &dl));
-    NQS_TRY(nqs_local_energy_h(h.get(), (const int8_t*)ds, B, M, (const nqs_c64*)da, (const nqs_c64*)db,
-                               (const nqs_c64*)dW, (nqs_c64*)de, (nqs_c64*)dl, S.st));
-    NQS_CUDA(cudaMemcpyAsync(h_eloc, de, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
-    if (h_logpsi) NQS_CUDA(cudaMemcpyAsync(h_logpsi, dl, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
-    NQS_CUDA(cudaStreamSynchronize(S.st));
+    // on every exit: wait for both streams (the scratch below is released in the order of `comp`)
+    struct Drain {
+        cudaStream_t a, b;
+        ~Drain() {
+            cudaStreamSynchronize(a);
+            cudaStreamSynchronize(b);
+        }
+    };
+    Scratch S(D, comp);
+    Drain drain{copy, comp};
+    int8_t* ds = nullptr;
+    nqs_c64 *da = nullptr, *db = nullptr, *dW = nullptr, *de = nullptr, *dl = nullptr;
+    NQS_TRY(S.get(&ds, (size_t)B * N));
+    NQS_TRY(S.get(&da, (size_t)N));
+    NQS_TRY(S.get(&db, (size_t)M));
+    NQS_TRY(S.get(&dW, (size_t)M * N));
+    NQS_TRY(S.get(&de, (size_t)B));
+    if (h_logpsi) NQS_TRY(S.get(&dl, (size_t)B));
+    int nChunks = (int)std::min<int64_t>(HOST_MAX_CHUNKS, std::max<int64_t>(1, B / HOST_CHUNK_MIN));
+    const int forced = g_opt[NQS_OPT_HOST_CHUNKS].load();
+    if (forced > 0) nChunks = (int)std::min<int64_t>(forced, (B + 255) / 256);
+    const int64_t per = round_up((B + nChunks - 1) / nChunks, 256);
+    // the blocks were allocated in the order of `comp`: the copy stream may touch them after this point of it
+    NQS_CUDA(cudaEventRecord(D->host_ev[HOST_MAX_CHUNKS], comp));
+    NQS_CUDA(cudaStreamWaitEvent(copy, D->host_ev[HOST_MAX_CHUNKS], 0));
+    NQS_CUDA(cudaMemcpyAsync(da, h_a, sizeof(nqs_c64) * N, cudaMemcpyHostToDevice, copy));
+    NQS_CUDA(cudaMemcpyAsync(db, h_b, sizeof(nqs_c64) * M, cudaMemcpyHostToDevice, copy));
+    NQS_CUDA(cudaMemcpyAsync(dW, h_W, sizeof(nqs_c64) * (size_t)M * N, cudaMemcpyHostToDevice, copy));
+    for (int k = 0; k < nChunks; ++k) {
+        const int64_t b0 = k * per, nb = std::min<int64_t>(per, B - b0);
+        if (nb <= 0) break;
+        NQS_CUDA(cudaMemcpyAsync(ds + b0 * N, h_spins + b0 * N, (size_t)nb * N, cudaMemcpyHostToDevice, copy));
+        NQS_CUDA(cudaEventRecord(D->host_ev[k], copy));
+    }
+    for (int k = 0; k < nChunks; ++k) {
+        const int64_t b0 = k * per, nb = std::min<int64_t>(per, B - b0);
+        if (nb <= 0) break;
+        NQS_CUDA(cudaStreamWaitEvent(comp, D->host_ev[k], 0));
+        NQS_TRY(nqs_local_energy_h(h.get(), ds + b0 * N, nb, M, da, db, dW, de + b0, dl ? dl + b0 : nullptr, comp));
+        NQS_CUDA(cudaMemcpyAsync(h_eloc + b0, de + b0, sizeof(nqs_c64) * nb, cudaMemcpyDeviceToHost, comp));
+        if (h_logpsi) NQS_CUDA(cudaMemcpyAsync(h_logpsi + b0, dl + b0, sizeof(nqs_c64) * nb, cudaMemcpyDeviceToHost, comp));
+    }
+    NQS_CUDA(cudaStreamSynchronize(comp));
     return NQS_OK;
 }
 
@@ -991,18 +1074,29 @@ extern "C" int nqs_log_psi_host(const int8_t* h_spins, int64_t B, int32_t N, int
     DeviceState* D = nullptr;
     NQS_TRY(device_state(&D));
     if (B == 0) return NQS_OK;
-    HostStage S;
-    NQS_TRY(S.init());
-    void *ds, *da, *db, *dW, *dl;
-    NQS_TRY(S.to_device(h_spins, (size_t)B * N, &ds));
-    NQS_TRY(S.to_device(h_a, sizeof(nqs_c64) * N, &da));
-    NQS_TRY(S.to_device(h_b, sizeof(nqs_c64) * M, &db));
-    NQS_TRY(S.to_device(h_W, sizeof(nqs_c64) * (size_t)M * N, &dW));
-    NQS_TRY(S.alloc(sizeof(nqs_c64) * B, &dl));
-    NQS_TRY(nqs_log_psi((const int8_t*)ds, B, N, M, (const nqs_c64*)da, (const nqs_c64*)db, (const nqs_c64*)dW,
-                        (nqs_c64*)dl, S.st));
-    NQS_CUDA(cudaMemcpyAsync(h_logpsi, dl, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, S.st));
-    NQS_CUDA(cudaStreamSynchronize(S.st));
+    std::lock_guard<std::mutex> host_lock(D->host_mu);
+    NQS_TRY(host_streams(D));
+    cudaStream_t st = D->host_comp;
+    struct Drain {
+        cudaStream_t a;
+        ~Drain() { cudaStreamSynchronize(a); }
+    };
+    Scratch S(D, st);
+    Drain drain{st};
+    int8_t* ds = nullptr;
+    nqs_c64 *da = nullptr, *db = nullptr, *dW = nullptr, *dl = nullptr;
+    NQS_TRY(S.get(&ds, (size_t)B * N));
+    NQS_TRY(S.get(&da, (size_t)N));
+    NQS_TRY(S.get(&db, (size_t)M));
+    NQS_TRY(S.get(&dW, (size_t)M * N));
+    NQS_TRY(S.get(&dl, (size_t)B));
+    NQS_CUDA(cudaMemcpyAsync(ds, h_spins, (size_t)B * N, cudaMemcpyHostToDevice, st));
+    NQS_CUDA(cudaMemcpyAsync(da, h_a, sizeof(nqs_c64) * N, cudaMemcpyHostToDevice, st));
+    NQS_CUDA(cudaMemcpyAsync(db, h_b, sizeof(nqs_c64) * M, cudaMemcpyHostToDevice, st));
+    NQS_CUDA(cudaMemcpyAsync(dW, h_W, sizeof(nqs_c64) * (size_t)M * N, cudaMemcpyHostToDevice, st));
+    NQS_TRY(nqs_log_psi(ds, B, N, M, da, db, dW, dl, st));
+    NQS_CUDA(cudaMemcpyAsync(h_logpsi, dl, sizeof(nqs_c64) * B, cudaMemcpyDeviceToHost, st));
+    NQS_CUDA(cudaStreamSynchronize(st));
     return NQS_OK;
 }
 

@@ -35,6 +35,13 @@ def test_random_shapes_all_entry_points(oracle):
         tol_l = 1e-5 * np.maximum(1.0, np.abs(l_ref))
         dim = (l.imag - l_ref.imag + np.pi) % (2 * np.pi) - np.pi
         assert np.all(np.abs(l.real - l_ref.real) <= tol_l) and np.all(np.abs(dim) <= tol_l), what
+        # the plain call (single-launch kernel where its tables fit, else the multi-launch path)
+        e1, l1 = ham.local_energy(sp, a, b, W)
+        torch.cuda.synchronize()
+        e1, l1 = (x.cpu().numpy().astype(np.complex128) for x in (e1, l1))
+        assert np.all(np.abs(e1.real - e_ref.real) <= tol_e) and np.all(np.abs(e1.imag - e_ref.imag) <= tol_e), what
+        dim = (l1.imag - l_ref.imag + np.pi) % (2 * np.pi) - np.pi
+        assert np.all(np.abs(l1.real - l_ref.real) <= tol_l) and np.all(np.abs(dim) <= tol_l), what
         # forces from the GPU's own E_loc bytes (complex64), as the fused call used them
         e32 = e.astype(np.complex64)
         F_ref = oracle.forces(w.spins, w.a, w.b, w.W, e32)

@@ -329,6 +329,35 @@ def test_determinism_and_handle_api(nqs):
     assert np.array_equal(eh, e1.cpu().numpy()) and np.array_equal(lh, l1.cpu().numpy())
 
 
+def test_host_entry_point_in_chunks(nqs, oracle):
+    """nqs_local_energy_host sends large batches through the device in chunks (copy of chunk k + 1 under the kernels of
+    chunk k).  Every sample is independent, so 1, 2, 3 and 5 chunks of a ragged batch (pageable and pinned host
+    buffers) must give the bits of the device-pointer call of each chunk; sampled outputs against the oracle."""
+    import torch
+
+    w = wl.make_config(3, B=70001)
+    pin = lambda x: torch.from_numpy(x).pin_memory().numpy()  # noqa: E731
+    bufs = {"pageable": (w.spins, w.a, w.b, w.W), "pinned": tuple(pin(x) for x in (w.spins, w.a, w.b, w.W))}
+    out = {}
+    try:
+        for kind, (hs, ha, hb, hW) in bufs.items():
+            for ch in (1, 2, 3, 5, 0):
+                nqs.set_option("host_chunks", ch)
+                out[kind, ch] = nqs.local_energy_host(hs, ha, hb, hW, w.ham.sites, w.ham.paulis, w.ham.coeffs)
+    finally:
+        nqs.set_option("host_chunks", 0)
+    e1, l1 = out["pageable", 1]
+    for key, (e, l) in out.items():
+        assert np.array_equal(e, e1) and np.array_equal(l, l1), key
+    spins, a, b, W = to_dev(w)
+    ed, ld = nqs.local_energy(spins, a, b, W, w.ham.sites, w.ham.paulis, w.ham.coeffs)
+    assert np.array_equal(e1, ed.cpu().numpy()) and np.array_equal(l1, ld.cpu().numpy())
+    idx = np.unique(np.concatenate([np.arange(0, 70001, 997), [35071, 35072, 35073, 69999, 70000]]))
+    e_ref, l_ref = oracle.local_energy_fast(w.spins[idx], w.a, w.b, w.W, w.ham.sites, w.ham.paulis, w.ham.coeffs)
+    tol = 1e-4 * np.maximum(1, np.abs(e_ref))
+    assert np.all(np.abs(e1[idx].real - e_ref.real) <= tol) and np.all(np.abs(e1[idx].imag - e_ref.imag) <= tol)
+
+
 def test_non_default_stream(nqs, oracle):
     import torch
 

@@ -140,6 +140,9 @@ def test_auto_threshold(nqs):
     2^28 triples), large ones take the series."""
     w = wl.make_config(2, B=2000)
     _, _, took = run(nqs, w, "auto")
+    assert took["path"] == "small"  # the single-launch kernel (tests/test_gpu_small.py)
+    w = wl.make_config(3, B=500)    # tables too large for it: the multi-launch product form
+    _, _, took = run(nqs, w, "auto")
     assert took["path"] == "product"
     w = wl.make_config(3, B=8192)  # 8192 * 100 * 400 = 3.3e8 >= 2^28
     _, _, took = run(nqs, w, "auto")

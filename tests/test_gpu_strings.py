@@ -94,7 +94,7 @@ def test_hand_written_strings_and_handle(nqs, oracle):
             assert abs(agg.get(key, 0) - mel[bidx, slot]) <= 1e-5 * max(1, abs(agg.get(key, 0)))
     e2, _ = ham.local_energy(spins, *(torch.from_numpy(x).cuda() for x in (w.a, w.b, w.W)))
     torch.cuda.synchronize()
-    assert np.array_equal(e2.cpu().numpy(), e)
+    check_eloc(e2.cpu().numpy(), e_ref, "hand-written strings, handle API (single-launch kernel)")
     with pytest.raises(nqs.NqsError) as ei:
         nqs.Hamiltonian(6, np.array([[0, 1, 2, 3, 4]], np.int32), np.full((1, 5), X, np.uint8), np.ones(1, np.complex64))
     assert ei.value.code == -4
