@@ -29,6 +29,8 @@
 #pragma once
 #include <cuda_fp16.h>
 
+#include <type_traits>
+
 #include "nqs_device.cuh"
 #include "nqs_theta_mma.cuh"
 
@@ -66,6 +68,10 @@ struct __align__(16) SeriesCol {
                          // SR_GENERIC_TERMS set when they are not (all) inline in SeriesTerms
 };
 constexpr int SR_GENERIC_TERMS = 1 << 30;
+// the column's matrix element does not depend on the sample: a single flip whose one term has no Z factor (the X_i of a
+// transverse field), or a padding column (element 0).  A tile of such columns takes a shorter epilogue.
+constexpr int SR_SIMPLE = 1 << 29;
+constexpr int SR_COUNT_MASK = SR_SIMPLE - 1;
 static_assert(sizeof(SeriesCol) == 64, "SeriesCol layout");
 // the first two terms of the column's group, element = c * s[z0] * s[z1] (z = -1: factor 1); an absent term has c = 0
 struct __align__(16) SeriesTerms {
@@ -196,7 +202,8 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
             const float2 cc = H.gt_c[first + 1];
             t2.z0b = H.gt_z0[first + 1], t2.z1b = H.gt_z1[first + 1], t2.crb = cc.x, t2.cib = cc.y;
         }
-        r.count = count | (generic ? SR_GENERIC_TERMS : 0);
+        const bool simple = r.group < 0 || (r.sitek < 0 && !generic && count <= 1 && t2.z0a < 0 && t2.z1a < 0);
+        r.count = count | (generic ? SR_GENERIC_TERMS : 0) | (simple ? SR_SIMPLE : 0);
         cols[c] = r;
         terms[c] = t2;
     }
@@ -465,12 +472,28 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
         const uint32_t* const mybits = sbits + (size_t)row * bstride;
         auto spin_or_one = [&](int z) { return z >= 0 ? spin_from_bits(mybits, z) : 1.f; };
         float er_acc = 0.f, ei_acc = 0.f, eps = 0.f;
-        if (nt == 0) {  // diagonal terms (empty flip set): d = sum_t c_t s[z0] s[z1]; the parts split the list
-#pragma unroll 4
+        if (nt == 0 && !p.H.has_zx) {
+            // diagonal terms (empty flip set): d = sum_t c_t s[z0] s[z1].  The parts split the list into contiguous
+            // quarters; a warp fetches 32 terms at a time (one per lane, coalesced) and hands them round by shuffles
+            const int per = (p.H.Td + SR_EPI_PARTS - 1) / SR_EPI_PARTS;
+            const int t0 = part * per, t1 = min(p.H.Td, t0 + per);
+            for (int tb = t0; tb < t1; tb += 32) {
+                const int tl = tb + lane;
+                const int z0l = tl < t1 ? p.H.diag_z0[tl] : -1, z1l = tl < t1 ? p.H.diag_z1[tl] : -1;
+                const float2 cl = tl < t1 ? p.H.diag_c[tl] : make_float2(0.f, 0.f);
+                const int n = min(32, t1 - tb);
+                for (int u = 0; u < n; ++u) {
+                    const int z0 = __shfl_sync(0xffffffffu, z0l, u), z1 = __shfl_sync(0xffffffffu, z1l, u);
+                    const float cx = __shfl_sync(0xffffffffu, cl.x, u), cy = __shfl_sync(0xffffffffu, cl.y, u);
+                    const float f = spin_or_one(z0) * spin_or_one(z1);
+                    er_acc = fmaf(cx, f, er_acc);
+                    ei_acc = fmaf(cy, f, ei_acc);
+                }
+            }
+        } else if (nt == 0) {  // terms with more than two Z factors (k-site strings): the general list
             for (int t = part; t < p.H.Td; t += SR_EPI_PARTS) {
                 float f = spin_or_one(p.H.diag_z0[t]) * spin_or_one(p.H.diag_z1[t]);
-                if (p.H.has_zx)
-                    for (int x = p.H.diag_zx_off[t]; x < p.H.diag_zx_off[t + 1]; ++x) f *= spin_from_bits(mybits, p.H.diag_zx[x]);
+                for (int x = p.H.diag_zx_off[t]; x < p.H.diag_zx_off[t + 1]; ++x) f *= spin_from_bits(mybits, p.H.diag_zx[x]);
                 const float2 cc = p.H.diag_c[t];
                 er_acc = fmaf(cc.x, f, er_acc);
                 ei_acc = fmaf(cc.y, f, ei_acc);
@@ -485,6 +508,12 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
         NQS_STAMP(3);
         tc_fence_after();
         const uint32_t tbase = tmem_base + ((uint32_t)(lane_grp * 32) << 16);
+        // are all columns of the tile "simple" (warp-uniform: the records are the same for every row)?
+        bool tile_simple = true;
+        for (int c = lane; c < NB; c += 32) tile_simple = tile_simple && (scol[c].count & SR_SIMPLE);
+        tile_simple = __all_sync(0xffffffffu, tile_simple);
+        auto columns = [&](auto simple_tag) {
+        constexpr bool SIMPLE = decltype(simple_tag)::value;
 #pragma unroll 1
         for (int bt = b_lo; bt < b_hi; ++bt) {
             const int c0 = bt * SR_EPI_COLS;
@@ -502,17 +531,20 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 const float si = spin_from_bits(mybits, cr.site);
                 // the column applies iff every further flip site q has s_q s_i equal to the column's relative sign
                 bool active = cr.group >= 0;
-                if (cr.sitek >= 0) {
+                if (!SIMPLE && cr.sitek >= 0) {
                     active = active && (si * spin_from_bits(mybits, cr.sitek) == ((cr.par & 1) ? -1.f : 1.f));
                     const int s2 = cr.sx & 0xffff, s3 = (cr.sx >> 16) & 0xffff;
                     if (s2 != 0xffff) active = active && (si * spin_from_bits(mybits, s2) == ((cr.par & 2) ? -1.f : 1.f));
                     if (s3 != 0xffff) active = active && (si * spin_from_bits(mybits, s3) == ((cr.par & 4) ? -1.f : 1.f));
                 }
                 // summed matrix element of the group (Eq. 39): two inline terms, or (rare) the general list
-                const float fa = spin_or_one(tm.z0a) * spin_or_one(tm.z1a), fb = spin_or_one(tm.z0b) * spin_or_one(tm.z1b);
-                float mr = fmaf(tm.cra, fa, tm.crb * fb), mi = fmaf(tm.cia, fa, tm.cib * fb);
-                if (cr.count & SR_GENERIC_TERMS) {
-                    const int first = p.H.grp_first[cr.group], count = cr.count & ~SR_GENERIC_TERMS;
+                float mr = tm.cra, mi = tm.cia;  // SIMPLE: one term without Z factors (or none: 0)
+                if (!SIMPLE) {
+                    const float fa = spin_or_one(tm.z0a) * spin_or_one(tm.z1a), fb = spin_or_one(tm.z0b) * spin_or_one(tm.z1b);
+                    mr = fmaf(tm.cra, fa, tm.crb * fb), mi = fmaf(tm.cia, fa, tm.cib * fb);
+                }
+                if (!SIMPLE && (cr.count & SR_GENERIC_TERMS)) {
+                    const int first = p.H.grp_first[cr.group], count = cr.count & SR_COUNT_MASK;
                     for (int u = 0; u < count; ++u) {
                         float f = spin_or_one(p.H.gt_z0[first + u]) * spin_or_one(p.H.gt_z1[first + u]);
                         if (p.H.has_zx)
@@ -545,6 +577,9 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 eps += live ? bound : 0.f;
             }
         }
+        };
+        if (tile_simple) columns(std::true_type{});
+        else columns(std::false_type{});
         NQS_STAMP(4);
         // the other column parts hand their sums to part 0, which owns the row's output (fixed order: deterministic)
         if (part > 0) sred[(part - 1) * SR_M + row] = make_float4(er_acc, ei_acc, eps, 0.f);
