@@ -757,11 +757,6 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         NQS_TRY(S.get(&tab, (size_t)nTiles * M_pad * TC));
         NQS_TRY(S.get(&rho, (size_t)C_pad));
         NQS_TRY(S.get(&partial, (size_t)B * nTiles));
-        const long long total = (long long)M_pad * C_pad;
-        const unsigned tgrid = (unsigned)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
-        table_kernel<<<tgrid, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, h->C, TC, nTiles,
-                                            h->dev, tab, rho);
-        NQS_LAUNCHED();
     }
     // series operands that do not depend on the samples
     const int NB = h->NB, nNT = h->nNT, nJC = M_pad / 16;
@@ -837,6 +832,13 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     NQS_PROF(5, st);
     const int* gate = (use_series && use_product) ? status : nullptr;
     const bool fused_finalize = use_product && !use_series && nTiles == 1;  // eloc_kernel writes E_loc itself
+    if (use_product) {  // the product form's tables (behind the series: only if the guard failed)
+        const long long total = (long long)M_pad * C_pad;
+        const unsigned tgrid = (unsigned)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
+        table_kernel<<<tgrid, 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad, h->C, TC, nTiles,
+                                            h->dev, tab, rho, gate);
+        NQS_LAUNCHED();
+    }
     if (use_product && !tp_now) {  // fallback pass: tanh(theta) for the product form, only if the guard failed
         ThetaOut o;
         o.tp = tp;

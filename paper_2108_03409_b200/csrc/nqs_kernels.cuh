@@ -20,7 +20,8 @@ namespace nqs {
 // ----------------------------------------------------------------------------------------
 __global__ void table_kernel(const float2* __restrict__ W, const float2* __restrict__ a, int N, int M, int M_pad,
                              int C, int TC, int nTiles, DevHam H,
-                             float4* __restrict__ tab, float4* __restrict__ rho) {
+                             float4* __restrict__ tab, float4* __restrict__ rho, const int* __restrict__ gate) {
+    if (gate && !(gate[0] & 1)) return;  // fallback pass: only if the series guard failed
     const int C_pad = nTiles * TC;
     const long long total = (long long)M_pad * C_pad;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;

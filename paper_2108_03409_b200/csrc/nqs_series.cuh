@@ -110,32 +110,41 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
     for (int j8 = tid; j8 < M_pad / 8; j8 += 256) {
         float v[SR_PLANES][8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            const int j = j8 * 8 + q;
-            float Tr = 0.f, Ti = 0.f;
-            if (live_col && j < M) {
-                const float2 w = column_sum(H, c, W + (long long)j * N);
-                float lr, li;
-                lncosh_tanh(2.f * w.x, 2.f * w.y, lr, li, Tr, Ti);
-                lkr += (double)lr;
-                lki += (double)li;
-                const float m2 = fmaf(Tr, Tr, Ti * Ti);
-                n2 += m2;
-                n4 = fmaf(m2, m2, n4);
-                n6 = fmaf(m2 * m2, m2, n6);
-                n8 = fmaf(m2 * m2, m2 * m2, n8);
-                tmx = fmaxf(tmx, m2);
+        for (int q2 = 0; q2 < 8; q2 += 2) {
+            // log cosh 2V and T = tanh 2V of two hidden units at a time (packed Taylor series for |2V|^2 < 0.36, the
+            // closed form otherwise: nqs_device.cuh)
+            const int j0 = j8 * 8 + q2;
+            const bool l0 = live_col && j0 < M, l1 = live_col && j0 + 1 < M;
+            const float2 w0 = l0 ? column_sum(H, c, W + (long long)j0 * N) : make_float2(0.f, 0.f);
+            const float2 w1 = l1 ? column_sum(H, c, W + (long long)(j0 + 1) * N) : make_float2(0.f, 0.f);
+            float2 lr2, li2, Tr2, Ti2;
+            lncosh_tanh2(make_float2(2.f * w0.x, 2.f * w1.x), make_float2(2.f * w0.y, 2.f * w1.y), lr2, li2, Tr2, Ti2);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int q = q2 + h;
+                const bool lv = h ? l1 : l0;
+                const float Tr = lv ? (h ? Tr2.y : Tr2.x) : 0.f, Ti = lv ? (h ? Ti2.y : Ti2.x) : 0.f;
+                if (lv) {
+                    lkr += (double)(h ? lr2.y : lr2.x);
+                    lki += (double)(h ? li2.y : li2.x);
+                    const float m2 = fmaf(Tr, Tr, Ti * Ti);
+                    n2 += m2;
+                    n4 = fmaf(m2, m2, n4);
+                    n6 = fmaf(m2 * m2, m2, n6);
+                    n8 = fmaf(m2 * m2, m2 * m2, n8);
+                    tmx = fmaxf(tmx, m2);
+                }
+                const float sr = Tr * SR_SB1, si = Ti * SR_SB1;
+                v[0][q] = __half2float(__float2half_rn(sr));
+                v[1][q] = __half2float(__float2half_rn(si));
+                v[2][q] = sr - v[0][q];
+                v[3][q] = si - v[1][q];
+                const float T2r = fmaf(Tr, Tr, -Ti * Ti), T2i = 2.f * Tr * Ti;
+                v[4][q] = 0.5f * SR_SB2 * T2r;
+                v[5][q] = 0.5f * SR_SB2 * T2i;
+                v[6][q] = (SR_SB1 / 3.f) * fmaf(Tr, T2r, -Ti * T2i);
+                v[7][q] = (SR_SB1 / 3.f) * fmaf(Tr, T2i, Ti * T2r);
             }
-            const float sr = Tr * SR_SB1, si = Ti * SR_SB1;
-            v[0][q] = __half2float(__float2half_rn(sr));
-            v[1][q] = __half2float(__float2half_rn(si));
-            v[2][q] = sr - v[0][q];
-            v[3][q] = si - v[1][q];
-            const float T2r = fmaf(Tr, Tr, -Ti * Ti), T2i = 2.f * Tr * Ti;
-            v[4][q] = 0.5f * SR_SB2 * T2r;
-            v[5][q] = 0.5f * SR_SB2 * T2i;
-            v[6][q] = (SR_SB1 / 3.f) * fmaf(Tr, T2r, -Ti * T2i);
-            v[7][q] = (SR_SB1 / 3.f) * fmaf(Tr, T2i, Ti * T2r);
         }
         const int jc = j8 >> 1, slab = j8 & 1;
         uint4* dst = B_packed + (((long long)nt * nJC + jc) * SR_PLANES) * (2 * NB) + slab * NB + cl;
