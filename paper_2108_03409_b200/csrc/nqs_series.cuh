@@ -68,10 +68,12 @@ struct __align__(16) SeriesCol {
                          // SR_GENERIC_TERMS set when they are not (all) inline in SeriesTerms
 };
 constexpr int SR_GENERIC_TERMS = 1 << 30;
-// the column's matrix element does not depend on the sample: a single flip whose one term has no Z factor (the X_i of a
-// transverse field), or a padding column (element 0).  A tile of such columns takes a shorter epilogue.
-constexpr int SR_SIMPLE = 1 << 29;
-constexpr int SR_COUNT_MASK = SR_SIMPLE - 1;
+// the column's matrix element is m0 + sigma m1 with constants m0, m1 whenever the column applies: at most two inline terms
+// whose Z factors sit on the column's own (one or two) flip sites -- the X_i of a transverse field, the XX + YY of a
+// Heisenberg bond (s_k = +/- s_i is fixed by the column's relative sign) -- or a padding column (0).  SeriesTerms then
+// holds m0 as a constant term and m1 as a term on s[site]; a tile of such columns takes a shorter epilogue.
+constexpr int SR_AFFINE = 1 << 29;
+constexpr int SR_COUNT_MASK = SR_AFFINE - 1;
 static_assert(sizeof(SeriesCol) == 64, "SeriesCol layout");
 // the first two terms of the column's group, element = c * s[z0] * s[z1] (z = -1: factor 1); an absent term has c = 0
 struct __align__(16) SeriesTerms {
@@ -211,8 +213,28 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
             const float2 cc = H.gt_c[first + 1];
             t2.z0b = H.gt_z0[first + 1], t2.z1b = H.gt_z1[first + 1], t2.crb = cc.x, t2.cib = cc.y;
         }
-        const bool simple = r.group < 0 || (r.sitek < 0 && !generic && count <= 1 && t2.z0a < 0 && t2.z1a < 0);
-        r.count = count | (generic ? SR_GENERIC_TERMS : 0) | (simple ? SR_SIMPLE : 0);
+        bool affine = !generic && r.sx == (int)0xffffffff;
+        if (affine) {
+            const float psign = (r.par & 1) ? -1.f : 1.f;
+            float m0r = 0.f, m0i = 0.f, m1r = 0.f, m1i = 0.f;
+            const int zs[2][2] = {{t2.z0a, t2.z1a}, {t2.z0b, t2.z1b}};
+            const float cs[2][2] = {{t2.cra, t2.cia}, {t2.crb, t2.cib}};
+            for (int u = 0; u < 2; ++u) {
+                int ni = 0, nk = 0;
+                for (int q = 0; q < 2; ++q) {
+                    const int z = zs[u][q];
+                    if (z < 0) continue;
+                    if (z == r.site) ++ni;
+                    else if (r.sitek >= 0 && z == r.sitek) ++nk;
+                    else affine = false;
+                }
+                const float f = (nk & 1) ? psign : 1.f;  // s_k = psign s_i where the column applies
+                if ((ni + nk) & 1) m1r = fmaf(cs[u][0], f, m1r), m1i = fmaf(cs[u][1], f, m1i);
+                else m0r = fmaf(cs[u][0], f, m0r), m0i = fmaf(cs[u][1], f, m0i);
+            }
+            if (affine) t2 = {-1, -1, m0r, m0i, r.site, -1, m1r, m1i};
+        }
+        r.count = count | (generic ? SR_GENERIC_TERMS : 0) | (affine ? SR_AFFINE : 0);
         cols[c] = r;
         terms[c] = t2;
     }
@@ -517,12 +539,12 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
         NQS_STAMP(3);
         tc_fence_after();
         const uint32_t tbase = tmem_base + ((uint32_t)(lane_grp * 32) << 16);
-        // are all columns of the tile "simple" (warp-uniform: the records are the same for every row)?
-        bool tile_simple = true;
-        for (int c = lane; c < NB; c += 32) tile_simple = tile_simple && (scol[c].count & SR_SIMPLE);
-        tile_simple = __all_sync(0xffffffffu, tile_simple);
-        auto columns = [&](auto simple_tag) {
-        constexpr bool SIMPLE = decltype(simple_tag)::value;
+        // are all columns of the tile affine (warp-uniform: the records are the same for every row)?
+        bool tile_affine = true;
+        for (int c = lane; c < NB; c += 32) tile_affine = tile_affine && (scol[c].count & SR_AFFINE);
+        tile_affine = __all_sync(0xffffffffu, tile_affine);
+        auto columns = [&](auto affine_tag) {
+        constexpr bool AFFINE = decltype(affine_tag)::value;
 #pragma unroll 1
         for (int bt = b_lo; bt < b_hi; ++bt) {
             const int c0 = bt * SR_EPI_COLS;
@@ -540,19 +562,21 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 const float si = spin_from_bits(mybits, cr.site);
                 // the column applies iff every further flip site q has s_q s_i equal to the column's relative sign
                 bool active = cr.group >= 0;
-                if (!SIMPLE && cr.sitek >= 0) {
+                if (cr.sitek >= 0) {
                     active = active && (si * spin_from_bits(mybits, cr.sitek) == ((cr.par & 1) ? -1.f : 1.f));
-                    const int s2 = cr.sx & 0xffff, s3 = (cr.sx >> 16) & 0xffff;
-                    if (s2 != 0xffff) active = active && (si * spin_from_bits(mybits, s2) == ((cr.par & 2) ? -1.f : 1.f));
-                    if (s3 != 0xffff) active = active && (si * spin_from_bits(mybits, s3) == ((cr.par & 4) ? -1.f : 1.f));
+                    if (!AFFINE) {
+                        const int s2 = cr.sx & 0xffff, s3 = (cr.sx >> 16) & 0xffff;
+                        if (s2 != 0xffff) active = active && (si * spin_from_bits(mybits, s2) == ((cr.par & 2) ? -1.f : 1.f));
+                        if (s3 != 0xffff) active = active && (si * spin_from_bits(mybits, s3) == ((cr.par & 4) ? -1.f : 1.f));
+                    }
                 }
                 // summed matrix element of the group (Eq. 39): two inline terms, or (rare) the general list
-                float mr = tm.cra, mi = tm.cia;  // SIMPLE: one term without Z factors (or none: 0)
-                if (!SIMPLE) {
+                float mr = fmaf(tm.crb, si, tm.cra), mi = fmaf(tm.cib, si, tm.cia);  // AFFINE: m0 + sigma m1
+                if (!AFFINE) {
                     const float fa = spin_or_one(tm.z0a) * spin_or_one(tm.z1a), fb = spin_or_one(tm.z0b) * spin_or_one(tm.z1b);
                     mr = fmaf(tm.cra, fa, tm.crb * fb), mi = fmaf(tm.cia, fa, tm.cib * fb);
                 }
-                if (!SIMPLE && (cr.count & SR_GENERIC_TERMS)) {
+                if (!AFFINE && (cr.count & SR_GENERIC_TERMS)) {
                     const int first = p.H.grp_first[cr.group], count = cr.count & SR_COUNT_MASK;
                     for (int u = 0; u < count; ++u) {
                         float f = spin_or_one(p.H.gt_z0[first + u]) * spin_or_one(p.H.gt_z1[first + u]);
@@ -587,7 +611,7 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
             }
         }
         };
-        if (tile_simple) columns(std::true_type{});
+        if (tile_affine) columns(std::true_type{});
         else columns(std::false_type{});
         NQS_STAMP(4);
         // the other column parts hand their sums to part 0, which owns the row's output (fixed order: deterministic)
