@@ -553,7 +553,22 @@ struct ThetaOut {
     float4* rown = nullptr;
     float* rowmax = nullptr;
     const int* gate = nullptr;   // device word: run only if (gate[0] & 1)
+    int S = 1;                   // tensor-core kernel, series path: hidden-unit tiles of a sample tile split over S CTAs
+    double2* lp_part = nullptr;  // [S][rows] partial log psi (S > 1)
 };
+
+// how many CTAs share the hidden units of one sample tile: the split that needs the fewest waves of the 2 x SMs CTA slots
+// (each extra CTA reloads the tile's spins and pays its own set-up: ~3 % per split)
+static int theta_split(long long nMT, int nNT, int sms) {
+    int best = 1;
+    double best_cost = 1e30;
+    for (int S = 1; S <= 8 && nNT / S >= 4; S *= 2) {
+        const long long waves = (nMT * S + 2ll * sms - 1) / (2ll * sms);
+        const double cost = (double)waves / S * (1.0 + 0.03 * (S - 1));
+        if (cost < best_cost - 1e-9) best_cost = cost, best = S;
+    }
+    return best;
+}
 
 static int launch_theta_simt(DeviceState* D, const int8_t* d_spins, int64_t B, int32_t N, int32_t M, int M_pad,
                              const nqs_c64* d_a, const nqs_c64* d_b, const nqs_c64* d_W, long long nPairsPad,
@@ -612,7 +627,10 @@ static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, in
     p.rown = o.rown;
     p.rowmax = o.rowmax;
     p.gate = o.gate;
-    theta_mma_kernel<<<(unsigned)nMT, TM_THREADS, smem, st>>>(p);
+    p.S = o.S;
+    p.lp_part = o.lp_part;
+    p.rows = nMT * TM_M;
+    theta_mma_kernel<<<(unsigned)(nMT * o.S), TM_THREADS, smem, st>>>(p);
     NQS_LAUNCHED();
     return NQS_OK;
 }
@@ -765,14 +783,18 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     SeriesTerms* sterms = nullptr;
     float4 *rown = nullptr, *spartial = nullptr;
     float* rowmax = nullptr;
+    double2* lp_part = nullptr;
+    int nS = 1;
     int* status = nullptr;
     if (use_series) {
         NQS_TRY(S.get(&sA, (size_t)(B_pad / SR_M) * nJC * SR_PLANES * SR_A_PLANE_U4));
         NQS_TRY(S.get(&sB, (size_t)nNT * nJC * SR_PLANES * 2 * NB));
         NQS_TRY(S.get(&scols, (size_t)nNT * NB));
         NQS_TRY(S.get(&sterms, (size_t)nNT * NB));
-        NQS_TRY(S.get(&rown, (size_t)B_pad));
-        NQS_TRY(S.get(&rowmax, (size_t)B_pad));
+        nS = fused_pack && !keep_tp && g_opt[NQS_OPT_THETA_SPLIT].load() != 1 ? theta_split(B_pad / TM_M, M_pad / TH_JT, D->sms) : 1;
+        NQS_TRY(S.get(&rown, (size_t)B_pad * nS));
+        NQS_TRY(S.get(&rowmax, (size_t)B_pad * nS));
+        if (nS > 1 && d_logpsi) NQS_TRY(S.get(&lp_part, (size_t)B_pad * nS));
         NQS_TRY(S.get(&spartial, (size_t)B * nNT));
         NQS_TRY(S.get(&status, 4));
         NQS_CUDA(cudaMemsetAsync(status, 0, 4 * sizeof(int), st));
@@ -788,7 +810,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         ThetaOut o;
         o.logpsi = d_logpsi;
         o.tp = tp_now ? tp : nullptr;
-        if (fused_pack) o.sA = sA, o.rown = rown, o.rowmax = rowmax;
+        if (fused_pack) o.sA = sA, o.rown = rown, o.rowmax = rowmax, o.S = nS, o.lp_part = lp_part;
         NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
     }
     NQS_PROF(2, st);
@@ -807,6 +829,8 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         gp.terms = sterms;
         gp.rown = rown;
         gp.rowmax = rowmax;
+        gp.nS = nS;
+        gp.rows = B_pad;
         gp.spins = d_spins;
         gp.B = B;
         gp.N = N;
@@ -826,7 +850,8 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     NQS_PROF(4, st);
     if (use_series) {
         series_guard_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(spartial, (long long)B, nNT, (float2*)d_eloc,
-                                                                         status);
+                                                                         status, lp_part, nS, (long long)B_pad,
+                                                                         (float2*)d_logpsi);
         NQS_LAUNCHED();
     }
     NQS_PROF(5, st);

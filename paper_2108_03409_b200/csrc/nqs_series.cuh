@@ -356,8 +356,10 @@ struct SeriesGemmParams {
     const uint4* B_packed;   // [nNT][nJC][8][2 NB]
     const SeriesCol* cols;   // [nNT * NB]
     const SeriesTerms* terms;  // [nNT * NB]
-    const float4* rown;      // [B_pad]
-    const float* rowmax;     // [B_pad]
+    const float4* rown;      // [B_pad] (n2t, n4t, n6t, n8t);  nS > 1: [nS][B_pad] partial sums of |t|^P (theta kernel split
+    const float* rowmax;     // [B_pad] max |t|;                over nS CTAs per sample tile): combined here
+    int nS;                  // number of partials (1: final values)
+    long long rows;          // B_pad: stride of the partials
     const int8_t* spins;     // [B][N]
     long long B;
     int N, nJC, NB, nNT;
@@ -531,8 +533,17 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
             }
         }
         NQS_STAMP(2);
-        const float4 rn = p.rown[b];
-        const float rmax = p.rowmax[b];
+        float4 rn = p.rown[b];
+        float rmax = p.rowmax[b];
+        if (p.nS > 1) {  // fixed order: deterministic
+            for (int k = 1; k < p.nS; ++k) {
+                const float4 o = p.rown[k * p.rows + b];
+                rn.x += o.x, rn.y += o.y, rn.z += o.z, rn.w += o.w;
+                rmax = fmaxf(rmax, p.rowmax[k * p.rows + b]);
+            }
+            rn = make_float4(sqrtf(rn.x), sqrtf(rn.y), sqrtf(rn.z), sqrtf(rn.w));
+            rmax = sqrtf(rmax);
+        }
         const int nBatch = NB / SR_EPI_COLS;
         const int b_lo = nBatch * part / SR_EPI_PARTS, b_hi = nBatch * (part + 1) / SR_EPI_PARTS;
         mbar_wait_sleep(t_full, 0, 256);
@@ -643,10 +654,20 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
 // E_loc = sum of the column tiles' partial sums (the diagonal rides in tile 0); guard: the call fails as a
 // whole if any sample's error bound exceeds SR_GUARD_FRACTION * 1e-4 * max(1, |E_loc|) (or is NaN).
 // status[0] |= 1 when the guard fails (read by eloc_kernel / finalize_kernel), status[1] counts the samples.
+// nS > 1: log psi = sum of the theta kernel's nS partial sums (float64, fixed order).
 __global__ void series_guard_kernel(const float4* __restrict__ partial, long long B, int nNT, float2* __restrict__ eloc,
-                                    int* __restrict__ status) {
+                                    int* __restrict__ status, const double2* __restrict__ lp_part, int nS,
+                                    long long rows, float2* __restrict__ logpsi) {
     const long long b = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (b >= B) return;
+    if (nS > 1 && logpsi) {
+        double lr = 0.0, li = 0.0;
+        for (int k = 0; k < nS; ++k) {
+            const double2 v = lp_part[k * rows + b];
+            lr += v.x, li += v.y;
+        }
+        logpsi[b] = make_float2((float)lr, (float)li);
+    }
     float er = 0.f, ei = 0.f, eps = 0.f;
     for (int t = 0; t < nNT; ++t) {
         const float4 v = partial[b * nNT + t];

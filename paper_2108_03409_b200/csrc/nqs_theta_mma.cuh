@@ -222,6 +222,14 @@ struct ThetaMmaParams {
     float4* rown;            // [rows] (with sA)
     float* rowmax;           // [rows] (with sA)
     const int* gate;         // nullptr, or: run only if (gate[0] & 1) -- the series guard failed (fallback pass)
+    // S > 1 (series path only): the hidden-unit tiles of a sample tile are split over S CTAs (grid = sample tiles x S)
+    // so that the grid is a near-whole number of waves of the 2 x 148 CTA slots; every CTA then leaves PARTIAL sums
+    //   lp_part[js][b] = (Re, Im) of its share of log psi (float64; the visible bias a.s rides in js = 0)
+    //   rown[js][b]    = (sum |t|^2, sum |t|^4, sum |t|^6, sum |t|^8) (no square root),  rowmax[js][b] = max |t|^2
+    // which series_gemm_kernel / series_guard_kernel combine in a fixed order.
+    int S;
+    double2* lp_part;        // [S][rows] (S > 1)
+    long long rows;          // padded number of rows = stride of the partial arrays
 };
 
 __device__ __forceinline__ unsigned tm_pack_h2(float2 v) {
@@ -247,7 +255,9 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
     float* const nrm_x = reinterpret_cast<float*>(lp_x + 2 * TM_M);  // [128][5]
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const long long mt = blockIdx.x;
+    const int S = p.S, js = (int)(blockIdx.x % S);
+    const long long mt = blockIdx.x / S;
+    const int nt0 = (int)((long long)p.nNT * js / S), nt1 = (int)((long long)p.nNT * (js + 1) / S);  // this CTA's unit tiles
     const int nKC = K16 / (TM_KC / 16);
 
     if (tid == 0) {
@@ -274,7 +284,7 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
             mbar_expect_tx(a_full, a_bytes);
             bulk_g2s(sA, p.A_packed + mt * (long long)K16 * TM_M, a_bytes, a_full);
             int it = 0;
-            for (int nt = 0; nt < p.nNT; ++nt)
+            for (int nt = nt0; nt < nt1; ++nt)
                 for (int kc = 0; kc < nKC; ++kc, ++it) {
                     const int s = it % TH_STAGES;
                     mbar_wait(&b_empty[s], ((it / TH_STAGES) & 1) ^ 1);
@@ -289,9 +299,9 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
             mbar_wait(a_full, 0);
             const uint32_t sA_u = smem_u32(sA), sB_u = smem_u32(sB);
             int it = 0;
-            for (int nt = 0; nt < p.nNT; ++nt) {
-                const int set = nt & 1;
-                mbar_wait(&t_empty[set], ((nt >> 1) & 1) ^ 1);
+            for (int nt = nt0; nt < nt1; ++nt) {
+                const int ln = nt - nt0, set = ln & 1;
+                mbar_wait(&t_empty[set], ((ln >> 1) & 1) ^ 1);
                 tc_fence_after();
                 for (int kc = 0; kc < nKC; ++kc, ++it) {
                     const int s = it % TH_STAGES;
@@ -322,14 +332,14 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
         double lpr = 0.0, lpi = 0.0;
         float2 n2 = make_float2(0.f, 0.f), n4 = n2, n6 = n2, n8 = n2;  // the two halves of a unit pair accumulate apart
         float tmx = 0.f;
-        for (int nt = 0; nt < p.nNT; ++nt) {
+        for (int nt = nt0; nt < nt1; ++nt) {
             // scale and bias of this warp's 8 hidden units: lane u (mod 8) holds unit u, fetched before the
             // accumulator wait and handed round by shuffles
-            const int set = nt & 1;
+            const int ln = nt - nt0, set = ln & 1;
             const int jmine = nt * TH_JT + half * 8 + (lane & 7);
             const float my_sc = p.scale[jmine];
             const float2 my_b = jmine < p.M ? p.bvec[jmine] : make_float2(0.f, 0.f);
-            mbar_wait(&t_full[set], (nt >> 1) & 1);
+            mbar_wait(&t_full[set], (ln >> 1) & 1);
             tc_fence_after();
             {   // 8 hidden units per warp and tile = one 16-byte slab of every series plane
                 int v0[32], v1[32];
@@ -420,7 +430,7 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
             }
         }
         // visible bias, split between the two column halves of a row
-        if (b < p.B && p.logpsi) {
+        if (b < p.B && p.logpsi && js == 0) {
             float ar = 0.f, ai = 0.f;
             const int i_lo = half ? p.N / 2 : 0, i_hi = half ? p.N : p.N / 2;
             for (int i = i_lo; i < i_hi; ++i) {
@@ -444,7 +454,15 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
             nrm_x[5 * row + 4] = tmx;
         }
         asm volatile("bar.sync 1, 256;" ::: "memory");
-        if (half == 0) {
+        if (half == 0 && S > 1) {  // partial sums of this CTA's share of the hidden units
+            const long long o = (long long)js * p.rows + b;
+            if (p.logpsi) p.lp_part[o] = make_double2(lpr + lp_x[2 * row], lpi + lp_x[2 * row + 1]);
+            if (p.sA) {
+                p.rown[o] = make_float4(n2.x + n2.y + nrm_x[5 * row + 0], n4.x + n4.y + nrm_x[5 * row + 1],
+                                        n6.x + n6.y + nrm_x[5 * row + 2], n8.x + n8.y + nrm_x[5 * row + 3]);
+                p.rowmax[o] = fmaxf(tmx, nrm_x[5 * row + 4]);
+            }
+        } else if (half == 0) {
             if (b < p.B && p.logpsi)
                 p.logpsi[b] = make_float2((float)(lpr + lp_x[2 * row]), (float)(lpi + lp_x[2 * row + 1]));
             if (p.sA) {

@@ -172,3 +172,29 @@ def test_series_with_the_simt_theta_kernel(nqs, oracle):
     assert took["path"] == "series" and not took["guard_failed"], took
     check_eloc(e1, e_ref, "series, SIMT theta, config 3")
     check_logpsi(l1, l_ref, "series, SIMT theta, config 3")
+
+
+def test_theta_split_over_ctas(nqs, oracle):
+    """On the series path the hidden-unit tiles of a sample tile are split over S CTAs of the theta kernel (S chosen
+    for whole waves; partial log psi and row norms combined in a fixed order).  The operand planes do not depend on the
+    split, so E_loc must have the same bits as with NQS_OPT_THETA_SPLIT = 1; log psi is the same float64 sum in another
+    order (<= 1 ulp of the float32 result) and is checked against the oracle either way; deterministic run to run."""
+    for k, B in ((5, 2000), (3, 4500), (4, 1300)):   # 16 / 36 / 11 sample tiles: S = 8, 8, 8 resp. what fits M
+        w = wl.make_config(k, B=B)
+        e_ref, l_ref = oracle_on(oracle, w, slice(None), "fast")
+        out = {}
+        for split in (1, 0, 0):
+            nqs.set_option("theta_split", split)
+            try:
+                e, l, took = run(nqs, w, "series_only")
+            finally:
+                nqs.set_option("theta_split", 0)
+            assert took["path"] == "series" and not took["guard_failed"], took
+            check_logpsi(l, l_ref, f"c{k} theta_split={split}")
+            out.setdefault(split, []).append((e, l))
+        (e1, l1), = out[1]
+        (e0, l0), (e0b, l0b) = out[0]
+        check_eloc(e0, e_ref, f"c{k} split")
+        assert np.array_equal(e1, e0), "E_loc must not depend on the split of the theta kernel"
+        assert np.array_equal(e0, e0b) and np.array_equal(l0, l0b), "run-to-run determinism"
+        assert np.abs(l1 - l0).max() <= 2e-7 * max(1.0, np.abs(l_ref).max())
