@@ -170,13 +170,17 @@ int nqs_local_energy_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t 
  *   NQS_OPT_THETA_SPLIT 0 = automatic: on the series path the hidden units of a sample tile are split over 1, 2, 4 or 8
  *                       CTAs of the theta kernel, whichever needs the fewest waves of the 2 x SMs CTA slots (partial
  *                       log psi / row norms combined in a fixed order: deterministic)         1 = never split
+ *   NQS_OPT_SERIES_WIDE 0 = automatic: more than 128 table columns are tiled in column tiles of up to 224 (the series
+ *                       GEMM then makes two passes over the hidden units with one accumulator pair in TMEM at a time,
+ *                       csrc/nqs_series.cuh) where that fits in shared memory           1 = tiles of <= 128 columns only;
+ *                       the two give the same bits
  *   NQS_OPT_HOST_CHUNKS 0 = automatic: nqs_local_energy_host sends the batch through the device in B / 32768 chunks
  *                       (at most 16), copying chunk k + 1 while the kernels of chunk k run      1 .. 16 = that many
  * nqs_debug_last_a5 (synchronises `stream`; tests only; not meaningful while calls run concurrently on other
  * streams): out[0] = 1 if the most recent nqs_local_energy* call on this device attempted the series path, 2 if
  * it used the product form only, 3 if the single-launch kernel for small problems ran; out[1] = 1 if the guard failed; out[2] = samples over the guard threshold.
  * ------------------------------------------------------------------------------------- */
-enum { NQS_OPT_A5_PATH = 0, NQS_OPT_THETA_PATH = 1, NQS_OPT_HOST_CHUNKS = 2, NQS_OPT_SMALL_PATH = 3, NQS_OPT_THETA_SPLIT = 4, NQS_OPT_COUNT = 5 };
+enum { NQS_OPT_A5_PATH = 0, NQS_OPT_THETA_PATH = 1, NQS_OPT_HOST_CHUNKS = 2, NQS_OPT_SMALL_PATH = 3, NQS_OPT_THETA_SPLIT = 4, NQS_OPT_SERIES_WIDE = 5, NQS_OPT_COUNT = 6 };
 int nqs_set_option(int32_t key, int32_t value);
 int nqs_get_option(int32_t key, int32_t *value);
 int nqs_debug_last_a5(int32_t out[3], void *stream);

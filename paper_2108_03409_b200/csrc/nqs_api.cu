@@ -197,8 +197,10 @@ struct nqs_hamiltonian {
     int C = 0;
     // launch plan (static for the handle): column tiling of the product-form a5 kernel ...
     int WC = 1, WS = 2, TC = 16, nTiles = 1, C_pad = 16;
-    // ... and of the tensor-core series kernel
+    // ... and of the tensor-core series kernel: narrow tiles (NB <= 128, all four accumulator ranges in TMEM) and, where
+    // that makes fewer tiles and fits in shared memory, wide ones (NB <= 224, two passes; NBw = 0: not available)
     int NB = 16, nNT = 1;
+    int NBw = 0, nNTw = 0;
 };
 
 static constexpr int KJ = 16;
@@ -231,6 +233,13 @@ static void plan_tiles(nqs_hamiltonian* h) {
     h->nNT = C > 0 ? (C + 127) / 128 : 1;
     const int per = C > 0 ? (C + h->nNT - 1) / h->nNT : 16;
     h->NB = (per + 15) / 16 * 16;
+    h->NBw = h->nNTw = 0;
+    if (C > 128) {
+        const int ntw = (C + SR_WIDE_MAX_NB - 1) / SR_WIDE_MAX_NB;
+        const int nbw = ((C + ntw - 1) / ntw + 15) / 16 * 16;
+        if (ntw < h->nNT && h->hc.N <= SR_MAX_N && series_gemm_smem_bytes(nbw, h->hc.N, true) <= 227 * 1024)
+            h->NBw = nbw, h->nNTw = ntw;
+    }
 }
 
 static int upload(nqs_hamiltonian* h, DeviceState* D, bool pooled, cudaStream_t st) {
@@ -777,7 +786,8 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         NQS_TRY(S.get(&partial, (size_t)B * nTiles));
     }
     // series operands that do not depend on the samples
-    const int NB = h->NB, nNT = h->nNT, nJC = M_pad / 16;
+    const bool wide = use_series && h->NBw > 0 && g_opt[NQS_OPT_SERIES_WIDE].load() != 1;
+    const int NB = wide ? h->NBw : h->NB, nNT = wide ? h->nNTw : h->nNT, nJC = M_pad / 16;
     uint4 *sA = nullptr, *sB = nullptr;
     SeriesCol* scols = nullptr;
     SeriesTerms* sterms = nullptr;
@@ -820,8 +830,11 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     }
     NQS_PROF(3, st);
     if (use_series) {
-        const size_t smem = series_gemm_smem_bytes(NB, N);
-        NQS_TRY(ensure_smem(D, series_gemm_kernel, smem));
+        const size_t smem = series_gemm_smem_bytes(NB, N, wide);
+        if (wide) NQS_TRY(ensure_smem(D, series_gemm_kernel<true>, smem));
+        else NQS_TRY(ensure_smem(D, series_gemm_kernel<false>, smem));
+        float2* even = nullptr;
+        if (wide) NQS_TRY(S.get(&even, (size_t)(B_pad / SR_M) * nNT * NB * SR_M));
         SeriesGemmParams gp;
         gp.A_packed = sA;
         gp.B_packed = sB;
@@ -839,12 +852,14 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         gp.nNT = nNT;
         gp.H = h->dev;
         gp.partial = spartial;
+        gp.even = even;
 #ifdef NQS_SERIES_TIMELINE
         gp.timeline = g_series_timeline;
 #endif
         const long long blocks = (B_pad / SR_M) * nNT;
         if (blocks > 0x7fffffffll) return fail(NQS_ERR_UNSUPPORTED, "B x column tiles exceeds the grid limit");
-        series_gemm_kernel<<<(unsigned)blocks, SR_THREADS, smem, st>>>(gp);
+        if (wide) series_gemm_kernel<true><<<(unsigned)blocks, SR_THREADS, smem, st>>>(gp);
+        else series_gemm_kernel<false><<<(unsigned)blocks, SR_THREADS, smem, st>>>(gp);
         NQS_LAUNCHED();
     }
     NQS_PROF(4, st);

@@ -85,9 +85,16 @@ struct __align__(16) SeriesTerms {
 static_assert(sizeof(SeriesTerms) == 32, "SeriesTerms layout");
 
 __host__ __device__ inline int series_bits_stride(int N) { return (N + 31) / 32 | 1; }  // odd: conflict-free rows
-__host__ __device__ inline size_t series_gemm_smem_bytes(int NB, int N) {
-    return (size_t)SR_STAGES * (SR_A_STAGE_BYTES + 256 * NB) + (size_t)NB * (sizeof(SeriesCol) + sizeof(SeriesTerms)) +
-           (size_t)SR_M * series_bits_stride(N) * 4 + (size_t)(SR_EPI_PARTS - 1) * SR_M * 16 + 256;
+// wide = false: a stage holds all eight planes of both operands (32 KB + 256 NB bytes), NB <= 128.
+// wide = true : column tiles of NB <= 224 with the (re, im) accumulators of ONE of the two series sums in TMEM at a time: a
+//               stage holds six planes (hi, lo, cube: 24 KB + 192 NB bytes); the partial sums of the column parts reuse
+//               the first stage at the end.
+constexpr int SR_WIDE_PLANES = 6;
+constexpr int SR_WIDE_MAX_NB = 224;
+__host__ __device__ inline size_t series_gemm_smem_bytes(int NB, int N, bool wide = false) {
+    const size_t fixed = (size_t)NB * (sizeof(SeriesCol) + sizeof(SeriesTerms)) + (size_t)SR_M * series_bits_stride(N) * 4 + 256;
+    if (wide) return (size_t)SR_STAGES * (SR_WIDE_PLANES * SR_A_PLANE_U4 * 16 + 192 * NB) + fixed;
+    return (size_t)SR_STAGES * (SR_A_STAGE_BYTES + 256 * NB) + fixed + (size_t)(SR_EPI_PARTS - 1) * SR_M * 16;
 }
 
 __device__ __forceinline__ unsigned pack_h2(float a, float b) {
@@ -365,6 +372,7 @@ struct SeriesGemmParams {
     int N, nJC, NB, nNT;
     DevHam H;
     float4* partial;         // [B][nNT]: (Re, Im of sum_c m R [+ diagonal in tile 0], guard eps, 0)
+    float2* even;            // WIDE: [nMT][nNT][NB][128 rows] scratch for the EVEN sums (written and read back by the same thread)
 #ifdef NQS_SERIES_TIMELINE
     long long* timeline;     // [blocks][8] clock64 stamps of the first epilogue thread (development builds only)
 #endif
@@ -375,20 +383,36 @@ struct SeriesGemmParams {
 #define NQS_STAMP(k)
 #endif
 
+// WIDE = false: all four accumulator ranges (ODD.re, ODD.im, EVEN.re, EVEN.im) of a tile of NB <= 128 columns in TMEM,
+//               20 MMAs per chunk of 16 hidden units, 32 KB + 256 NB bytes of operands per chunk.
+// WIDE = true : tiles of NB <= 224 columns.  What bounds the main loop is the operand bytes an SM takes in per MMA
+//               cycle (~45 B/clk), i.e. (128 + NB) / (128 NB): a tile twice as wide needs 1.6 x
+//               fewer bytes per MAC, but its four accumulator ranges no longer fit in the 512 TMEM columns.  So the
+//               kernel makes two passes over the hidden units: pass A accumulates EVEN (4 MMAs per chunk on the t^2 /
+//               T^2 planes) and the epilogue threads move it to a global scratch array (each thread writes and later
+//               reads back only its own (row, columns): L2-resident, no fence); pass B accumulates ODD (16 MMAs per chunk)
+//               into the same TMEM columns and the epilogue proceeds as before.  Every accumulator element sees the
+//               same addends in the same order as in the narrow kernel: bit-identical E_loc.
+template <bool WIDE>
 __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const SeriesGemmParams p) {
     extern __shared__ __align__(128) unsigned char sr_smem[];
     const int NB = p.NB;
-    const uint32_t b_stage_bytes = 256u * NB, stage_bytes = SR_A_STAGE_BYTES + b_stage_bytes;
+    constexpr uint32_t A_STAGE = WIDE ? SR_WIDE_PLANES * SR_A_PLANE_U4 * 16 : SR_A_STAGE_BYTES;
+    const uint32_t b_plane = 32u * NB, b_lbo = 16u * NB;
+    const uint32_t b_stage_bytes = (WIDE ? SR_WIDE_PLANES : SR_PLANES) * b_plane, stage_bytes = A_STAGE + b_stage_bytes;
     SeriesCol* const scol = reinterpret_cast<SeriesCol*>(sr_smem + (size_t)SR_STAGES * stage_bytes);
     SeriesTerms* const sterm = reinterpret_cast<SeriesTerms*>(scol + NB);
-    float4* const sred = reinterpret_cast<float4*>(sterm + NB);  // [parts - 1][128]: partial sums of the other column parts
-    uint32_t* const sbits = reinterpret_cast<uint32_t*>(sred + (SR_EPI_PARTS - 1) * SR_M);
+    // [parts - 1][128] partial sums of the other column parts; WIDE: over the first stage (dead after the last MMA)
+    float4* const sred = WIDE ? reinterpret_cast<float4*>(sr_smem) : reinterpret_cast<float4*>(sterm + NB);
+    uint32_t* const sbits = WIDE ? reinterpret_cast<uint32_t*>(sterm + NB)
+                                 : reinterpret_cast<uint32_t*>(reinterpret_cast<float4*>(sterm + NB) + (SR_EPI_PARTS - 1) * SR_M);
     const int bstride = series_bits_stride(p.N);
     uint64_t* const bars = reinterpret_cast<uint64_t*>(sbits + (size_t)SR_M * bstride + (((size_t)SR_M * bstride) & 1));
     uint64_t* const full = bars;
     uint64_t* const empty = bars + SR_STAGES;
     uint64_t* const t_full = bars + 2 * SR_STAGES;
-    uint32_t* const tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * SR_STAGES + 1);
+    uint64_t* const t_free = bars + 2 * SR_STAGES + 1;  // WIDE: the EVEN sums have left TMEM
+    uint32_t* const tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * SR_STAGES + 2);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 #ifdef NQS_SERIES_TIMELINE
@@ -405,6 +429,7 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
             mbar_init(&empty[s], 1);
         }
         mbar_init(t_full, 1);
+        mbar_init(t_free, SR_EPI_WARPS);
         fence_mbar_init();
     }
     if (warp == 1) tmem_alloc(tmem_slot, 512);
@@ -418,43 +443,91 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
         if (lane == 0) {
             const uint4* gA = p.A_packed + mt * (long long)nJC * SR_PLANES * SR_A_PLANE_U4;
             const uint4* gB = p.B_packed + (long long)nt * nJC * SR_PLANES * (2 * NB);
-            for (int kc = 0; kc < nJC; ++kc) {
-                const int s = kc % SR_STAGES;
-                mbar_wait(&empty[s], ((kc / SR_STAGES) & 1) ^ 1);
-                unsigned char* const st = sr_smem + (size_t)s * stage_bytes;
-                mbar_expect_tx(&full[s], stage_bytes);
-                bulk_g2s(st, gA + (long long)kc * SR_PLANES * SR_A_PLANE_U4, SR_A_STAGE_BYTES, &full[s]);
-                bulk_g2s(st + SR_A_STAGE_BYTES, gB + (long long)kc * SR_PLANES * (2 * NB), b_stage_bytes, &full[s]);
+            const uint32_t a_plane = SR_A_PLANE_U4 * 16;
+            if (WIDE) {
+                // pass A: the square planes (4, 5) of both operands; pass B: hi, lo (planes 0 .. 3) and cube (6, 7)
+                for (int it = 0; it < 2 * nJC; ++it) {
+                    const int s = it % SR_STAGES, kc = it < nJC ? it : it - nJC;
+                    mbar_wait(&empty[s], ((it / SR_STAGES) & 1) ^ 1);
+                    unsigned char* const stA = sr_smem + (size_t)s * stage_bytes;
+                    unsigned char* const stB = stA + A_STAGE;
+                    const unsigned char* const srcA = reinterpret_cast<const unsigned char*>(gA + (long long)kc * SR_PLANES * SR_A_PLANE_U4);
+                    const unsigned char* const srcB = reinterpret_cast<const unsigned char*>(gB + (long long)kc * SR_PLANES * (2 * NB));
+                    if (it < nJC) {
+                        mbar_expect_tx(&full[s], 2 * a_plane + 2 * b_plane);
+                        bulk_g2s(stA, srcA + 4 * a_plane, 2 * a_plane, &full[s]);
+                        bulk_g2s(stB, srcB + 4 * b_plane, 2 * b_plane, &full[s]);
+                    } else {
+                        mbar_expect_tx(&full[s], 6 * a_plane + 6 * b_plane);
+                        bulk_g2s(stA, srcA, 4 * a_plane, &full[s]);
+                        bulk_g2s(stA + 4 * a_plane, srcA + 6 * a_plane, 2 * a_plane, &full[s]);
+                        bulk_g2s(stB, srcB, 4 * b_plane, &full[s]);
+                        bulk_g2s(stB + 4 * b_plane, srcB + 6 * b_plane, 2 * b_plane, &full[s]);
+                    }
+                }
+            } else {
+                for (int kc = 0; kc < nJC; ++kc) {
+                    const int s = kc % SR_STAGES;
+                    mbar_wait(&empty[s], ((kc / SR_STAGES) & 1) ^ 1);
+                    unsigned char* const st = sr_smem + (size_t)s * stage_bytes;
+                    mbar_expect_tx(&full[s], stage_bytes);
+                    bulk_g2s(st, gA + (long long)kc * SR_PLANES * SR_A_PLANE_U4, SR_A_STAGE_BYTES, &full[s]);
+                    bulk_g2s(st + SR_A_STAGE_BYTES, gB + (long long)kc * SR_PLANES * (2 * NB), b_stage_bytes, &full[s]);
+                }
             }
         }
     } else if (warp == 1) {
         if (lane == 0) {
             const uint32_t s0 = smem_u32(sr_smem);
             const uint32_t idesc = series_idesc(NB);
-            const uint32_t b_plane = 32u * NB, b_lbo = 16u * NB;
-            // accumulator column ranges: ODD.re, ODD.im, EVEN.re, EVEN.im
-            const uint32_t d_or = tmem_base, d_oi = tmem_base + NB, d_er = tmem_base + 2 * NB, d_ei = tmem_base + 3 * NB;
-            for (int kc = 0; kc < nJC; ++kc) {
-                const int s = kc % SR_STAGES;
-                mbar_wait(&full[s], (kc / SR_STAGES) & 1);
-                tc_fence_after();
-                const uint32_t sa = s0 + (uint32_t)s * stage_bytes, sb = sa + SR_A_STAGE_BYTES;
-                auto A = [&](int pl) { return umma_desc(sa + (uint32_t)pl * 4096u, 2048u, 128u); };
-                auto Bd = [&](int pl) { return umma_desc(sb + (uint32_t)pl * b_plane, b_lbo, 128u); };
-                // one complex product (a.re, a.im = planes pa, pa + 1) x (b.re, b.im = planes pb, pb + 1)
-                auto cprod = [&](int pa, int pb, uint32_t dre, uint32_t dim, uint32_t first) {
-                    umma_f16(dre, A(pa), Bd(pb), idesc, first);
-                    umma_f16(dre, A(pa + 1), Bd(pb + 1), idesc | SR_IDESC_NEG_A, 1u);
-                    umma_f16(dim, A(pa), Bd(pb + 1), idesc, first);
-                    umma_f16(dim, A(pa + 1), Bd(pb), idesc, 1u);
-                };
-                const uint32_t first = kc ? 1u : 0u;
-                cprod(0, 0, d_or, d_oi, first);   // t.hi T.hi
-                cprod(0, 2, d_or, d_oi, 1u);      // t.hi T.lo
-                cprod(2, 0, d_or, d_oi, 1u);      // t.lo T.hi
-                cprod(6, 6, d_or, d_oi, 1u);      // t^3 T^3 / 3
-                cprod(4, 4, d_er, d_ei, first);   // t^2 T^2 / 2
-                tc_commit(&empty[s]);
+            // accumulator column ranges: ODD.re, ODD.im, EVEN.re, EVEN.im (WIDE: EVEN first, then ODD, in the same columns)
+            const uint32_t d_or = tmem_base, d_oi = tmem_base + NB;
+            const uint32_t d_er = WIDE ? d_or : tmem_base + 2 * NB, d_ei = WIDE ? d_oi : tmem_base + 3 * NB;
+            uint32_t sa = 0, sb = 0;
+            auto A = [&](int pl) { return umma_desc(sa + (uint32_t)pl * 4096u, 2048u, 128u); };
+            auto Bd = [&](int pl) { return umma_desc(sb + (uint32_t)pl * b_plane, b_lbo, 128u); };
+            // one complex product (a.re, a.im = planes pa, pa + 1) x (b.re, b.im = planes pb, pb + 1)
+            auto cprod = [&](int pa, int pb, uint32_t dre, uint32_t dim, uint32_t first) {
+                umma_f16(dre, A(pa), Bd(pb), idesc, first);
+                umma_f16(dre, A(pa + 1), Bd(pb + 1), idesc | SR_IDESC_NEG_A, 1u);
+                umma_f16(dim, A(pa), Bd(pb + 1), idesc, first);
+                umma_f16(dim, A(pa + 1), Bd(pb), idesc, 1u);
+            };
+            if (WIDE) {
+                for (int it = 0; it < 2 * nJC; ++it) {
+                    const int s = it % SR_STAGES;
+                    if (it == nJC) {  // EVEN is complete: hand it to the epilogue warps, wait until it has left TMEM
+                        tc_commit(t_full);
+                        mbar_wait(t_free, 0);
+                    }
+                    mbar_wait(&full[s], (it / SR_STAGES) & 1);
+                    tc_fence_after();
+                    sa = s0 + (uint32_t)s * stage_bytes, sb = sa + A_STAGE;
+                    if (it < nJC) {
+                        cprod(0, 0, d_er, d_ei, it ? 1u : 0u);          // t^2 T^2 / 2  (stage slots 0, 1)
+                    } else {
+                        const uint32_t first = it > nJC ? 1u : 0u;
+                        cprod(0, 0, d_or, d_oi, first);   // t.hi T.hi
+                        cprod(0, 2, d_or, d_oi, 1u);      // t.hi T.lo
+                        cprod(2, 0, d_or, d_oi, 1u);      // t.lo T.hi
+                        cprod(4, 4, d_or, d_oi, 1u);      // t^3 T^3 / 3  (stage slots 4, 5)
+                    }
+                    tc_commit(&empty[s]);
+                }
+            } else {
+                for (int kc = 0; kc < nJC; ++kc) {
+                    const int s = kc % SR_STAGES;
+                    mbar_wait(&full[s], (kc / SR_STAGES) & 1);
+                    tc_fence_after();
+                    sa = s0 + (uint32_t)s * stage_bytes, sb = sa + A_STAGE;
+                    const uint32_t first = kc ? 1u : 0u;
+                    cprod(0, 0, d_or, d_oi, first);   // t.hi T.hi
+                    cprod(0, 2, d_or, d_oi, 1u);      // t.hi T.lo
+                    cprod(2, 0, d_or, d_oi, 1u);      // t.lo T.hi
+                    cprod(6, 6, d_or, d_oi, 1u);      // t^3 T^3 / 3
+                    cprod(4, 4, d_er, d_ei, first);   // t^2 T^2 / 2
+                    tc_commit(&empty[s]);
+                }
             }
             tc_commit(t_full);
         }
@@ -546,10 +619,29 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
         }
         const int nBatch = NB / SR_EPI_COLS;
         const int b_lo = nBatch * part / SR_EPI_PARTS, b_hi = nBatch * (part + 1) / SR_EPI_PARTS;
-        mbar_wait_sleep(t_full, 0, 256);
+        const uint32_t tbase = tmem_base + ((uint32_t)(lane_grp * 32) << 16);
+        // WIDE: this thread's slice of the EVEN scratch, [column][row] so that a warp's stores and loads coalesce
+        float2* const even = WIDE ? p.even + ((mt * p.nNT + nt) * (long long)NB) * SR_M + row : nullptr;
+        if (WIDE) {
+            mbar_wait_sleep(t_full, 0, 256);  // pass A: EVEN is in TMEM
+            tc_fence_after();
+#pragma unroll 1
+            for (int bt = b_lo; bt < b_hi; ++bt) {
+                const int c0 = bt * SR_EPI_COLS;
+                float ver[SR_EPI_COLS], vei[SR_EPI_COLS];
+                tmem_ld8_nowait(tbase + (uint32_t)c0, ver);
+                tmem_ld8_nowait(tbase + (uint32_t)(NB + c0), vei);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int q = 0; q < SR_EPI_COLS; ++q) even[(long long)(c0 + q) * SR_M] = make_float2(ver[q], vei[q]);
+            }
+            tc_fence_before();  // the loads have completed: the columns may be overwritten by pass B
+            __syncwarp();
+            if (lane == 0) mbar_arrive(t_free);
+        }
+        mbar_wait_sleep(t_full, WIDE ? 1u : 0u, 256);
         NQS_STAMP(3);
         tc_fence_after();
-        const uint32_t tbase = tmem_base + ((uint32_t)(lane_grp * 32) << 16);
         // are all columns of the tile affine (warp-uniform: the records are the same for every row)?
         bool tile_affine = true;
         for (int c = lane; c < NB; c += 32) tile_affine = tile_affine && (scol[c].count & SR_AFFINE);
@@ -562,8 +654,16 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
             float vor[SR_EPI_COLS], voi[SR_EPI_COLS], ver[SR_EPI_COLS], vei[SR_EPI_COLS];
             tmem_ld8_nowait(tbase + (uint32_t)c0, vor);
             tmem_ld8_nowait(tbase + (uint32_t)(NB + c0), voi);
-            tmem_ld8_nowait(tbase + (uint32_t)(2 * NB + c0), ver);
-            tmem_ld8_nowait(tbase + (uint32_t)(3 * NB + c0), vei);
+            if (WIDE) {
+#pragma unroll
+                for (int q = 0; q < SR_EPI_COLS; ++q) {
+                    const float2 ev = even[(long long)(c0 + q) * SR_M];
+                    ver[q] = ev.x, vei[q] = ev.y;
+                }
+            } else {
+                tmem_ld8_nowait(tbase + (uint32_t)(2 * NB + c0), ver);
+                tmem_ld8_nowait(tbase + (uint32_t)(3 * NB + c0), vei);
+            }
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             // branch-free per column, so that the columns of a batch overlap in the pipeline
 #pragma unroll

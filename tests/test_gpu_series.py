@@ -198,3 +198,28 @@ def test_theta_split_over_ctas(nqs, oracle):
         assert np.array_equal(e1, e0), "E_loc must not depend on the split of the theta kernel"
         assert np.array_equal(e0, e0b) and np.array_equal(l0, l0b), "run-to-run determinism"
         assert np.abs(l1 - l0).max() <= 2e-7 * max(1.0, np.abs(l_ref).max())
+
+
+def test_wide_column_tiles(nqs, oracle):
+    """More than 128 table columns: the series GEMM tiles them in column tiles of up to 224 and makes two passes over the
+    hidden units (EVEN, parked in a scratch array, then ODD) with one accumulator pair in TMEM at a time.  Every
+    accumulator element sees the same addends in the same order as with tiles of <= 128 columns (NQS_OPT_SERIES_WIDE =
+    1); only the order in which a row's columns are summed changes with the tiling, so the two agree to float32
+    rounding of that sum (not bit for bit) and each is judged against the oracle: TFIM (affine columns), Heisenberg
+    pair flips, a ragged batch; deterministic run to run."""
+    for k, B in ((5, 1000), (4, 777), (5, 129)):
+        w = wl.make_config(k, B=B)
+        e_ref, l_ref = oracle_on(oracle, w, slice(None), "fast")
+        out = {}
+        for mode in (1, 0, 0):
+            nqs.set_option("series_wide", mode)
+            try:
+                e, l, took = run(nqs, w, "series_only")
+            finally:
+                nqs.set_option("series_wide", 0)
+            assert took["path"] == "series" and not took["guard_failed"]
+            check_eloc(e, e_ref, f"c{k} B={B} series_wide={mode}")
+            out.setdefault(mode, []).append(e)
+        assert np.array_equal(out[0][0], out[0][1]), "run-to-run determinism"
+        scale = np.abs(e_ref).max()
+        assert np.abs(out[1][0] - out[0][0]).max() <= 4e-6 * scale, (k, B, np.abs(out[1][0] - out[0][0]).max(), scale)
