@@ -559,6 +559,7 @@ struct ThetaOut {
     nqs_c64* logpsi = nullptr;   // [B]
     bool raw = false;
     uint4* sA = nullptr;         // series operand planes (tensor-core kernel only), with rown / rowmax
+    bool sA_wide = false;        // their layout (series_plane_index)
     float4* rown = nullptr;
     float* rowmax = nullptr;
     const int* gate = nullptr;   // device word: run only if (gate[0] & 1)
@@ -633,6 +634,8 @@ static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, in
     p.logpsi = (float2*)o.logpsi;
     p.raw_theta = o.raw ? 1 : 0;
     p.sA = o.sA;
+    p.sA_wide = o.sA_wide ? 1 : 0;
+    p.sA_tiles = nMT;
     p.rown = o.rown;
     p.rowmax = o.rowmax;
     p.gate = o.gate;
@@ -809,7 +812,8 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         NQS_TRY(S.get(&status, 4));
         NQS_CUDA(cudaMemsetAsync(status, 0, 4 * sizeof(int), st));
         series_table_kernel<<<(unsigned)(nNT * NB), 256, 0, st>>>((const float2*)d_W, (const float2*)d_a, N, M, M_pad,
-                                                                  h->C, NB, h->dev, sB, scols, sterms);
+                                                                  h->C, NB, h->dev, sB, wide ? 1 : 0, scols,
+                                                                  sterms);
         NQS_LAUNCHED();
     }
     NQS_PROF(1, st);
@@ -820,12 +824,13 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         ThetaOut o;
         o.logpsi = d_logpsi;
         o.tp = tp_now ? tp : nullptr;
-        if (fused_pack) o.sA = sA, o.rown = rown, o.rowmax = rowmax, o.S = nS, o.lp_part = lp_part;
+        if (fused_pack) o.sA = sA, o.rown = rown, o.rowmax = rowmax, o.S = nS, o.lp_part = lp_part, o.sA_wide = wide;
         NQS_TRY(launch_theta(D, d_spins, B, N, M, M_pad, d_a, d_b, d_W, nPairsPad, o, st));
     }
     NQS_PROF(2, st);
     if (use_series && !fused_pack) {
-        series_pack_kernel<<<(unsigned)(B_pad / SR_M), 256, 0, st>>>(tp, nPairsPad, M_pad, sA, rown, rowmax);
+        series_pack_kernel<<<(unsigned)(B_pad / SR_M), 256, 0, st>>>(tp, nPairsPad, M_pad, sA, wide ? 1 : 0, rown,
+                                                                             rowmax);
         NQS_LAUNCHED();
     }
     NQS_PROF(3, st);
@@ -838,6 +843,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
         SeriesGemmParams gp;
         gp.A_packed = sA;
         gp.B_packed = sB;
+        gp.nMT = B_pad / SR_M;
         gp.cols = scols;
         gp.terms = sterms;
         gp.rown = rown;

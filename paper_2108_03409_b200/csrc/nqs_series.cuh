@@ -108,7 +108,8 @@ __device__ __forceinline__ unsigned pack_h2(float a, float b) {
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restrict__ W, const float2* __restrict__ a,
                                                            int N, int M, int M_pad, int C, int NB, DevHam H,
-                                                           uint4* __restrict__ B_packed, SeriesCol* __restrict__ cols,
+                                                           uint4* __restrict__ B_packed, int wide,
+                                                           SeriesCol* __restrict__ cols,
                                                            SeriesTerms* __restrict__ terms) {
     const int c = blockIdx.x, tid = threadIdx.x;
     const int nt = c / NB, cl = c % NB;
@@ -156,10 +157,11 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
             }
         }
         const int jc = j8 >> 1, slab = j8 & 1;
-        uint4* dst = B_packed + (((long long)nt * nJC + jc) * SR_PLANES) * (2 * NB) + slab * NB + cl;
+        uint4* const dst = B_packed + slab * NB + cl;
+        const int nNT = gridDim.x / NB;
 #pragma unroll
         for (int pl = 0; pl < SR_PLANES; ++pl)
-            dst[(long long)pl * 2 * NB] = make_uint4(pack_h2(v[pl][0], v[pl][1]), pack_h2(v[pl][2], v[pl][3]),
+            dst[series_plane_index(wide != 0, nt, jc, pl, nNT, nJC) * (2 * NB)] = make_uint4(pack_h2(v[pl][0], v[pl][1]), pack_h2(v[pl][2], v[pl][3]),
                                                      pack_h2(v[pl][4], v[pl][5]), pack_h2(v[pl][6], v[pl][7]));
     }
     // block reduction in a fixed order (deterministic)
@@ -253,7 +255,7 @@ __global__ void __launch_bounds__(256) series_table_kernel(const float2* __restr
 // rown[b] = (n2t, n4t, n6t, n8t), nPt = sqrt(sum_j |t_bj|^P);  rowmax[b] = max_j |t_bj|
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) series_pack_kernel(const float4* __restrict__ tp, long long nPairsPad, int M_pad,
-                                                          uint4* __restrict__ A_packed, float4* __restrict__ rown,
+                                                          uint4* __restrict__ A_packed, int wide, float4* __restrict__ rown,
                                                           float* __restrict__ rowmax) {
     const int tid = threadIdx.x, pl = tid & 63, jsub = tid >> 6;
     const long long mt = blockIdx.x;
@@ -264,7 +266,7 @@ __global__ void __launch_bounds__(256) series_pack_kernel(const float4* __restri
         float4 t[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) t[q] = tp[(long long)(j8 * 8 + q) * nPairsPad + pair];
-        uint4* dst = A_packed + ((mt * nJC + (j8 >> 1)) * SR_PLANES) * SR_A_PLANE_U4 + (j8 & 1) * SR_M + 2 * pl;
+        uint4* const dst = A_packed + (j8 & 1) * SR_M + 2 * pl;
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             float v[SR_PLANES][8];
@@ -290,7 +292,7 @@ __global__ void __launch_bounds__(256) series_pack_kernel(const float4* __restri
             }
 #pragma unroll
             for (int p = 0; p < SR_PLANES; ++p)
-                dst[p * SR_A_PLANE_U4 + h] = make_uint4(pack_h2(v[p][0], v[p][1]), pack_h2(v[p][2], v[p][3]),
+                dst[series_plane_index(wide != 0, mt, j8 >> 1, p, gridDim.x, nJC) * SR_A_PLANE_U4 + h] = make_uint4(pack_h2(v[p][0], v[p][1]), pack_h2(v[p][2], v[p][3]),
                                                         pack_h2(v[p][4], v[p][5]), pack_h2(v[p][6], v[p][7]));
         }
     }
@@ -359,8 +361,9 @@ __device__ __forceinline__ float spin_from_bits(const uint32_t* __restrict__ bit
 }
 
 struct SeriesGemmParams {
-    const uint4* A_packed;   // [nMT][nJC][8][256]
-    const uint4* B_packed;   // [nNT][nJC][8][2 NB]
+    const uint4* A_packed;   // [nMT][nJC][8][256];  WIDE: the wide layout of series_plane_index (planes of 256 uint4)
+    const uint4* B_packed;   // [nNT][nJC][8][2 NB]; WIDE: the same with planes of 2 NB uint4
+    long long nMT;           // sample tiles in A_packed
     const SeriesCol* cols;   // [nNT * NB]
     const SeriesTerms* terms;  // [nNT * NB]
     const float4* rown;      // [B_pad] (n2t, n4t, n6t, n8t);  nS > 1: [nS][B_pad] partial sums of |t|^P (theta kernel split
@@ -445,24 +448,26 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
             const uint4* gB = p.B_packed + (long long)nt * nJC * SR_PLANES * (2 * NB);
             const uint32_t a_plane = SR_A_PLANE_U4 * 16;
             if (WIDE) {
-                // pass A: the square planes (4, 5) of both operands; pass B: hi, lo (planes 0 .. 3) and cube (6, 7)
-                for (int it = 0; it < 2 * nJC; ++it) {
-                    const int s = it % SR_STAGES, kc = it < nJC ? it : it - nJC;
+                // pass A: the square planes of three chunks per stage (contiguous in the wide layout); pass B: the six
+                // planes hi, lo, cube of one chunk per stage.  Two bulk copies per stage either way.
+                const unsigned char* const baseA = reinterpret_cast<const unsigned char*>(p.A_packed);
+                const unsigned char* const baseB = reinterpret_cast<const unsigned char*>(p.B_packed);
+                const int nA = (nJC + 2) / 3;
+                for (int it = 0; it < nA + nJC; ++it) {
+                    const int s = it % SR_STAGES;
                     mbar_wait(&empty[s], ((it / SR_STAGES) & 1) ^ 1);
                     unsigned char* const stA = sr_smem + (size_t)s * stage_bytes;
                     unsigned char* const stB = stA + A_STAGE;
-                    const unsigned char* const srcA = reinterpret_cast<const unsigned char*>(gA + (long long)kc * SR_PLANES * SR_A_PLANE_U4);
-                    const unsigned char* const srcB = reinterpret_cast<const unsigned char*>(gB + (long long)kc * SR_PLANES * (2 * NB));
-                    if (it < nJC) {
-                        mbar_expect_tx(&full[s], 2 * a_plane + 2 * b_plane);
-                        bulk_g2s(stA, srcA + 4 * a_plane, 2 * a_plane, &full[s]);
-                        bulk_g2s(stB, srcB + 4 * b_plane, 2 * b_plane, &full[s]);
+                    if (it < nA) {
+                        const int kc = 3 * it, nc = min(3, nJC - kc);
+                        mbar_expect_tx(&full[s], (uint32_t)nc * 2 * (a_plane + b_plane));
+                        bulk_g2s(stA, baseA + series_plane_index(true, mt, kc, 4, p.nMT, nJC) * a_plane, (uint32_t)nc * 2 * a_plane, &full[s]);
+                        bulk_g2s(stB, baseB + series_plane_index(true, nt, kc, 4, p.nNT, nJC) * b_plane, (uint32_t)nc * 2 * b_plane, &full[s]);
                     } else {
-                        mbar_expect_tx(&full[s], 6 * a_plane + 6 * b_plane);
-                        bulk_g2s(stA, srcA, 4 * a_plane, &full[s]);
-                        bulk_g2s(stA + 4 * a_plane, srcA + 6 * a_plane, 2 * a_plane, &full[s]);
-                        bulk_g2s(stB, srcB, 4 * b_plane, &full[s]);
-                        bulk_g2s(stB + 4 * b_plane, srcB + 6 * b_plane, 2 * b_plane, &full[s]);
+                        const int kc = it - nA;
+                        mbar_expect_tx(&full[s], 6 * (a_plane + b_plane));
+                        bulk_g2s(stA, baseA + series_plane_index(true, mt, kc, 0, p.nMT, nJC) * a_plane, 6 * a_plane, &full[s]);
+                        bulk_g2s(stB, baseB + series_plane_index(true, nt, kc, 0, p.nNT, nJC) * b_plane, 6 * b_plane, &full[s]);
                     }
                 }
             } else {
@@ -494,19 +499,22 @@ __global__ void __launch_bounds__(SR_THREADS, 1) series_gemm_kernel(const Series
                 umma_f16(dim, A(pa + 1), Bd(pb), idesc, 1u);
             };
             if (WIDE) {
-                for (int it = 0; it < 2 * nJC; ++it) {
+                const int nA = (nJC + 2) / 3;
+                for (int it = 0; it < nA + nJC; ++it) {
                     const int s = it % SR_STAGES;
-                    if (it == nJC) {  // EVEN is complete: hand it to the epilogue warps, wait until it has left TMEM
+                    if (it == nA) {  // EVEN is complete: hand it to the epilogue warps, wait until it has left TMEM
                         tc_commit(t_full);
                         mbar_wait(t_free, 0);
                     }
                     mbar_wait(&full[s], (it / SR_STAGES) & 1);
                     tc_fence_after();
                     sa = s0 + (uint32_t)s * stage_bytes, sb = sa + A_STAGE;
-                    if (it < nJC) {
-                        cprod(0, 0, d_er, d_ei, it ? 1u : 0u);          // t^2 T^2 / 2  (stage slots 0, 1)
+                    if (it < nA) {
+                        const int nc = min(3, nJC - 3 * it);
+                        for (int u = 0; u < nc; ++u)
+                            cprod(2 * u, 2 * u, d_er, d_ei, (it | u) ? 1u : 0u);   // t^2 T^2 / 2 of chunk 3 it + u
                     } else {
-                        const uint32_t first = it > nJC ? 1u : 0u;
+                        const uint32_t first = it > nA ? 1u : 0u;
                         cprod(0, 0, d_or, d_oi, first);   // t.hi T.hi
                         cprod(0, 2, d_or, d_oi, 1u);      // t.hi T.lo
                         cprod(2, 0, d_or, d_oi, 1u);      // t.lo T.hi

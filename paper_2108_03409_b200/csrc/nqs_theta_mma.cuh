@@ -205,6 +205,16 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 //   16 t^3 (re im);   rown[b] = (n2t, n4t, n6t, n8t), nPt = sqrt(sum_j |t_bj|^P);   rowmax[b] = max_j |t_bj|
 constexpr float TM_SERIES_SA = 16.f;  // == SR_SA of nqs_series.cuh (static_assert there)
 
+// Index (in planes) of plane pl (0 .. 7: hi.re hi.im lo.re lo.im sq.re sq.im cu.re cu.im) of chunk jc of tile `tile` in a
+// packed operand array of nTiles x nJC chunks.  Narrow layout: eight planes per chunk, contiguous.  Wide layout (column
+// tiles of up to 224, nqs_series.cuh): the six planes of the ODD pass per chunk, contiguous, and behind all of them the
+// two square planes of every chunk, contiguous over the chunks of a tile -- one bulk copy fetches three chunks of them.
+__host__ __device__ inline long long series_plane_index(bool wide, long long tile, int jc, int pl, long long nTiles, int nJC) {
+    if (!wide) return (tile * nJC + jc) * 8 + pl;
+    if (pl == 4 || pl == 5) return nTiles * nJC * 6 + (tile * nJC + jc) * 2 + (pl - 4);
+    return (tile * nJC + jc) * 6 + (pl < 4 ? pl : pl - 2);
+}
+
 struct ThetaMmaParams {
     const uint4* A_packed;   // [nMT][K16][128]
     const uint4* B_packed;   // [nNT][K16][256]
@@ -219,6 +229,8 @@ struct ThetaMmaParams {
     float2* logpsi;          // [B] or nullptr
     int raw_theta;           // 1: tp receives theta itself instead of tanh(theta) (nqs_metropolis)
     uint4* sA;               // series operand planes or nullptr
+    int sA_wide;             // their layout (series_plane_index)
+    long long sA_tiles;      // sample tiles in sA
     float4* rown;            // [rows] (with sA)
     float* rowmax;           // [rows] (with sA)
     const int* gate;         // nullptr, or: run only if (gate[0] & 1) -- the series guard failed (fallback pass)
@@ -423,9 +435,11 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
                         wd[6][pq] = tm_pack_h2(cr);
                         wd[7][pq] = tm_pack_h2(ci);
                     }
-                    uint4* dst = p.sA + ((mt * nJC + (jbase >> 4)) * 8) * (2 * TM_M) + ((jbase >> 3) & 1) * TM_M + row;
+                    uint4* const dst = p.sA + ((jbase >> 3) & 1) * TM_M + row;
 #pragma unroll
-                    for (int pl = 0; pl < 8; ++pl) dst[pl * 2 * TM_M] = make_uint4(wd[pl][0], wd[pl][1], wd[pl][2], wd[pl][3]);
+                    for (int pl = 0; pl < 8; ++pl)
+                        dst[series_plane_index(p.sA_wide != 0, mt, jbase >> 4, pl, p.sA_tiles, nJC) * (2 * TM_M)] =
+                            make_uint4(wd[pl][0], wd[pl][1], wd[pl][2], wd[pl][3]);
                 }
             }
         }
