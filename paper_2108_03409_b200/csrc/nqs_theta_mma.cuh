@@ -435,11 +435,19 @@ __global__ void __launch_bounds__(TM_THREADS, 2) theta_mma_kernel(const ThetaMma
                         wd[6][pq] = tm_pack_h2(cr);
                         wd[7][pq] = tm_pack_h2(ci);
                     }
+                    // planes 0 .. 3 (hi, lo) and 6, 7 (cube) from `dm`, planes 4, 5 (square) from `dq` (series_plane_index)
+                    const bool wide = p.sA_wide != 0;
                     uint4* const dst = p.sA + ((jbase >> 3) & 1) * TM_M + row;
+                    uint4* const dm = dst + series_plane_index(wide, mt, jbase >> 4, 0, p.sA_tiles, nJC) * (2 * TM_M);
+                    uint4* const dq = dst + series_plane_index(wide, mt, jbase >> 4, 4, p.sA_tiles, nJC) * (2 * TM_M);
+                    uint4* const dc = dm + (wide ? 4 : 6) * (2 * TM_M);
 #pragma unroll
-                    for (int pl = 0; pl < 8; ++pl)
-                        dst[series_plane_index(p.sA_wide != 0, mt, jbase >> 4, pl, p.sA_tiles, nJC) * (2 * TM_M)] =
-                            make_uint4(wd[pl][0], wd[pl][1], wd[pl][2], wd[pl][3]);
+                    for (int pl = 0; pl < 4; ++pl) dm[pl * 2 * TM_M] = make_uint4(wd[pl][0], wd[pl][1], wd[pl][2], wd[pl][3]);
+#pragma unroll
+                    for (int pl = 0; pl < 2; ++pl) {
+                        dq[pl * 2 * TM_M] = make_uint4(wd[4 + pl][0], wd[4 + pl][1], wd[4 + pl][2], wd[4 + pl][3]);
+                        dc[pl * 2 * TM_M] = make_uint4(wd[6 + pl][0], wd[6 + pl][1], wd[6 + pl][2], wd[6 + pl][3]);
+                    }
                 }
             }
         }
