@@ -35,8 +35,8 @@ L2_FLUSH_BYTES = 256 << 20
 # summarised under profiles/ -- (workload, kernel) -> (bytes, file).  No capture for that pair => traffic is null.
 NCU_DRAM_TRAFFIC = {
     ("c5_tfim_20x20", "eloc_kernel"): (897_815_552, "profiles/r1_v3_ncu_summary.md"),
-    ("c5_tfim_20x20", "series_gemm_kernel"): (1_834_899_000, "profiles/r2c_ncu_summary.md"),
-    ("c2_tfim_chain_N40", "small_eloc_kernel"): (780_800, "profiles/r2c_ncu_summary.md"),
+    ("c5_tfim_20x20", "series_gemm_kernel"): (2_227_869_000, "profiles/r2d_ncu_summary.md"),
+    ("c2_tfim_chain_N40", "small_eloc_kernel"): (780_800, "profiles/r2d_ncu_summary.md"),
 }
 # nominal ratio of the dense INT8 to the dense BF16/FP16 tensor peak (B200_PROFILING.md: 4.5 vs 2.25 P)
 INT8_OVER_BF16 = 2.0
