@@ -350,6 +350,10 @@ def run_ours(args) -> None:
                     "peak_source": "148 SMs x 128 FP32 lanes x 2 x clocks.max.sm (DESIGN.md); FMA = 2 flop; "
                                    "algorithmic work = 8 FMA per (sample, column, hidden unit)"}
         traffic = NCU_DRAM_TRAFFIC.get((w.name, dom))
+        if (w.name, dom) == ("c5_tfim_20x20", "series_gemm_kernel"):
+            # context from the same ncu capture (not measured in this run): the chip is power-limited under tensor load
+            roof["ncu_context"] = {"sm_ghz_during_kernel": 1.515, "tensor_pipe_active": 0.837,
+                                   "l2_to_sm_fill_bytes": 9_121_392_000, "source": "profiles/r2d_ncu_summary.md"}
         roof["traffic"] = traffic[0] if traffic else None
         roof["traffic_source"] = traffic[1] if traffic else "no ncu --set full capture of this kernel at this workload"
         # FP32 floor of the cheapest FP32 formulation (SURVEY 8(d) rule (i)): product-form a5 + per-unit work, and a2
