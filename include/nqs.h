@@ -96,8 +96,8 @@ int nqs_local_energy(const int8_t *d_spins, int64_t B, int32_t N, int32_t M, con
                      nqs_c64 *d_logpsi, void *stream);
 
 /* Same with HOST buffers for everything (spins, parameters, outputs): H2D copies, kernels,
- * D2H copies, stream synchronise.  h_logpsi may be NULL.  Batches of 65536 samples and more go through
- * the device in chunks of >= 32768 samples on two library-owned streams, so that the copy of chunk k + 1
+ * D2H copies, stream synchronise.  h_logpsi may be NULL.  Batches of more than ~47000 samples go through
+ * the device in chunks of 37888 samples (B200) on two library-owned streams, so that the copy of chunk k + 1
  * overlaps the kernels of chunk k (pinned host buffers are needed for the overlap; pageable ones work,
  * serially).  Calls on the same device are serialised. */
 int nqs_local_energy_host(const int8_t *h_spins, int64_t B, int32_t N, int32_t M, const nqs_c64 *h_a,
@@ -174,8 +174,9 @@ int nqs_local_energy_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t 
  *                       GEMM then makes two passes over the hidden units with one accumulator pair in TMEM at a time,
  *                       csrc/nqs_series.cuh) where that fits in shared memory           1 = tiles of <= 128 columns only;
  *                       the two give the same bits
- *   NQS_OPT_HOST_CHUNKS 0 = automatic: nqs_local_energy_host sends the batch through the device in B / 32768 chunks
- *                       (at most 16), copying chunk k + 1 while the kernels of chunk k run      1 .. 16 = that many
+ *   NQS_OPT_HOST_CHUNKS 0 = automatic: nqs_local_energy_host sends the batch through the device in chunks of 2 x SMs x 128
+ *                       samples (whole waves of the kernels; at most 16 chunks, a short remainder joins the last),
+ *                       copying chunk k + 1 while the kernels of chunk k run      1 .. 16 = that many equal chunks
  * nqs_debug_last_a5 (synchronises `stream`; tests only; not meaningful while calls run concurrently on other
  * streams): out[0] = 1 if the most recent nqs_local_energy* call on this device attempted the series path, 2 if
  * it used the product form only, 3 if the single-launch kernel for small problems ran; out[1] = 1 if the guard failed; out[2] = samples over the guard threshold.

@@ -1043,8 +1043,8 @@ extern "C" int nqs_enumerate_connected(const int8_t* d_spins, int64_t B, int32_t
 // Host buffers in, host buffers out (the end-to-end leg of bench.py).  The batch goes through the device in chunks:
 // the parameters and the first chunk of spins are copied, then the kernels of chunk k run on the compute stream while
 // the copy stream brings chunk k + 1 -- the transfer of all but the first chunk hides behind the kernels.  Chunks are
-// at least HOST_CHUNK_MIN samples (a chunk must still fill the 296 CTA slots of the theta kernel) and a multiple of
-// 256; every sample's result is independent of the chunking except that the series guard decides per chunk.
+// whole waves of the kernels (2 x SMs sample tiles of 128 = 37888 samples on a B200, at least HOST_CHUNK_MIN); every
+// sample's result is independent of the chunking except that the series guard decides per chunk.
 constexpr int64_t HOST_CHUNK_MIN = 32768;
 
 static int host_streams(DeviceState* D) {
@@ -1087,10 +1087,25 @@ extern "C" int nqs_local_energy_host(const int8_t* h_spins, int64_t B, int32_t N
     NQS_TRY(S.get(&dW, (size_t)M * N));
     NQS_TRY(S.get(&de, (size_t)B));
     if (h_logpsi) NQS_TRY(S.get(&dl, (size_t)B));
-    int nChunks = (int)std::min<int64_t>(HOST_MAX_CHUNKS, std::max<int64_t>(1, B / HOST_CHUNK_MIN));
+    // chunk boundaries: automatic = whole waves of the kernels -- 2 x SMs sample tiles of 128 fill the CTA slots of the
+    // theta kernel exactly once and give the series GEMM a multiple of SMs CTAs whatever the number of column tiles; a
+    // short remainder joins the chunk before it.  NQS_OPT_HOST_CHUNKS = n: n equal chunks.
+    int64_t start[HOST_MAX_CHUNKS + 1];
+    int nChunks = 0;
     const int forced = g_opt[NQS_OPT_HOST_CHUNKS].load();
-    if (forced > 0) nChunks = (int)std::min<int64_t>(forced, (B + 255) / 256);
-    const int64_t per = round_up((B + nChunks - 1) / nChunks, 256);
+    if (forced > 0) {
+        nChunks = (int)std::min<int64_t>(forced, (B + 255) / 256);
+        const int64_t per = round_up((B + nChunks - 1) / nChunks, 256);
+        for (int k = 0; k <= nChunks; ++k) start[k] = std::min<int64_t>(B, k * per);
+    } else {
+        const int64_t unit = std::max<int64_t>(HOST_CHUNK_MIN, 2ll * D->sms * 128);
+        start[0] = 0;
+        while (nChunks < HOST_MAX_CHUNKS - 1 && B - start[nChunks] >= unit + unit / 4) {
+            start[nChunks + 1] = start[nChunks] + unit;
+            ++nChunks;
+        }
+        start[++nChunks] = B;
+    }
     // the blocks were allocated in the order of `comp`: the copy stream may touch them after this point of it
     NQS_CUDA(cudaEventRecord(D->host_ev[HOST_MAX_CHUNKS], comp));
     NQS_CUDA(cudaStreamWaitEvent(copy, D->host_ev[HOST_MAX_CHUNKS], 0));
@@ -1098,14 +1113,14 @@ extern "C" int nqs_local_energy_host(const int8_t* h_spins, int64_t B, int32_t N
     NQS_CUDA(cudaMemcpyAsync(db, h_b, sizeof(nqs_c64) * M, cudaMemcpyHostToDevice, copy));
     NQS_CUDA(cudaMemcpyAsync(dW, h_W, sizeof(nqs_c64) * (size_t)M * N, cudaMemcpyHostToDevice, copy));
     for (int k = 0; k < nChunks; ++k) {
-        const int64_t b0 = k * per, nb = std::min<int64_t>(per, B - b0);
-        if (nb <= 0) break;
+        const int64_t b0 = start[k], nb = start[k + 1] - b0;
+        if (nb <= 0) continue;
         NQS_CUDA(cudaMemcpyAsync(ds + b0 * N, h_spins + b0 * N, (size_t)nb * N, cudaMemcpyHostToDevice, copy));
         NQS_CUDA(cudaEventRecord(D->host_ev[k], copy));
     }
     for (int k = 0; k < nChunks; ++k) {
-        const int64_t b0 = k * per, nb = std::min<int64_t>(per, B - b0);
-        if (nb <= 0) break;
+        const int64_t b0 = start[k], nb = start[k + 1] - b0;
+        if (nb <= 0) continue;
         NQS_CUDA(cudaStreamWaitEvent(comp, D->host_ev[k], 0));
         NQS_TRY(nqs_local_energy_h(h.get(), ds + b0 * N, nb, M, da, db, dW, de + b0, dl ? dl + b0 : nullptr, comp));
         NQS_CUDA(cudaMemcpyAsync(h_eloc + b0, de + b0, sizeof(nqs_c64) * nb, cudaMemcpyDeviceToHost, comp));
