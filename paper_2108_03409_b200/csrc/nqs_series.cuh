@@ -13,7 +13,10 @@
 // size |x| and |x|^2).  Complex arithmetic = four real MMAs per product, the minus sign of Re by the
 // negate-A bit of the instruction descriptor.  5 products x 4 = 20 MMAs (M = 128, N = NB, K = 16) per
 // 16 hidden units; all odd-k products accumulate into one pair (re, im) of TMEM column ranges and the
-// even-k product into a second one, so an accumulator tile is 4 NB <= 512 TMEM columns.
+// even-k product into a second one, so an accumulator tile is 4 NB <= 512 TMEM columns (NB <= 128).  Hamiltonians
+// with more than 128 table columns take column tiles of NB <= 224 instead, with ONE pair in TMEM at a time and two
+// passes over the hidden units (series_gemm_kernel<true>): fewer operand bytes into the SM per MAC, which is what
+// bounds the narrow kernel's main loop.
 //
 // The series is only valid where |t T| is small.  The kernel evaluates, per sample, a bound on the
 // error it made (truncation + FP16 operand rounding, from row norms of t and column norms of T by
