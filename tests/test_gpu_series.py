@@ -50,12 +50,18 @@ def run(nqs, w, path):
     (33, 40, 515, 200, 0.003, 304),  # > 128 columns: two column tiles
     (70, 33, 300, 700, 0.001, 305),  # many pair-flip groups, both parities
 ])
-def test_series_only_random_terms_vs_definition(nqs, oracle, N, M, B, T, sigma, seed):
+@pytest.mark.parametrize("narrow_only", [0, 1])
+def test_series_only_random_terms_vs_definition(nqs, oracle, N, M, B, T, sigma, seed, narrow_only):
     """Small parameters (inside the guard), general term lists: the series kernel ALONE (no fallback) against
-    definition mode -- matrix elements, parities, diagonal, ragged tiles.  (Random complex coefficients make
-    sum |m| large against |E_loc|, so the guard is strict here: sigma is chosen small.)"""
+    definition mode -- matrix elements, parities, diagonal, ragged tiles; with the default tiling (wide two-pass
+    column tiles where there are more than 128 columns) and with narrow tiles only.  (Random complex coefficients
+    make sum |m| large against |E_loc|, so the guard is strict here: sigma is chosen small.)"""
     w = wl.make_random(N, M, B, T, sigma, seed)
-    e, l, took = run(nqs, w, "series_only")
+    nqs.set_option("series_wide", narrow_only)
+    try:
+        e, l, took = run(nqs, w, "series_only")
+    finally:
+        nqs.set_option("series_wide", 0)
     assert took["path"] == "series" and not took["guard_failed"], took
     e_ref, l_ref = oracle_on(oracle, w, slice(None), "definition")
     check_eloc(e, e_ref, f"series N={N}")
