@@ -35,8 +35,8 @@ L2_FLUSH_BYTES = 256 << 20
 # summarised under profiles/ -- (workload, kernel) -> (bytes, file).  No capture for that pair => traffic is null.
 NCU_DRAM_TRAFFIC = {
     ("c5_tfim_20x20", "eloc_kernel"): (897_815_552, "profiles/r1_v3_ncu_summary.md"),
-    ("c5_tfim_20x20", "series_gemm_kernel"): (2_227_869_000, "profiles/r2d_ncu_summary.md"),
-    ("c2_tfim_chain_N40", "small_eloc_kernel"): (780_800, "profiles/r2d_ncu_summary.md"),
+    ("c5_tfim_20x20", "series_gemm_kernel"): (2_228_427_000, "profiles/r2e_ncu_summary.md"),
+    ("c2_tfim_chain_N40", "small_eloc_kernel"): (780_800, "profiles/r2e_ncu_summary.md"),
 }
 # nominal ratio of the dense INT8 to the dense BF16/FP16 tensor peak (B200_PROFILING.md: 4.5 vs 2.25 P)
 INT8_OVER_BF16 = 2.0
@@ -353,7 +353,7 @@ def run_ours(args) -> None:
         if (w.name, dom) == ("c5_tfim_20x20", "series_gemm_kernel"):
             # context from the same ncu capture (not measured in this run): the chip is power-limited under tensor load
             roof["ncu_context"] = {"sm_ghz_during_kernel": 1.515, "tensor_pipe_active": 0.837,
-                                   "l2_to_sm_fill_bytes": 9_121_392_000, "source": "profiles/r2d_ncu_summary.md"}
+                                   "l2_to_sm_fill_bytes": 9_121_392_000, "source": "profiles/r2e_ncu_summary.md"}
         roof["traffic"] = traffic[0] if traffic else None
         roof["traffic_source"] = traffic[1] if traffic else "no ncu --set full capture of this kernel at this workload"
         # FP32 floor of the cheapest FP32 formulation (SURVEY 8(d) rule (i)): product-form a5 + per-unit work, and a2
