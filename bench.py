@@ -352,7 +352,7 @@ def run_ours(args) -> None:
         traffic = NCU_DRAM_TRAFFIC.get((w.name, dom))
         if (w.name, dom) == ("c5_tfim_20x20", "series_gemm_kernel"):
             # context from the same ncu capture (not measured in this run): the chip is power-limited under tensor load
-            roof["ncu_context"] = {"sm_ghz_during_kernel": 1.515, "tensor_pipe_active": 0.837,
+            roof["ncu_context"] = {"sm_ghz_during_kernel": 1.48, "tensor_pipe_active": 0.837,
                                    "l2_to_sm_fill_bytes": 9_121_392_000, "source": "profiles/r2e_ncu_summary.md"}
         roof["traffic"] = traffic[0] if traffic else None
         roof["traffic_source"] = traffic[1] if traffic else "no ncu --set full capture of this kernel at this workload"
