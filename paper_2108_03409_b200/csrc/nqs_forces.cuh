@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(256) force_gscale_kernel(const float4* __restr
     }
 }
 
-// B operand: thread <-> (row j', k16 = 16 consecutive samples).  G 2^(27-e) rounded to an integer Q,
+// B operand: thread <-> (row j', k16 = 16 consecutive samples), consecutive threads <-> consecutive j'.  G 2^(27-e) rounded to an integer Q,
 // |Q| <= 2^27, digits d0..d3: Q = d0 + 128 d1 + 128^2 d2 + 128^3 d3, d0..d2 in [-64, 63].
 // B_packed[jtile][k16][n = 8*jl + 4*part + digit][16 bytes]: a thread writes one 128-byte line.
 __global__ void __launch_bounds__(256) force_pack_g_kernel(const float4* __restrict__ tp, long long nPairsPad,
@@ -129,8 +129,11 @@ __global__ void __launch_bounds__(256) force_pack_g_kernel(const float4* __restr
                                                            uint4* __restrict__ B_packed) {
     const long long total = (long long)nJT * TM_JT * K16;
     for (long long idx = blockIdx.x * 256ll + threadIdx.x; idx < total; idx += (long long)gridDim.x * 256) {
-        const int k16 = (int)(idx % K16);
-        const int j = (int)(idx / K16);
+        // lanes <-> 32 consecutive hidden units of one 16-sample slab: a warp writes one contiguous 4 KB block of
+        // B_packed and reads whole 128-byte lines of tp (each lane its own), the coefficients by broadcast
+        const int nJ = nJT * TM_JT;
+        const int j = (int)(idx % nJ);
+        const int k16 = (int)(idx / nJ);
         const int e = gexp[j];
         unsigned d[2][4][4];
 #pragma unroll
