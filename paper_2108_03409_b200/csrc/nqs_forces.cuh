@@ -56,16 +56,23 @@ __global__ void __launch_bounds__(256) stats_partial_kernel(const float2* __rest
     if (threadIdx.x < 4) partial[blockIdx.x * 4 + threadIdx.x] = sh[threadIdx.x][0];
 }
 
+// one warp: lane l adds the partials l, l + 32, ... in that order, lane 0 then adds the 32 lane sums in lane order
+// (a fixed order: deterministic; the 1024 dependent loads of a single thread took 40 us)
 __global__ void stats_final_kernel(const double* __restrict__ partial, int nblk, double* __restrict__ stats) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    if (blockIdx.x != 0 || threadIdx.x >= 32) return;
+    const int lane = threadIdx.x;
     double s[4] = {0, 0, 0, 0};
-    for (int k = 0; k < nblk; ++k)
+    for (int k = lane; k < nblk; k += 32)
         for (int q = 0; q < 4; ++q) s[q] += partial[k * 4 + q];
-    const double mr = s[1] / s[0], mi = s[2] / s[0];
+    double t[4] = {0, 0, 0, 0};
+    for (int l = 0; l < 32; ++l)
+        for (int q = 0; q < 4; ++q) t[q] += __shfl_sync(0xffffffffu, s[q], l);
+    if (lane != 0) return;
+    const double mr = t[1] / t[0], mi = t[2] / t[0];
     stats[0] = mr;
     stats[1] = mi;
-    stats[2] = s[3] / s[0] - (mr * mr + mi * mi);
-    stats[3] = s[0];
+    stats[2] = t[3] / t[0] - (mr * mr + mi * mi);
+    stats[3] = t[0];
 }
 
 // c_b = w_b (E_b - mean) / sum w as float2; 0 for the padding samples b >= B
