@@ -254,32 +254,58 @@ __global__ void __launch_bounds__(SM_MAX_THREADS) small_eloc_kernel(const SmallP
     __syncthreads();
     NQS_SSTAMP(4);
 
-    // a6 (+ the visible bias of log psi): one thread per sample, fixed order
-    for (int r = tid; r < SB; r += SM_THREADS) {
+    // a6 (+ the visible bias of log psi): four adjacent lanes per sample, each a quarter of the diagonal terms, of the
+    // columns and of the sites; the four partial sums are added in lane order (fixed: deterministic)
+    for (int base = 0; base < 4 * SB; base += SM_THREADS) {
+        const int item = base + tid;
+        const bool on = item < 4 * SB;                      // whole warps stay in the loop for the shuffles
+        const int r = on ? item >> 2 : 0, q4 = item & 3;
         const long long b = b0 + r;
-        if (b >= p.B) continue;
         const int8_t* const srow = sp + r * ss;
-        const float2 d = diagonal_element(p.H, srow);
-        float er = d.x, ei = d.y;
-        for (int c = 0; c < C; ++c) {
-            er += contrib[r * C + c].x;
-            ei += contrib[r * C + c].y;
+        float er = 0.f, ei = 0.f, ar = 0.f, ai = 0.f;
+        if (on) {
+            for (int t = q4; t < p.H.Td; t += 4) {
+                const int z0 = p.H.diag_z0[t], z1 = p.H.diag_z1[t];
+                float f = 1.f;
+                if (z0 >= 0) f *= (float)srow[z0];
+                if (z1 >= 0) f *= (float)srow[z1];
+                if (p.H.has_zx)
+                    for (int x = p.H.diag_zx_off[t]; x < p.H.diag_zx_off[t + 1]; ++x) f *= (float)srow[p.H.diag_zx[x]];
+                const float2 cc = p.H.diag_c[t];
+                er = fmaf(cc.x, f, er);
+                ei = fmaf(cc.y, f, ei);
+            }
+            for (int c = q4; c < C; c += 4) {
+                er += contrib[r * C + c].x;
+                ei += contrib[r * C + c].y;
+            }
+            if (p.logpsi)
+                for (int i = q4; i < N; i += 4) {
+                    const float sv = (float)srow[i];
+                    const float2 av = p.a[i];
+                    ar = fmaf(av.x, sv, ar);
+                    ai = fmaf(av.y, sv, ai);
+                }
         }
-        p.eloc[b] = make_float2(er, ei);
-        if (p.logpsi) {
-            double lr = 0.0, li = 0.0;
-            for (int k = 0; k < JL; ++k) {
-                lr += lp[(r * JL + k) * 2];
-                li += lp[(r * JL + k) * 2 + 1];
+        const int l0 = (tid & 31) & ~3;
+        float sr = 0.f, si = 0.f, br = 0.f, bi = 0.f;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            sr += __shfl_sync(0xffffffffu, er, l0 + k);
+            si += __shfl_sync(0xffffffffu, ei, l0 + k);
+            br += __shfl_sync(0xffffffffu, ar, l0 + k);
+            bi += __shfl_sync(0xffffffffu, ai, l0 + k);
+        }
+        if (on && q4 == 0 && b < p.B) {
+            p.eloc[b] = make_float2(sr, si);
+            if (p.logpsi) {
+                double lr = 0.0, li = 0.0;
+                for (int k = 0; k < JL; ++k) {
+                    lr += lp[(r * JL + k) * 2];
+                    li += lp[(r * JL + k) * 2 + 1];
+                }
+                p.logpsi[b] = make_float2((float)(lr + (double)br), (float)(li + (double)bi));
             }
-            float ar = 0.f, ai = 0.f;
-            for (int i = 0; i < N; ++i) {
-                const float s = (float)srow[i];
-                const float2 av = p.a[i];
-                ar = fmaf(av.x, s, ar);
-                ai = fmaf(av.y, s, ai);
-            }
-            p.logpsi[b] = make_float2((float)(lr + (double)ar), (float)(li + (double)ai));
         }
     }
     __syncthreads();
