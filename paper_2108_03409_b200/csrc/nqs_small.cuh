@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(SM_MAX_THREADS) small_eloc_kernel(const SmallP
                 const int j = j0 + u * JL;
                 wo[u] = (j < M ? j : j0) * N;
             }
-#pragma unroll 2
+#pragma unroll 4
             for (int i = 0; i < N; ++i) {
                 const float2 s2 = bc2((float)srow[i]);
 #pragma unroll
