@@ -227,6 +227,45 @@ int nqs_profile_last(float ms[NQS_PROFILE_SEGMENTS]);
 int nqs_energy_stats(const nqs_c64 *d_x, const float *d_weights, int64_t B, double *d_stats, void *stream);
 
 /* ---------------------------------------------------------------------------------------
+ * nqs_energy_stats for callers that are not able to allocate device memory (Eq. 5).
+ *
+ * Who this is for.  Every other device entry point takes its scratch memory from a pool the library grows with
+ * the CUDA allocator.  That is not possible for a host program whose own allocator has already claimed (almost)
+ * all of the device's memory -- the paper's own environment is the example: a JAX/XLA process reserves the whole
+ * GPU at start-up unless told otherwise, and inside such a process a library-side allocation
+ * simply fails with "out of memory" although the program has plenty of room in its own arena.  It is also not
+ * acceptable in a sampling / optimisation loop with a latency bound, because an allocation that has to go to the
+ * driver may stall the whole device, nor in a deployment where device memory is handed out by a budget the
+ * library is not part of.  Such callers still own d_x, d_weights and d_stats (carved out of their arena) and
+ * pass them in; what they can not provide for is memory the library would take behind their back.
+ *
+ * What it does.  Same arguments, same kernels, same launch geometry and therefore the same bits in d_stats as
+ * nqs_energy_stats.  The difference is where the per-block partial sums live: in a fixed 8 KB array (256 records
+ * of four float64 sums) that is part of the library image itself, so it exists on every GPU that loads the
+ * library, from load until the process exits, and costs nothing at call time.  This entry point makes no call to
+ * cudaMalloc / cudaFree, to the stream-ordered allocator or to any library routine that allocates, and does not
+ * create the library's pool.
+ *
+ * Limit.  B <= NQS_STATS_STATIC_MAX_B (2^26 samples = 512 MiB of complex64 input, 64 times the largest batch the
+ * paper uses, N_MC = 10^6 at PAPER.md:622).  A larger B returns NQS_ERR_UNSUPPORTED with a message that names the
+ * limit; nothing is launched.  (The 256 records are filled by a strided loop, so the array itself does not grow
+ * with B; the cap is the range this entry point is specified and tested for.)
+ *
+ * First call on a device.  The first call made while a given device is current looks up the array's address on
+ * that device (cudaGetSymbolAddress) and remembers it; later calls on that device reuse it.  Make that first call
+ * during set-up, before any stream capture is begun, with the device you mean to use already current.
+ *
+ * One array for everybody.  All calls on a device, from every stream and every thread, use the same 8 KB, and the
+ * array keeps whatever the previous call left in it.  No clearing is needed: each call overwrites every record it
+ * is going to read before it reads it.  But two calls whose kernels can run on the GPU at the same time (different
+ * streams without an event between them, or two host threads on different streams) overwrite each other's partial
+ * sums and both results are then garbage -- keep calls on a device in one stream, or order them with events.
+ * Asynchronous on `stream`; B == 0 is a no-op; weights as in nqs_energy_stats.
+ * ------------------------------------------------------------------------------------- */
+#define NQS_STATS_STATIC_MAX_B (1ll << 26)
+int nqs_energy_stats_static(const nqs_c64 *d_x, const float *d_weights, int64_t B, double *d_stats, void *stream);
+
+/* ---------------------------------------------------------------------------------------
  * Force vector of the RBM (Eq. 16; energy gradient Eq. 7, :81-89):
  *   F_k = <<E_loc O_k^*>>^c = <<O_k^* E_loc>> - <<O_k^*>> <<E_loc>>,
  *   O_k(s) = d log psi(s) / d theta_k (Eq. 8, :93):  O_{a_i} = s_i, O_{b_j} = tanh theta_j,

@@ -10,6 +10,8 @@ from .binding import (  # noqa: F401
     MICROBENCH_KINDS,
     NqsError,
     energy_stats,
+    energy_stats_static,
+    STATS_STATIC_MAX_B,
     A5_PATHS,
     PROFILE_SEGMENTS,
     connected_groups,

@@ -61,6 +61,7 @@ def load_library() -> ctypes.CDLL:
             lib.nqs_fisher.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_vmc_step_h.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_energy_stats.argtypes = [vp, vp, i64, vp, vp]
+            lib.nqs_energy_stats_static.argtypes = [vp, vp, i64, vp, vp]
             lib.nqs_forces.argtypes = [vp, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
             lib.nqs_microbench.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float)]
             lib.nqs_local_energy_forces_h.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -77,7 +78,7 @@ def load_library() -> ctypes.CDLL:
                          "nqs_metropolis_trace", "nqs_set_option", "nqs_get_option", "nqs_debug_last_a5",
                          "nqs_launch_count", "nqs_fisher", "nqs_vmc_step_h", "nqs_hamiltonian_create_k",
                          "nqs_hamiltonian_compile_host_k", "nqs_hamiltonian_info_k", "nqs_local_energy_k",
-                         "nqs_metropolis_shared"):
+                         "nqs_metropolis_shared", "nqs_energy_stats_static"):
                 getattr(lib, name).restype = ctypes.c_int
             _lib = lib
     return _lib
@@ -327,6 +328,34 @@ def energy_stats(x, weights=None):
     stats = torch.empty(4, dtype=torch.float64, device=x.device)
     with torch.cuda.device(x.device):
         _check(load_library().nqs_energy_stats(
+            _dev(x, torch.complex64, "x"), _dev(weights, torch.float32, "weights") if weights is not None else None,
+            x.shape[0], ctypes.c_void_p(stats.data_ptr()), _stream()))
+    return stats
+
+
+STATS_STATIC_MAX_B = 1 << 26  # NQS_STATS_STATIC_MAX_B of include/nqs.h
+
+
+def energy_stats_static(x, weights=None, out=None):
+    """nqs_energy_stats_static: nqs_energy_stats for a caller that can not let the library allocate.
+
+    Meant for a program whose own allocator already holds the GPU's memory (a JAX/XLA process with preallocation
+    on, as in the paper's set-up), or that runs under a memory budget or a latency bound: the library takes
+    nothing from the CUDA allocator here, its partial sums sit in a fixed 8 KB array inside the library image.
+    The caller brings the output too: `out` is a float64 CUDA tensor [4] from the caller's own memory and is
+    returned filled with (Re mean, Im mean, variance, sum of weights).  Only when `out` is None does this wrapper
+    make one with torch.empty, as a convenience for tests -- that allocation is torch's, outside the library.
+    x.shape[0] must not exceed STATS_STATIC_MAX_B (NqsError NQS_ERR_UNSUPPORTED otherwise).  All calls on a
+    device share the array: run them on one stream or order them with events, and make the first call on each
+    device before any stream capture starts (include/nqs.h).
+    """
+    import torch
+
+    stats = torch.empty(4, dtype=torch.float64, device=x.device) if out is None else out
+    if stats.dtype != torch.float64 or stats.numel() != 4 or not stats.is_cuda or not stats.is_contiguous():
+        raise ValueError("out must be a contiguous float64 CUDA tensor of 4 elements")
+    with torch.cuda.device(x.device):
+        _check(load_library().nqs_energy_stats_static(
             _dev(x, torch.complex64, "x"), _dev(weights, torch.float32, "weights") if weights is not None else None,
             x.shape[0], ctypes.c_void_p(stats.data_ptr()), _stream()))
     return stats

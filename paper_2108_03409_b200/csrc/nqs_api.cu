@@ -1239,6 +1239,68 @@ extern "C" int nqs_energy_stats(const nqs_c64* d_x, const float* d_weights, int6
     return launch_stats(D, d_x, d_weights, B, d_stats, (cudaStream_t)stream);
 }
 
+// ----------------------------------------------------------------------------------------
+// nqs_energy_stats_static (include/nqs.h): the same two kernels as nqs_energy_stats, launched in the same
+// geometry, for callers that must not allocate.  The per-block partial sums do not come from the library's pool
+// but from the fixed array below, which is part of the loaded module: every device that loads libnqs_b200.so
+// holds these 8 KB from module load to process exit, whether or not this entry point is ever called.
+//
+// In host code `g_stats_static_scratch` is only a handle for the runtime, NOT a device address: handing it to a
+// kernel would make the kernel read and write some unrelated location (or fault).  The address the kernels get is
+// the one cudaGetSymbolAddress reports for the device that is current, looked up once per device and kept in
+// g_stats_static_ptr.  This entry point deliberately stays clear of device_state() (which creates the pool and
+// allocates the status block) and of Scratch: it calls no cudaMalloc*, cudaFree* or pool routine.
+// ----------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_stats_static_scratch[4 * ST_BLOCKS];  // ST_BLOCKS records {sum w, sum w Re x, sum w Im x, sum w |x|^2}
+static double* g_stats_static_ptr[MAX_DEVICES] = {};  // device address of the array, per device ordinal (g_stats_static_mu)
+static std::mutex g_stats_static_mu;
+
+// Device address of the scratch array on the CURRENT device; the first call per device does the lookup.
+static int stats_static_scratch(double** out) {
+    int dev = 0;
+    NQS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) return fail(NQS_ERR_UNSUPPORTED, "device ordinal >= 64");
+    std::lock_guard<std::mutex> lk(g_stats_static_mu);
+    if (!g_stats_static_ptr[dev]) {
+        void* p = nullptr;
+        NQS_CUDA(cudaGetSymbolAddress(&p, g_stats_static_scratch));
+        if (!p) return fail(NQS_ERR_CUDA, "nqs_energy_stats_static: cudaGetSymbolAddress returned a null address");
+        g_stats_static_ptr[dev] = static_cast<double*>(p);
+    }
+    *out = g_stats_static_ptr[dev];
+    return NQS_OK;
+}
+
+extern "C" int nqs_energy_stats_static(const nqs_c64* d_x, const float* d_weights, int64_t B, double* d_stats,
+                                       void* stream) {
+    if (B < 0) return fail(NQS_ERR_INVALID_ARG, "nqs_energy_stats_static: B < 0");
+    if (B == 0) return NQS_OK;
+    if (!d_x || !d_stats) return fail(NQS_ERR_INVALID_ARG, "nqs_energy_stats_static: NULL pointer");
+    if (B > (int64_t)NQS_STATS_STATIC_MAX_B)
+        return fail(NQS_ERR_UNSUPPORTED,
+                    "nqs_energy_stats_static: B = " + std::to_string((long long)B) + " exceeds NQS_STATS_STATIC_MAX_B = " +
+                        std::to_string((long long)NQS_STATS_STATIC_MAX_B) +
+                        " (the limit of the fixed scratch array; use nqs_energy_stats for larger batches)");
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n == 0) {
+        cudaGetLastError();
+        return fail(NQS_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
+    }
+    double* partial = nullptr;
+    NQS_TRY(stats_static_scratch(&partial));
+    cudaStream_t st = (cudaStream_t)stream;
+    // one record per block, as in launch_stats; stats_partial_kernel writes all four sums of every record
+    // 0 .. nblk-1 and stats_final_kernel reads exactly those, so nothing left behind by an earlier call is ever
+    // read and nothing has to be cleared first
+    const int nblk = (int)((B + 255) / 256 < ST_BLOCKS ? (B + 255) / 256 : ST_BLOCKS);
+    stats_partial_kernel<<<nblk, 256, 0, st>>>((const float2*)d_x, d_weights, (long long)B, partial);
+    NQS_LAUNCHED();
+    stats_final_kernel<<<1, 32, 0, st>>>(partial, nblk, d_stats);
+    NQS_LAUNCHED();
+    return NQS_OK;
+}
+
 // F[k] = sum_b conj(O_k(s_b)) cb[b] for all K = N + M + M N parameters: the exact int8 contraction over the
 // samples of nqs_forces.cuh.  tp = tanh(theta) pair records, cb [B_pad] (0 for the padding samples).
 // spT_out != NULL: the transposed int8 spins it packs ([nIT][K16][128] uint4) are handed to `keeper`.
