@@ -35,8 +35,10 @@
  *   - The entry points that take a term list (nqs_local_energy, nqs_local_energy_host,
  *     nqs_enumerate_connected) compile and upload the Hamiltonian on a cache miss; that upload is a
  *     pageable-memory copy in stream order (the runtime may synchronise `stream` once for it, and a
- *     miss cannot be captured into a CUDA graph).  A cache hit costs a key comparison.  An evicted
- *     Hamiltonian is freed in stream order after its most recent use.
+ *     miss cannot be captured into a CUDA graph).  A cache hit costs a key comparison and makes `stream`
+ *     wait for the event that closed the upload (a no-op on the stream that uploaded).  An evicted
+ *     Hamiltonian is freed in stream order after its most recent use on every stream that used it (one
+ *     event per stream; an entry used from more than 16 streams is freed with a synchronising cudaFree).
  *   - *_host entry points take HOST buffers, copy them to the device, run the same kernels,
  *     copy the result back and synchronise before returning.
  *   - Return value: 0 (NQS_OK) or a negative NQS_ERR_* code; nqs_last_error() then returns a
@@ -165,8 +167,9 @@ int nqs_local_energy_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t 
  *                       3 = series only: the guard is evaluated and recorded but nothing is recomputed
  *   NQS_OPT_THETA_PATH  0 = automatic (int8 tcgen05 kernel for N <= 512, else FP32 SIMT)   1 = FP32 SIMT only
  *   NQS_OPT_SMALL_PATH  0 = automatic: below the series' size threshold, when columns x M x 16 bytes of tables and the
- *                       per-sample state of >= 16 samples fit in 200 KB of shared memory, ONE kernel does the whole call
- *                       (csrc/nqs_small.cuh; theta accumulated in float64)                 1 = never (multi-launch path)
+ *                       per-sample state of >= 4 samples fit in 200 KB of shared memory, ONE kernel does the whole call
+ *                       (csrc/nqs_small.cuh; theta summed in float32 from W split into two exact float32 levels, the
+ *                       log cosh terms accumulated in float64)                               1 = never (multi-launch path)
  *   NQS_OPT_THETA_SPLIT 0 = automatic: on the series path the hidden units of a sample tile are split over 1, 2, 4 or 8
  *                       CTAs of the theta kernel, whichever needs the fewest waves of the 2 x SMs CTA slots (partial
  *                       log psi / row norms combined in a fixed order: deterministic)         1 = never split

@@ -192,7 +192,14 @@ struct nqs_hamiltonian {
     int device = -1;       // -1: host-only compile
     void* d_blob = nullptr;
     bool pooled = false;   // blob came from the device pool (cache entries): freed in stream order
-    cudaEvent_t last_use = nullptr;
+    // cache entries are shared between streams: `uploaded` marks the end of the stream-ordered upload (a hit on
+    // another stream waits for it), `uses` holds one last-use event per stream that has read the blob (the free waits
+    // for all of them); beyond MAX_USE_STREAMS streams the free falls back to a synchronising cudaFree
+    static constexpr size_t MAX_USE_STREAMS = 16;
+    cudaEvent_t uploaded = nullptr;
+    mutable std::mutex use_mu;
+    mutable std::vector<std::pair<cudaStream_t, cudaEvent_t>> uses;
+    mutable bool uses_overflow = false;
     DevHam dev{};
     int C = 0;
     // launch plan (static for the handle): column tiling of the product-form a5 kernel ...
@@ -295,11 +302,12 @@ static int upload(nqs_hamiltonian* h, DeviceState* D, bool pooled, cudaStream_t 
         NQS_CUDA(cudaMallocFromPoolAsync(&h->d_blob, total, D->pool, st));
         h->pooled = true;
         NQS_CUDA(cudaMemcpyAsync(h->d_blob, blob.data(), total, cudaMemcpyHostToDevice, st));
+        NQS_CUDA(cudaEventCreateWithFlags(&h->uploaded, cudaEventDisableTiming));
+        NQS_CUDA(cudaEventRecord(h->uploaded, st));
     } else {
         NQS_CUDA(cudaMalloc(&h->d_blob, total));
         NQS_CUDA(cudaMemcpy(h->d_blob, blob.data(), total, cudaMemcpyHostToDevice));
     }
-    NQS_CUDA(cudaEventCreateWithFlags(&h->last_use, cudaEventDisableTiming));
     const int* di = reinterpret_cast<const int*>(h->d_blob);
     const float2* dc = reinterpret_cast<const float2*>(reinterpret_cast<const unsigned char*>(h->d_blob) + int_bytes);
     DevHam& Dv = h->dev;
@@ -336,18 +344,24 @@ static int upload(nqs_hamiltonian* h, DeviceState* D, bool pooled, cudaStream_t 
     return NQS_OK;
 }
 
-// frees a handle; pooled blobs are freed in stream order after the handle's most recent use
+// frees a handle; pooled blobs are freed in stream order after the most recent use on EVERY stream that read them
 static void destroy_handle(nqs_hamiltonian* h) {
     if (!h) return;
+    int cur = -1;
+    const bool switch_dev = h->device >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != h->device;
+    if (switch_dev) cudaSetDevice(h->device);  // an evicted entry may belong to another device than the caller's
     if (h->d_blob) {
-        if (h->pooled) {
-            if (h->last_use) cudaStreamWaitEvent(nullptr, h->last_use, 0);
+        if (h->pooled && !h->uses_overflow) {
+            if (h->uploaded) cudaStreamWaitEvent(nullptr, h->uploaded, 0);
+            for (auto& u : h->uses) cudaStreamWaitEvent(nullptr, u.second, 0);
             cudaFreeAsync(h->d_blob, nullptr);
         } else {
             cudaFree(h->d_blob);  // waits for the device: kernels still reading the blob finish first
         }
     }
-    if (h->last_use) cudaEventDestroy(h->last_use);
+    if (h->uploaded) cudaEventDestroy(h->uploaded);
+    for (auto& u : h->uses) cudaEventDestroy(u.second);
+    if (switch_dev) cudaSetDevice(cur);
     delete h;
 }
 
@@ -450,6 +464,9 @@ static int cached_hamiltonian(int32_t N, int32_t T, int32_t K, const int32_t* s,
         if (it->device == dev && it->N == N && it->T == T && it->K == K && it->key == key) {
             g_cache.splice(g_cache.begin(), g_cache, it);
             *out = g_cache.front().h;
+            // the blob was uploaded in the order of the stream that missed: any other stream waits for that copy
+            // (no cost when `st` is that stream or the copy has long finished)
+            if ((*out)->uploaded) NQS_CUDA(cudaStreamWaitEvent(st, (*out)->uploaded, 0));
             return NQS_OK;
         }
     nqs_hamiltonian* h = nullptr;
@@ -461,8 +478,24 @@ static int cached_hamiltonian(int32_t N, int32_t T, int32_t K, const int32_t* s,
     return NQS_OK;
 }
 
+// records that work reading the blob has been enqueued on `st` (one event per stream, re-recorded at every use)
 static void mark_use(const nqs_hamiltonian* h, cudaStream_t st) {
-    if (h->last_use) cudaEventRecord(h->last_use, st);
+    if (!h->pooled) return;  // user handles are freed with a synchronising cudaFree
+    std::lock_guard<std::mutex> lk(h->use_mu);
+    if (h->uses_overflow) return;
+    for (auto& u : h->uses)
+        if (u.first == st) {
+            cudaEventRecord(u.second, st);
+            return;
+        }
+    cudaEvent_t ev = nullptr;
+    if (h->uses.size() >= nqs_hamiltonian::MAX_USE_STREAMS ||
+        cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) {
+        h->uses_overflow = true;
+        return;
+    }
+    cudaEventRecord(ev, st);
+    h->uses.emplace_back(st, ev);
 }
 
 extern "C" int nqs_release(void) {

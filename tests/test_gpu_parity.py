@@ -372,6 +372,38 @@ def test_non_default_stream(nqs, oracle):
     check_eloc(e.cpu().numpy(), e_ref, "stream")
 
 
+def test_cached_hamiltonian_shared_between_streams(nqs, oracle):
+    """a term list compiled on a cache miss is uploaded in the order of the stream that missed.  A hit
+    from ANOTHER (non-blocking) stream must wait for that upload, and an eviction must wait for the readers on every
+    stream.  Miss on s1 behind a long-running kernel, immediate hit on s2, then nine other term lists push the entry
+    out while both streams still hold work."""
+    import torch
+
+    w = wl.make_config(3, B=4096)
+    coeffs = (w.ham.coeffs * np.complex64(1.25 - 0.5j)).astype(np.complex64)  # a term list no other test has cached
+    spins, a, b, W = to_dev(w)
+    small = wl.make_config(1)
+    sp1, a1, b1, W1 = to_dev(small)
+    nqs.release()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s1):
+        torch.cuda._sleep(400_000_000)  # ~0.2 s: the upload of the miss below is still pending when s2 hits
+        e1, l1 = nqs.local_energy(spins, a, b, W, w.ham.sites, w.ham.paulis, coeffs)
+    with torch.cuda.stream(s2):
+        e2, l2 = nqs.local_energy(spins, a, b, W, w.ham.sites, w.ham.paulis, coeffs)
+        for k in range(9):  # the cache holds eight entries
+            nqs.local_energy(sp1, a1, b1, W1, small.ham.sites, small.ham.paulis,
+                             (small.ham.coeffs * np.complex64(2.0 + k)).astype(np.complex64))
+    with torch.cuda.stream(s1):
+        e3, _ = nqs.local_energy(spins, a, b, W, w.ham.sites, w.ham.paulis, coeffs)  # a miss again: recompiled
+    torch.cuda.synchronize()
+    e_ref, l_ref = oracle.local_energy_fast(w.spins, w.a, w.b, w.W, w.ham.sites, w.ham.paulis, coeffs)
+    check_eloc(e1.cpu().numpy(), e_ref, "miss on s1")
+    check_logpsi(l1.cpu().numpy(), l_ref, "miss on s1")
+    assert torch.equal(e1, e2) and torch.equal(l1, l2) and torch.equal(e1, e3)
+
+
 def test_error_codes(nqs):
     import torch
 
