@@ -88,8 +88,10 @@ __global__ void __launch_bounds__(SM_MAX_THREADS) small_eloc_kernel(const SmallP
         float mx = 0.f;
         for (int i = l8; i < N; i += 8) mx = fmaxf(mx, fmaxf(fabsf(wrow[i].x), fabsf(wrow[i].y)));
         for (int o = 4; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o, 8));
+        // a row below 2^-100 keeps e = 0 like an all-zero row (Wh = 0, Wl = W: the sums of such values need no split);
+        // 2^(11 - e) would otherwise overflow to inf for max|W_j| < ~2^-116 and inf * 0 = NaN poison theta
         int e = 0;
-        if (mx > 0.f && mx < 3.0e38f) (void)frexpf(mx, &e);  // mx = f 2^e, f in [0.5, 1)
+        if (mx > 7.8e-31f && mx < 3.0e38f) (void)frexpf(mx, &e);  // mx = f 2^e, f in [0.5, 1)
         const float up = ldexpf(1.f, 11 - e), dn = ldexpf(1.f, e - 11);
         for (int i = l8; i < N && j < M; i += 8) {
             const float2 w = wrow[i];

@@ -111,6 +111,30 @@ def test_large_parameters_exponent_renormalisation(nqs, oracle):
     check_logpsi(l, l_ref, "sigma 0.5", rtol=1e-4)
 
 
+def test_hidden_unit_rows_of_vanishing_weight(nqs, oracle):
+    """the two-level split of W scales each row by 2^(11 - e), e the exponent of max|W_j|; for a row
+    with 0 < max|W_j| < ~2^-116 that scale overflowed to inf and inf * 0 made theta NaN.  Rows at 1e-36, in the
+    subnormal range and exactly zero, beside ordinary rows; the multi-launch path handles the same inputs."""
+    N, M, B = 16, 32, 200
+    a, b, W = wl.rbm_parameters(N, M, 0.05, [94, 0])
+    W = W.copy()
+    W[3] *= np.float32(1e-35)   # ~5e-37: normal float32, far below 2^-116
+    W[7] *= np.float32(1e-36)
+    W[7] *= np.float32(1e-6)    # ~5e-44: subnormal
+    W[11] = 0
+    assert 0 < np.abs(W[3]).max() < 2.0 ** -116 and 0 < np.abs(W[7]).max() < 1.2e-38
+    ham = wl.tfim(wl.chain_bonds(N), N, 1.0, 0.7)
+    w = wl.Workload("chain_N16_tiny_rows", N, M, B, wl.iid_spins(B, N, [94, 1]), a, b, W, ham)
+    e, l, took = run(nqs, w)
+    assert took["path"] == "small"
+    e_ref, l_ref = oracle_on(oracle, w, slice(None), "definition")
+    check_eloc(e, e_ref, "tiny rows")
+    check_logpsi(l, l_ref, "tiny rows")
+    e2, l2, took2 = run(nqs, w, small=False)
+    assert took2["path"] == "product"
+    check_eloc(e2, e_ref, "tiny rows, multi-launch")
+
+
 def test_selection_rule(nqs):
     """Tables that do not fit in shared memory (config-3 shapes: 100 x 400 x 16 bytes) and calls that keep tanh(theta)
     for the force vector take the multi-launch path; NQS_OPT_A5_PATH = 1 still means eloc_kernel."""
