@@ -325,7 +325,8 @@ int nqs_vmc_step_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t B, i
  * exp(2 theta), recomputed from the spins every two sweeps (2 N steps) and updated in place by one
  * complex multiplication per hidden unit on each accepted move.  Valid for |Re theta| < 22: beyond that
  * |exp(2 theta) + 1|^2 leaves the float32 range, the log-ratio becomes NaN and the chain stops accepting; such a
- * chain is REPORTED, not silently frozen: d_accepted[c] = -1 (its spins are then meaningless).  Sites outside
+ * chain is REPORTED, not silently frozen: d_accepted[c] = -1 (its spins are then meaningless).  A proposal with
+ * psi(s') = 0 exactly (log-ratio -inf) is an ordinary rejection, not an overflow.  Sites outside
  * [0,N) are undefined behaviour.  S = 0 is a no-op.  Asynchronous.
  * NQS_ERR_UNSUPPORTED if one chain's state (8 M + N bytes) does not fit shared memory twice.
  * ------------------------------------------------------------------------------------- */
@@ -344,7 +345,9 @@ int nqs_metropolis_trace(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const
  * single-spin-flip Metropolis chain of p(s) (its proposal sequence is a fixed, chain-independent schedule -- e.g. a
  * random permutation of the sites per sweep -- and its uniforms are its own).  The table rows exp(+-4W)[site] are
  * then fetched once per thread block and step instead of once per chain, and the chain state lives in registers:
- * several times the throughput of nqs_metropolis.  M <= 2048 (NQS_ERR_UNSUPPORTED above).  Same arithmetic,
+ * several times the throughput of nqs_metropolis.  M <= 2048, and the block's shared memory -- 128 + 64 M_pad +
+ * warps x N_pad + 12 N bytes, M_pad = M rounded up to 16 -- must fit 227 KB, i.e. N up to a few thousand sites
+ * (NQS_ERR_UNSUPPORTED otherwise; nqs_metropolis has no such bound on N).  Same arithmetic,
  * acceptance rule, float32 caveat and theta refresh (every 2 N steps) as nqs_metropolis. */
 int nqs_metropolis_shared(int8_t *d_spins, int64_t C, int32_t N, int32_t M, const nqs_c64 *d_a,
                           const nqs_c64 *d_b, const nqs_c64 *d_W, int32_t S, const int32_t *d_sites,

@@ -572,7 +572,7 @@ static int validate_spins(DeviceState* D, const int8_t* d_spins, int64_t B, int3
     NQS_TRY(S.get(&bad, 1));
     NQS_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), st));
     const long long total = (long long)B * N;
-    const unsigned grid = (unsigned)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
+    const unsigned grid = (unsigned)((total + 255) / 256 < D->sms * 8 ? (total + 255) / 256 : D->sms * 8);
     validate_spins_kernel<<<grid, 256, 0, st>>>(d_spins, total, bad);
     NQS_LAUNCHED();
     int h_bad = 0;
@@ -642,7 +642,7 @@ static int launch_theta_mma(DeviceState* D, const int8_t* d_spins, int64_t B, in
     NQS_TRY(S.get(&B_packed, (size_t)nNT * K16 * TH_N));
     NQS_TRY(S.get(&scale, (size_t)nNT * TH_JT));
     const long long a_items = nMT * K16 * TM_M;
-    const unsigned agrid = (unsigned)((a_items + 255) / 256 < 148 * 16 ? (a_items + 255) / 256 : 148 * 16);
+    const unsigned agrid = (unsigned)((a_items + 255) / 256 < D->sms * 16 ? (a_items + 255) / 256 : D->sms * 16);
     pack_spins_kernel<<<agrid, 256, 0, st>>>(d_spins, (long long)B, N, K16, nMT, A_packed, o.gate);
     NQS_LAUNCHED();
     pack_w_kernel<<<(unsigned)(nNT * TH_JT), 128, 0, st>>>((const float2*)d_W, N, M, K16, B_packed, scale, o.gate);
@@ -1351,9 +1351,9 @@ static int force_contract(DeviceState* D, const int8_t* d_spins, int64_t B, int3
     NQS_TRY(S.get(&B_packed, (size_t)nJT * K16 * TM_N));
     force_gscale_kernel<<<(unsigned)(nJT * TM_JT), 256, 0, st>>>(tp, nPairsPad, cb, M, gexp);
     NQS_LAUNCHED();
-    force_pack_g_kernel<<<148 * 8, 256, 0, st>>>(tp, nPairsPad, cb, M, K16, nJT, gexp, B_packed);
+    force_pack_g_kernel<<<(unsigned)D->sms * 8, 256, 0, st>>>(tp, nPairsPad, cb, M, K16, nJT, gexp, B_packed);
     NQS_LAUNCHED();
-    force_pack_spins_kernel<<<148 * 8, 256, 0, st>>>(d_spins, (long long)B, N, K16, nIT, A_packed);
+    force_pack_spins_kernel<<<(unsigned)D->sms * 8, 256, 0, st>>>(d_spins, (long long)B, N, K16, nIT, A_packed);
     NQS_LAUNCHED();
     NQS_TRY(ensure_smem(D, force_mma_kernel, FM_SMEM));
     ForceMmaParams p;
@@ -1455,7 +1455,7 @@ static int fisher_impl(const int8_t* d_spins, int64_t B, int32_t N, int32_t M, c
     float scale = ldexpf(4.f, e);
     if (scale > 16384.f) scale = 16384.f;
     const long long nB8 = B_pad / 8;
-    fisher_pack_kernel<<<148 * 16, 256, 0, st>>>(tp, nPairsPad, spT, K16, sw, Fc, N, M, (int)K, nKT, nB8, scale, X);
+    fisher_pack_kernel<<<(unsigned)D->sms * 16, 256, 0, st>>>(tp, nPairsPad, spT, K16, sw, Fc, N, M, (int)K, nKT, nB8, scale, X);
     NQS_LAUNCHED();
     NQS_TRY(ensure_smem(D, fisher_gemm_kernel, FS_SMEM));
     FisherGemmParams p;
@@ -1620,6 +1620,16 @@ extern "C" int nqs_metropolis_shared(int8_t* d_spins, int64_t C, int32_t N, int3
     const int ppl_need = (M_pad / 2 + 31) / 32;
     if (ppl_need > 32)
         return fail(NQS_ERR_UNSUPPORTED, "nqs_metropolis_shared: M > 2048 (the chain state lives in registers)");
+    {   // the ring of table rows, the chains' spins and the per-site data must fit the 227 KB a CTA may opt into
+        const int warps = ppl_need <= 1 ? MetroSharedCfg<1>::WARPS : ppl_need <= 2 ? MetroSharedCfg<2>::WARPS
+                        : ppl_need <= 4 ? MetroSharedCfg<4>::WARPS : ppl_need <= 8 ? MetroSharedCfg<8>::WARPS
+                        : ppl_need <= 13 ? MetroSharedCfg<13>::WARPS : ppl_need <= 16 ? MetroSharedCfg<16>::WARPS
+                        : ppl_need <= 25 ? MetroSharedCfg<25>::WARPS : MetroSharedCfg<32>::WARPS;
+        const size_t need = metropolis_shared_smem_bytes(warps, N, M_pad);
+        if (need > 227 * 1024)
+            return fail(NQS_ERR_UNSUPPORTED, "nqs_metropolis_shared: N = " + std::to_string(N) + ", M = " + std::to_string(M) +
+                                                 " need " + std::to_string(need) + " bytes of shared memory per block (limit 232448); use nqs_metropolis");
+    }
     const long long C_pad = round_up(C, 256);
     const long long nPairsPad = C_pad / 2;
     Scratch Sc(D, st);

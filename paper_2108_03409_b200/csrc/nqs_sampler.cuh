@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(CPB * 32, 1) metropolis_kernel(const MetroPara
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) lg += __shfl_xor_sync(0xffffffffu, lg, o);
         const float lk = p.lk2[site];
-        bad |= !(fabsf(lg) <= 3.0e38f);  // NaN / inf: a hidden unit left the float32 range of exp(2 theta)
+        bad |= !(lg <= 3.0e38f);  // NaN / +inf: a hidden unit left the float32 range of exp(2 theta); -inf is psi(s') = 0, a plain rejection
         const bool accept = log2f(ul) < (sgi > 0 ? lk : -lk) + lg;  // u == 0: -inf, always accepted
         if (lane == 0 && p.decisions) p.decisions[(long long)step * p.C + c] = accept ? 1 : 0;
         if (accept) {
@@ -341,7 +341,7 @@ __global__ void __launch_bounds__(MetroSharedCfg<PPL>::NT, 1) metropolis_shared_
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) lg += __shfl_xor_sync(0xffffffffu, lg, o);
         const float lk = lk_s[site];
-        bad |= !(fabsf(lg) <= 3.0e38f);  // NaN / inf: a hidden unit left the float32 range of exp(2 theta)
+        bad |= !(lg <= 3.0e38f);  // NaN / +inf: a hidden unit left the float32 range of exp(2 theta); -inf is psi(s') = 0, a plain rejection
         const bool accept = live_chain && (log2f(ul) < (sgi > 0 ? lk : -lk) + lg);  // u == 0: -inf, always accepted
         if (lane == 0 && live_chain && p.decisions) p.decisions[(long long)step * p.C + c] = accept ? 1 : 0;
         if (accept) {

@@ -267,3 +267,32 @@ def test_saturated_chain_is_reported_not_frozen(nqs):
     # kernels.)  With the original small parameters nothing is flagged:
     acc_ok = nqs.metropolis_shared(t(spins), t(w.a), t(w.b), t(w.W), t(sites1), t(u)).cpu().numpy()
     assert np.all(acc_ok >= 0)
+
+
+def test_shared_site_kernel_refuses_shapes_beyond_its_shared_memory(nqs):
+    """ADVICE round 2: the shared-site kernel keeps every site's table offsets and each chain's spins in shared memory;
+    a lattice too large for the 227 KB of a block must come back as NQS_ERR_UNSUPPORTED (as include/nqs.h documents)
+    before anything is launched -- not as a CUDA error from the launch.  nqs_metropolis takes the same shape."""
+    import torch
+
+    N, M, C, S = 12000, 16, 4, 3
+    rng = np.random.default_rng(77)
+    d = torch.device("cuda:0")
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x)).to(d)  # noqa: E731
+    spins0 = np.where(rng.random((C, N)) < 0.5, 1, -1).astype(np.int8)
+    a = (1e-3 * (rng.standard_normal(N) + 1j * rng.standard_normal(N))).astype(np.complex64)
+    b = (1e-3 * (rng.standard_normal(M) + 1j * rng.standard_normal(M))).astype(np.complex64)
+    W = (1e-3 * (rng.standard_normal((M, N)) + 1j * rng.standard_normal((M, N)))).astype(np.complex64)
+    sites1 = rng.integers(0, N, S).astype(np.int32)
+    u = rng.random((S, C), dtype=np.float32)
+    spins = t(spins0)
+    n0 = nqs.launch_count()
+    with pytest.raises(nqs.NqsError) as err:
+        nqs.metropolis_shared(spins, t(a), t(b), t(W), t(sites1), t(u))
+    assert err.value.code == -4 and "shared memory" in str(err.value), err.value
+    assert nqs.launch_count() == n0
+    torch.cuda.synchronize()
+    assert np.array_equal(spins.cpu().numpy(), spins0)
+    sites = np.ascontiguousarray(np.broadcast_to(sites1[:, None], (S, C)))
+    acc = nqs.metropolis(spins, t(a), t(b), t(W), t(sites), t(u)).cpu().numpy()
+    assert np.all((acc >= 0) & (acc <= S))
