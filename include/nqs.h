@@ -180,11 +180,21 @@ int nqs_local_energy_h(const nqs_hamiltonian *h, const int8_t *d_spins, int64_t 
  *   NQS_OPT_HOST_CHUNKS 0 = automatic: nqs_local_energy_host sends the batch through the device in chunks of 2 x SMs x 128
  *                       samples (whole waves of the kernels; at most 16 chunks, a short remainder joins the last),
  *                       copying chunk k + 1 while the kernels of chunk k run      1 .. 16 = that many equal chunks
+ *   NQS_OPT_SERIES_LATCH 0 = automatic: with NQS_OPT_A5_PATH = 0 a Hamiltonian handle (or cached term list) remembers that
+ *                       the guard refused its last series attempt: the result of every attempt lands in pinned host
+ *                       memory and is read at the next call WITHOUT synchronising (so it may lag by the calls still in
+ *                       flight).  After a refusal the next 8 calls with that handle run the product form alone -- no
+ *                       series operands, GEMM or guard are enqueued -- then one call probes the series again; the skip
+ *                       doubles up to 64 calls while the probes keep failing and returns to 8 once one passes.  The
+ *                       latch is per handle, not per parameter set: calls that alternate between parameters inside and
+ *                       outside the guard's window on ONE handle run mostly on the product form (slower, never less
+ *                       accurate).                                                           1 = no latch: every large
+ *                       call attempts the series (round-2 behaviour)
  * nqs_debug_last_a5 (synchronises `stream`; tests only; not meaningful while calls run concurrently on other
  * streams): out[0] = 1 if the most recent nqs_local_energy* call on this device attempted the series path, 2 if
  * it used the product form only, 3 if the single-launch kernel for small problems ran; out[1] = 1 if the guard failed; out[2] = samples over the guard threshold.
  * ------------------------------------------------------------------------------------- */
-enum { NQS_OPT_A5_PATH = 0, NQS_OPT_THETA_PATH = 1, NQS_OPT_HOST_CHUNKS = 2, NQS_OPT_SMALL_PATH = 3, NQS_OPT_THETA_SPLIT = 4, NQS_OPT_SERIES_WIDE = 5, NQS_OPT_COUNT = 6 };
+enum { NQS_OPT_A5_PATH = 0, NQS_OPT_THETA_PATH = 1, NQS_OPT_HOST_CHUNKS = 2, NQS_OPT_SMALL_PATH = 3, NQS_OPT_THETA_SPLIT = 4, NQS_OPT_SERIES_WIDE = 5, NQS_OPT_SERIES_LATCH = 6, NQS_OPT_COUNT = 7 };
 int nqs_set_option(int32_t key, int32_t value);
 int nqs_get_option(int32_t key, int32_t *value);
 int nqs_debug_last_a5(int32_t out[3], void *stream);

@@ -110,7 +110,8 @@ def profile_last() -> dict:
     return {k: ms[i] for i, k in enumerate(PROFILE_SEGMENTS)}
 
 
-OPTIONS = {"a5_path": 0, "theta_path": 1, "host_chunks": 2, "small_path": 3, "theta_split": 4, "series_wide": 5}
+OPTIONS = {"a5_path": 0, "theta_path": 1, "host_chunks": 2, "small_path": 3, "theta_split": 4, "series_wide": 5,
+           "series_latch": 6}
 A5_PATHS = {"auto": 0, "product": 1, "series_guarded": 2, "series_only": 3}
 
 

@@ -106,7 +106,17 @@ struct DeviceState {
     cudaStream_t host_copy = nullptr, host_comp = nullptr;
     cudaEvent_t host_ev[HOST_MAX_CHUNKS + 1] = {};
     std::mutex host_mu;
+    // refusal latches of the automatic a5 path: LATCH_SLOTS records of four ints in pinned, device-mapped host memory,
+    // one per live handle, written by series_latch_kernel and read by the host without synchronising; never freed
+    // (a kernel of a handle that has since been destroyed may still write its slot: sequence numbers tell the
+    // records of the slot's next owner from it)
+    int* latch_host = nullptr;
+    int* latch_dev = nullptr;
+    std::vector<int> latch_free;
 };
+constexpr int LATCH_SLOTS = 64;
+constexpr int LATCH_SKIP0 = 8, LATCH_SKIP_MAX = 64;  // product-form calls after a refusal before the series is probed again
+static std::atomic<int> g_latch_seq{0};
 static DeviceState g_dev[MAX_DEVICES];
 static std::mutex g_dev_mu;
 
@@ -135,6 +145,10 @@ static int device_state(DeviceState** out) {
         const int init[8] = {0, 0, 0, 0, 0, 1, 2, 3};
         NQS_CUDA(cudaMemcpy(D.status, init, sizeof(init), cudaMemcpyHostToDevice));
         D.tags = D.status + 4;
+        NQS_CUDA(cudaHostAlloc((void**)&D.latch_host, LATCH_SLOTS * 4 * sizeof(int), cudaHostAllocMapped));
+        memset(D.latch_host, 0, LATCH_SLOTS * 4 * sizeof(int));
+        NQS_CUDA(cudaHostGetDevicePointer((void**)&D.latch_dev, D.latch_host, 0));
+        for (int k = LATCH_SLOTS - 1; k >= 0; --k) D.latch_free.push_back(k);
         NQS_CUDA(cudaDeviceGetAttribute(&D.sms, cudaDevAttrMultiProcessorCount, dev));
         D.ready = true;
     }
@@ -200,6 +214,11 @@ struct nqs_hamiltonian {
     mutable std::mutex use_mu;
     mutable std::vector<std::pair<cudaStream_t, cudaEvent_t>> uses;
     mutable bool uses_overflow = false;
+    // refusal latch (automatic a5 path): after a call whose series was refused by the guard, the next `skip_left`
+    // calls with this handle go straight to the product form, then the series is probed again; the skip length
+    // doubles from LATCH_SKIP0 to LATCH_SKIP_MAX while the probes keep failing and resets when one passes
+    int latch_slot = -1;  // record in DeviceState::latch_host, -1: none (no latch)
+    mutable int seq_first = 0, seq_last = 0, seq_seen = 0, skip_left = 0, skip_len = 8;
     DevHam dev{};
     int C = 0;
     // launch plan (static for the handle): column tiling of the product-form a5 kernel ...
@@ -297,6 +316,13 @@ static int upload(nqs_hamiltonian* h, DeviceState* D, bool pooled, cudaStream_t 
     if (!ints.empty()) memcpy(blob.data(), ints.data(), ints.size() * sizeof(int));
     if (!cs.empty()) memcpy(blob.data() + int_bytes, cs.data(), cs.size() * sizeof(nqs_c64));
     NQS_CUDA(cudaGetDevice(&h->device));
+    {
+        std::lock_guard<std::mutex> lk(g_dev_mu);
+        if (!D->latch_free.empty()) {
+            h->latch_slot = D->latch_free.back();
+            D->latch_free.pop_back();
+        }
+    }
     if (pooled) {
         // pageable source: the runtime stages the bytes before cudaMemcpyAsync returns, so `blob` may die
         NQS_CUDA(cudaMallocFromPoolAsync(&h->d_blob, total, D->pool, st));
@@ -361,6 +387,10 @@ static void destroy_handle(nqs_hamiltonian* h) {
     }
     if (h->uploaded) cudaEventDestroy(h->uploaded);
     for (auto& u : h->uses) cudaEventDestroy(u.second);
+    if (h->latch_slot >= 0 && h->device >= 0 && h->device < MAX_DEVICES) {
+        std::lock_guard<std::mutex> lk(g_dev_mu);
+        g_dev[h->device].latch_free.insert(g_dev[h->device].latch_free.begin(), h->latch_slot);  // reused last
+    }
     if (switch_dev) cudaSetDevice(cur);
     delete h;
 }
@@ -763,7 +793,7 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     const int opt = g_opt[NQS_OPT_A5_PATH].load();
     const bool series_ok = have_cols && N <= SR_MAX_N && series_gemm_smem_bytes(h->NB, N) <= 227 * 1024;
     const bool big = (double)B * h->C * M >= 268435456.0;  // 2^28 (sample, column, hidden unit) triples
-    const bool use_series = series_ok && (opt == 2 || opt == 3 || (opt == 0 && big));
+    bool use_series = series_ok && (opt == 2 || opt == 3 || (opt == 0 && big));  // the refusal latch below may clear it
     const bool use_product = have_cols && !(use_series && opt == 3);
 
     // small problems: a1 .. a6 in one launch (nqs_small.cuh) when the tables of a CTA fit in shared memory
@@ -805,6 +835,39 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
             g_prof_valid = g_prof_on;
             mark_use(h, st);
             return NQS_OK;
+        }
+    }
+
+    // refusal latch (automatic mode only): what the most recent finished series attempt of this handle reported is
+    // read from pinned memory -- no synchronisation, so it may lag by the calls still in flight.  A refusal sends the
+    // next skip_len calls to the product form alone (no series operands, no GEMM, no guard); then one call probes again.
+    int latch_seq = 0;
+    volatile int* latch_rec = nullptr;
+    if (opt == 0 && use_series && h->latch_slot >= 0 && g_opt[NQS_OPT_SERIES_LATCH].load() == 0) {
+        std::lock_guard<std::mutex> lk(h->use_mu);
+        volatile int* L = D->latch_host + 4 * h->latch_slot;
+        const int seq = L[0];
+        const int flag = L[1];
+        const bool own = h->seq_first != 0 && (unsigned)(seq - h->seq_first) <= (unsigned)(h->seq_last - h->seq_first);
+        if (own && seq != h->seq_seen) {
+            h->seq_seen = seq;
+            if (flag) {
+                h->skip_left = h->skip_len;
+                h->skip_len = h->skip_len * 2 < LATCH_SKIP_MAX ? h->skip_len * 2 : LATCH_SKIP_MAX;
+            } else {
+                h->skip_left = 0;
+                h->skip_len = LATCH_SKIP0;
+            }
+        }
+        if (h->skip_left > 0) {
+            --h->skip_left;
+            use_series = false;
+        } else {
+            latch_seq = g_latch_seq.fetch_add(1) + 1;
+            if (latch_seq == 0) latch_seq = g_latch_seq.fetch_add(1) + 1;  // 0 means "none"
+            if (!h->seq_first) h->seq_first = latch_seq;
+            h->seq_last = latch_seq;
+            latch_rec = D->latch_dev + 4 * h->latch_slot;
         }
     }
 
@@ -950,8 +1013,8 @@ static int local_energy_impl(const nqs_hamiltonian* h, const int8_t* d_spins, in
     // debug record of the decision (nqs_debug_last_a5): {guard flag, failed samples} of this call, path tag.
     // Product-only calls rewrite it only when the previous call on this device was not one of them.
     if (use_series) {
-        NQS_CUDA(cudaMemcpyAsync(D->status, status, 2 * sizeof(int), cudaMemcpyDeviceToDevice, st));
-        NQS_CUDA(cudaMemcpyAsync(D->status + 2, D->tags + 1, sizeof(int), cudaMemcpyDeviceToDevice, st));
+        series_latch_kernel<<<1, 32, 0, st>>>(status, D->status, latch_rec, latch_seq);
+        NQS_LAUNCHED();
         D->last_tag.store(1);
     } else if (D->last_tag.exchange(2) != 2) {
         NQS_CUDA(cudaMemsetAsync(D->status, 0, 2 * sizeof(int), st));

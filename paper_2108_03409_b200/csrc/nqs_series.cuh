@@ -795,4 +795,23 @@ __global__ void series_guard_kernel(const float4* __restrict__ partial, long lon
     }
 }
 
+// End of a series call: the debug record of the device ({guard flag, samples over, path tag 1}, nqs_debug_last_a5) and,
+// for calls in automatic mode, the refusal latch of the handle: a record in pinned host memory the NEXT call reads
+// without synchronising -- {sequence number of this call, guard flag, samples over}; the sequence number is written
+// last, behind a system-wide fence, so a reader that sees it sees the flag of the same call.
+__global__ void series_latch_kernel(const int* __restrict__ status, int* __restrict__ dstatus, volatile int* latch,
+                                    int seq) {
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    const int flag = status[0], over = status[1];
+    dstatus[0] = flag;
+    dstatus[1] = over;
+    dstatus[2] = 1;
+    if (latch) {
+        latch[1] = flag;
+        latch[2] = over;
+        __threadfence_system();
+        latch[0] = seq;
+    }
+}
+
 }  // namespace nqs

@@ -229,3 +229,56 @@ def test_wide_column_tiles(nqs, oracle):
         assert np.array_equal(out[0][0], out[0][1]), "run-to-run determinism"
         scale = np.abs(e_ref).max()
         assert np.abs(out[1][0] - out[0][0]).max() <= 4e-6 * scale, (k, B, np.abs(out[1][0] - out[0][0]).max(), scale)
+
+
+def test_refusal_latch_skips_the_series_after_a_refused_call(nqs, oracle):
+    """ADVICE / VERDICT round 2: in automatic mode a handle remembers that the guard refused its series.  Config-3 shapes
+    at trained-scale parameters (sigma = 0.05, far outside the guard's window), B large enough for the automatic path to
+    choose the series: call 1 attempts it and is refused; the next 8 calls enqueue the product form alone; call 10
+    probes again, is refused again, and 16 product-only calls follow.  Every call returns the product-form bits.  A
+    fresh handle with in-window parameters is untouched, and NQS_OPT_SERIES_LATCH = 1 restores an attempt per call."""
+    import torch
+
+    from test_gpu_parity import to_dev
+
+    w = wl.make_config(3, B=8192, sigma=0.05, seed=77)
+    spins, a, b, W = to_dev(w)
+    e_prod, _, took = run(nqs, w, "product")
+    assert took["path"] == "product"
+    ham = nqs.Hamiltonian(w.N, w.ham.sites, w.ham.paulis, w.ham.coeffs)  # a fresh handle: a fresh latch
+    paths, launches = [], []
+    for call in range(27):
+        n0 = nqs.launch_count()
+        e, _ = ham.local_energy(spins, a, b, W)
+        launches.append(nqs.launch_count() - n0)
+        took = nqs.debug_last_a5()  # synchronises: the latch record of this call has landed
+        paths.append(took["path"] + ("!" if took["guard_failed"] else ""))
+        assert np.array_equal(e.cpu().numpy(), e_prod), f"call {call}"
+    assert paths == ["series!"] + ["product"] * 8 + ["series!"] + ["product"] * 16 + ["series!"], paths
+    assert max(launches[1:9]) < launches[0] and len(set(launches[1:9])) == 1, launches
+    # without the latch every call attempts the series
+    nqs.set_option("series_latch", 1)
+    try:
+        for _ in range(3):
+            ham.local_energy(spins, a, b, W)
+            took = nqs.debug_last_a5()
+            assert took["path"] == "series" and took["guard_failed"], took
+    finally:
+        nqs.set_option("series_latch", 0)
+    # the latch belongs to the handle: still refusing here ...
+    ham.local_energy(spins, a, b, W)
+    assert nqs.debug_last_a5()["path"] == "product"
+    ham.close()
+    # ... while another handle, with parameters inside the window, takes the series at once and keeps taking it
+    w_ok = wl.make_config(3, B=8192)
+    ham2 = nqs.Hamiltonian(w_ok.N, w_ok.ham.sites, w_ok.ham.paulis, w_ok.ham.coeffs)
+    s2, a2, b2, W2 = to_dev(w_ok)
+    for _ in range(3):
+        e2, _ = ham2.local_energy(s2, a2, b2, W2)
+        took = nqs.debug_last_a5()
+        assert took["path"] == "series" and not took["guard_failed"], took
+    ham2.close()
+    idx = np.arange(0, w_ok.B, 64)
+    e_ref, _ = oracle_on(oracle, w_ok, idx, "fast")
+    check_eloc(e2.cpu().numpy()[idx], e_ref, "in-window handle")
+    torch.cuda.synchronize()
