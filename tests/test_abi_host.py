@@ -186,3 +186,19 @@ def test_k_site_strings_invalid_and_unsupported(nqs):
         nqs.hamiltonian_info_host(12, np.arange(9, dtype=np.int32)[None, :], np.full((1, 9), 3, np.uint8),
                                   np.ones(1, np.complex64))
     assert ei.value.code == -1
+
+
+@pytest.mark.parametrize("N,T,K,seed", [(8, 50, 6, 17), (9, 40, 8, 18), (8, 60, 8, 21)])
+def test_flip_sets_beyond_four_sites_are_refused_not_miscompiled(nqs, N, T, K, seed):
+    """The term lists on which tests/test_oracle_pins.py pins the oracle beyond the kernels' limit (flip sets of five to
+    eight sites): the host compiler must answer NQS_ERR_UNSUPPORTED for them -- and accept the same lists once the
+    strings with more than four X / Y factors are taken out."""
+    ham = wl.random_strings(N, T, K, np.random.default_rng([seed, 3]), max_flips=K)
+    n_flips = ((ham.paulis == wl.PAULI_X) | (ham.paulis == wl.PAULI_Y)).sum(axis=1)
+    assert n_flips.max() > 4
+    with pytest.raises(nqs.NqsError) as ei:
+        nqs.hamiltonian_info_host(N, ham.sites, ham.paulis, ham.coeffs)
+    assert ei.value.code == -4
+    keep = n_flips <= 4
+    info = nqs.hamiltonian_info_host(N, ham.sites[keep], ham.paulis[keep], ham.coeffs[keep])
+    assert info["G"] >= 1

@@ -53,16 +53,21 @@ def test_p1_bruteforce_random_terms(oracle, N, M, T, sigma, seed):
         _assert_logpsi(lp, psi, 1e-11, f"log psi {fn.__name__}")
 
 
-@pytest.mark.parametrize("N,M,T,K,sigma,seed", [(5, 4, 30, 3, 0.3, 15), (7, 6, 40, 4, 0.25, 16), (8, 5, 50, 6, 0.2, 17),
-                                                 (9, 7, 25, 8, 0.15, 18)])
-def test_p1_bruteforce_k_site_pauli_strings(oracle, N, M, T, K, sigma, seed):
+@pytest.mark.parametrize("N,M,T,K,sigma,seed,max_flips", [
+    (5, 4, 30, 3, 0.3, 15, 4), (7, 6, 40, 4, 0.25, 16, 4), (8, 5, 50, 6, 0.2, 17, 4), (9, 7, 25, 8, 0.15, 18, 4),
+    # flip sets of up to K sites: beyond what the CUDA path accepts (four), so that the oracle is already pinned there
+    (8, 5, 50, 6, 0.2, 17, 6), (9, 7, 40, 8, 0.15, 18, 8), (8, 4, 60, 8, 0.2, 21, 8)])
+def test_p1_bruteforce_k_site_pauli_strings(oracle, N, M, T, K, sigma, seed, max_flips):
     """k-site Pauli strings ("tensor products of branch-free operators"): term
-    arrays [T,K] with up to K operators per term, up to four of them flipping, against the dense Kronecker-product H
-    (which knows no flip / sign rule).  Several Y factors in one string pin the (-i)^n phase; strings with the same
-    flip set pin the grouping of fast mode."""
+    arrays [T,K] with up to K operators per term, up to `max_flips` of them flipping, against the dense Kronecker-product
+    H (which knows no flip / sign rule).  Several Y factors in one string pin the (-i)^n phase; strings with the same
+    flip set pin the grouping of fast mode.  The generator's limit on flipping factors is lifted to K in the last
+    cases (a shared generator must not be shaped by the kernel's limits)."""
     w = wl.make_random(N, M, 1 << N, 4, sigma, seed)
-    ham = wl.random_strings(N, T, K, np.random.default_rng([seed, 3]))
+    ham = wl.random_strings(N, T, K, np.random.default_rng([seed, 3]), max_flips=max_flips)
     assert ham.sites.shape == (T, K)
+    n_flips = ((ham.paulis == 1) | (ham.paulis == 2)).sum(axis=1)
+    assert n_flips.max() <= max_flips and (max_flips <= 4 or n_flips.max() > 4), n_flips.max()
     e_ref, psi, H = local_energy_all(N, w.a, w.b, w.W, ham.sites, ham.paulis, ham.coeffs)
     assert np.abs(H).max() > 0
     for fn in (oracle.local_energy_definition, oracle.local_energy_fast):
