@@ -341,7 +341,10 @@ def run_ours(args) -> None:
                                    "kind::f16 rate); algorithmic work = 20 real FP16 MACs per (sample, column, hidden "
                                    "unit), padding columns not counted",
                     "frac_of_sustained_peak": (achieved / peaks["bf16_tflops_sustained"]
-                                               if peaks["bf16_tflops_sustained"] else None)}
+                                               if peaks["bf16_tflops_sustained"] else None),
+                    # SURVEY 8(f)4 counts the series as K = 3 complex GEMMs = 12 real MACs per triple; the other 8 of
+                    # the 20 are the hi + lo split that FP16 operands need for the k = 1 term
+                    "frac_12mac": achieved / peaks["bf16_tflops"] * 12.0 / 20.0}
         else:
             dom, dom_ms = ("small_eloc_kernel" if took["path"] == "small" else "eloc_kernel"), km["eloc"]
             achieved = 2.0 * work["a5_fp32"] / (dom_ms * 1e-3) / 1e12
@@ -435,6 +438,49 @@ def run_ours(args) -> None:
         line["vmc_step"] = {"ms_per_call": v_ms, "samples_per_s": w.B / (v_ms * 1e-3),
                             "what": "nqs_local_energy_forces_h: E_loc, mean/variance and force vector of one batch, "
                                     "theta and tanh(theta) computed once; median of 5, L2 flushed"}
+        # trained-scale parameters (10 x the configuration's sigma: far outside the series guard's window), automatic
+        # path, a fresh handle: the first call attempts the series and is refused; the refusal latch then sends the
+        # following calls to the product form alone and probes the series again after 8, 16, ... calls
+        if series:
+            sig_t = 10.0 * w.meta["sigma"]
+            ta, tb, tW = (torch.from_numpy(x).to(dev) for x in wl.rbm_parameters(w.N, w.M, sig_t, [w.meta["seed"], 9]))
+            ham_t = nqs.Hamiltonian(w.N, w.ham.sites, w.ham.paulis, w.ham.coeffs)
+            n_t = 20
+            t_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_t)]
+            t_paths = []
+            for k in range(n_t):
+                flush.fill_(k)
+                t_ev[k][0].record()
+                ham_t.local_energy(spins, ta, tb, tW)
+                t_ev[k][1].record()
+                tk = nqs.debug_last_a5()  # synchronises, as a VMC loop does when it reads the energies
+                t_paths.append("series refused" if tk["path"] == "series" and tk["guard_failed"] else tk["path"])
+            t_ms = [s0.elapsed_time(s1) for s0, s1 in t_ev]
+            # the forced product form at the SAME parameters (larger theta: the closed-form log cosh / tanh branch)
+            nqs.set_option("a5_path", nqs.A5_PATHS["product"])
+            try:
+                tp_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+                for k in range(7):
+                    if k >= 2:
+                        flush.fill_(k)
+                        tp_ev[k - 2][0].record()
+                    ham_t.local_energy(spins, ta, tb, tW)
+                    if k >= 2:
+                        tp_ev[k - 2][1].record()
+                torch.cuda.synchronize()
+            finally:
+                nqs.set_option("a5_path", 0)
+            tp_ms = float(np.median([s0.elapsed_time(s1) for s0, s1 in tp_ev]))
+            ham_t.close()
+            line["trained_scale"] = {
+                "sigma": sig_t, "first_call_ms": t_ms[0], "refused_call_ms": float(np.mean(t_ms[1:])),
+                "median_call_ms": float(np.median(t_ms[1:])), "calls": n_t,
+                "series_attempts": int(sum(p_ != "product" for p_ in t_paths)),
+                "product_form_ms": tp_ms, "paths": t_paths,
+                "what": "same batch and Hamiltonian, parameters ~ N(0, sigma^2) at 10 x the configuration's sigma, automatic "
+                        "a5 path on a fresh handle; refused_call_ms = mean over calls 2..20 (includes the latch's re-probe "
+                        "after 8 product-form calls), median_call_ms = their median; product_form_ms = the forced product "
+                        "form at the same parameters (median of 5)"}
         # SURVEY.md 8(f) items 1 + 3: the quantum Fisher matrix S = <<O* O>>_c of the same batch (K <= 8192 parameters)
         K = w.N + w.M + w.M * w.N
         if K <= 8192:
