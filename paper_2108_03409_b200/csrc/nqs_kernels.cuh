@@ -333,7 +333,7 @@ __global__ void __launch_bounds__(WC * WS * 32, (WC * WS <= 10) ? 2 : 1) eloc_ke
         }
         mbar_wait(&mbar[s], (chunk >> 1) & 1);
 
-#pragma unroll 4
+#pragma unroll
         for (int jj = 0; jj < KJ; ++jj) {
             const float4 e = tabs[jj * TC + wc * 16 + lc];  // Cr Ci Sr Si
             const float4* const rrow = rec + jj * 4 * RSTR;
