@@ -14,10 +14,13 @@
 //
 // Both operands are pre-packed in global memory in exactly the shared-memory image the MMA wants
 // ([k16][row][16 bytes]), so every pipeline stage is ONE contiguous cp.async.bulk (TMA engine).
-// CTA = 128 samples, loops over all hidden tiles so log psi needs no cross-CTA reduction.
-// Warp roles: 0 = bulk-copy producer, 1 = TMEM allocator + MMA issuer (one elected lane),
-// 2..9 = epilogue (tcgen05.ld -> theta -> log cosh, tanh -> log psi, tp).  Two CTAs per SM share
-// the 512 TMEM columns, so one CTA's MMAs overlap the other's epilogue.
+// CTA = 128 samples (TM_THREADS = 320: warp 0 = bulk-copy producer, warp 1 = TMEM allocator + MMA issuer with one
+// elected lane, warps 2..9 = epilogue: tcgen05.ld -> theta -> log cosh, tanh -> log psi, tp / series planes).  A CTA
+// loops over its hidden tiles of TH_JT = 16 units (the constants further down; TM_JT = 32 below is the tile of the
+// force / Fisher kernels that share this file's operand layout) with two accumulator sets in TMEM, so the MMAs of the
+// next tile overlap the epilogue of the current one; two CTAs per SM share the 512 TMEM columns.  On the series path
+// the hidden tiles of a sample tile may be split over 1, 2, 4 or 8 CTAs (NQS_OPT_THETA_SPLIT): log psi and the row norms
+// are then partial sums combined in a fixed order by series_guard_kernel / series_gemm_kernel.
 #pragma once
 #include <cuda_fp16.h>
 
